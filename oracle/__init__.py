@@ -1,0 +1,202 @@
+"""ORACLE -- TEST INFRASTRUCTURE ONLY (see aa_oracle.c for the full header).
+
+Python face of the plain-C oracle: builds `libaa_oracle.so` with gcc and exposes
+the whole-observation computation of SURVEY.md §8(c) steps 1-8.  Only `tests/`,
+`__graft_entry__.smoke()` and `bench.py`'s cpu_baseline / `--impl reference`
+legs may import this package.  It imports nothing from the CUDA path; a
+workload is any object with the attributes
+``nchans nsamp tsamp f_top foff ranges(dm_low, dm_step, ndms, bin) widths
+snr_threshold norm_block``.
+"""
+from __future__ import annotations
+
+import ctypes
+import math
+import os
+import subprocess
+from concurrent.futures import ThreadPoolExecutor
+from typing import Dict, Iterable, List, Optional, Sequence, Tuple
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_LIB_PATH = os.path.join(_HERE, "libaa_oracle.so")
+_lib = None
+
+CAND_DTYPE = np.dtype([("dm_index", np.uint32), ("t_start", np.uint32),
+                       ("width", np.uint32), ("snr", np.float32)])
+
+
+def build(force: bool = False) -> str:
+    src = os.path.join(_HERE, "aa_oracle.c")
+    if force or not os.path.exists(_LIB_PATH) or os.path.getmtime(_LIB_PATH) < os.path.getmtime(src):
+        subprocess.check_call(["gcc", "-O2", "-ffp-contract=off", "-fopenmp", "-shared", "-fPIC",
+                               "-o", _LIB_PATH, src, "-lm"])
+    return _LIB_PATH
+
+
+def _load():
+    global _lib
+    if _lib is None:
+        build()
+        lib = ctypes.CDLL(_LIB_PATH)
+        i32, i64, u64, dbl, vp = ctypes.c_int, ctypes.c_int64, ctypes.c_uint64, ctypes.c_double, ctypes.c_void_p
+        lib.aaor_delays.restype = None
+        lib.aaor_delays.argtypes = [i32, dbl, dbl, dbl, i32, dbl, dbl, i32, vp]
+        lib.aaor_bin.restype = i32
+        lib.aaor_bin.argtypes = [vp, u64, i32, i32, u64, u64, vp]
+        lib.aaor_dedisperse.restype = i32
+        lib.aaor_dedisperse.argtypes = [vp, i32, u64, u64, vp, i32, u64, u64, vp]
+        lib.aaor_block_stats.restype = None
+        lib.aaor_block_stats.argtypes = [vp, u64, vp, vp, vp]
+        lib.aaor_sps_row.restype = i64
+        lib.aaor_sps_row.argtypes = [vp, u64, u64, u64, u64, vp, i32, dbl, u64, u64, vp, vp, vp, i64]
+        lib.aaor_snr_at.restype = i32
+        lib.aaor_snr_at.argtypes = [vp, u64, u64, u64, dbl, dbl, vp, i32, u64, vp]
+        lib.aaor_num_threads.restype = i32
+        _lib = lib
+    return _lib
+
+
+def num_threads() -> int:
+    return int(_load().aaor_num_threads())
+
+
+# ---- steps 1-3 ---------------------------------------------------------------
+def delays(w, r) -> np.ndarray:
+    """delta_r(c, i) as int64 [ndms][nchans] for range r (steps 1-2)."""
+    rg = w.ranges[r]
+    out = np.empty((rg.ndms, w.nchans), dtype=np.int64)
+    _load().aaor_delays(w.nchans, w.f_top, w.foff, w.tsamp, rg.bin, rg.dm_low, rg.dm_step,
+                        rg.ndms, out.ctypes.data)
+    return out
+
+
+def geometry(w) -> Dict:
+    """Step 3: maxshift (raw samples, multiple of every bin), T_valid, nout per range."""
+    lcm = 1
+    for rg in w.ranges:
+        lcm = lcm * rg.bin // math.gcd(lcm, rg.bin)
+    dl = [delays(w, r) for r in range(len(w.ranges))]
+    maxshift = max(int(d.max()) * rg.bin for d, rg in zip(dl, w.ranges))
+    maxshift = -(-maxshift // lcm) * lcm
+    t_valid = w.nsamp - maxshift
+    if t_valid <= 0:
+        raise ValueError("observation shorter than the DM sweep")
+    return {"maxshift": maxshift, "t_valid": t_valid,
+            "nout": [t_valid // rg.bin for rg in w.ranges], "delays": dl}
+
+
+# ---- steps 4-5 ---------------------------------------------------------------
+def dedisperse(x: np.ndarray, w, r: int, rows: Optional[Sequence[int]] = None,
+               tau_first: int = 0, ntau: Optional[int] = None, geo: Optional[Dict] = None) -> np.ndarray:
+    """D[r][rows][tau_first : tau_first+ntau] as uint32 (steps 4-5)."""
+    lib = _load()
+    geo = geo or geometry(w)
+    rg = w.ranges[r]
+    dl = geo["delays"][r]
+    if rows is not None:
+        dl = np.ascontiguousarray(dl[np.asarray(rows, dtype=np.int64)])
+    if ntau is None:
+        ntau = geo["nout"][r] - tau_first
+    assert x.dtype == np.uint8 and x.shape == (w.nsamp, w.nchans)
+    assert 255 * w.nchans * rg.bin < 2 ** 32
+    span = ntau + int(dl.max())                       # binned samples needed from tau_first on
+    y = np.empty((w.nchans, span), dtype=np.uint32)
+    if lib.aaor_bin(x.ctypes.data, w.nsamp, w.nchans, rg.bin, tau_first, span, y.ctypes.data) != 0:
+        raise ValueError("binned span runs past the observation")
+    D = np.empty((dl.shape[0], ntau), dtype=np.uint32)
+    rc = lib.aaor_dedisperse(y.ctypes.data, w.nchans, tau_first, span, dl.ctypes.data, dl.shape[0],
+                             tau_first, ntau, D.ctypes.data)
+    if rc != 0:
+        raise ValueError("delay window outside the binned span")
+    return D
+
+
+# ---- step 6 --------------------------------------------------------------------
+def block_stats(d: np.ndarray) -> Tuple[float, float, int]:
+    d = np.ascontiguousarray(d, dtype=np.uint32)
+    mu, sg, ns = ctypes.c_double(), ctypes.c_double(), ctypes.c_uint64()
+    _load().aaor_block_stats(d.ctypes.data, d.size, ctypes.byref(mu), ctypes.byref(sg), ctypes.byref(ns))
+    return mu.value, sg.value, ns.value
+
+
+# ---- steps 7-8 -----------------------------------------------------------------
+def sps_row(d: np.ndarray, w, r: int, *, d_first: int = 0, tau_a: int = 0,
+            tau_b: Optional[int] = None, nout: Optional[int] = None,
+            geo: Optional[Dict] = None) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
+    """Candidates (tau, width, S/N double; binned units) of one dedispersed row."""
+    lib = _load()
+    rg = w.ranges[r]
+    if nout is None:
+        nout = (geo or geometry(w))["nout"][r]
+    if tau_b is None:
+        tau_b = nout
+    L = w.norm_block // rg.bin
+    d = np.ascontiguousarray(d, dtype=np.uint32)
+    widths = np.asarray(w.widths, dtype=np.int32)
+    cap = max(1024, min(int(tau_b - tau_a), 1 << 22))
+    while True:
+        tau = np.empty(cap, dtype=np.uint64); ww = np.empty(cap, dtype=np.int32); sn = np.empty(cap, dtype=np.float64)
+        n = lib.aaor_sps_row(d.ctypes.data, d_first, d.size, nout, L, widths.ctypes.data, widths.size,
+                             float(w.snr_threshold), tau_a, tau_b, tau.ctypes.data, ww.ctypes.data,
+                             sn.ctypes.data, cap)
+        if n < 0:
+            raise ValueError("row segment does not cover the requested blocks")
+        if n <= cap:
+            return tau[:n].copy(), ww[:n].copy(), sn[:n].copy()
+        cap = int(n)
+
+
+def snr_at(d: np.ndarray, w, r: int, tau: int, mu: float, sigma: float, *, d_first: int = 0,
+           nout: Optional[int] = None) -> np.ndarray:
+    """S/N of every width at one tau (-inf where the boxcar does not fit)."""
+    d = np.ascontiguousarray(d, dtype=np.uint32)
+    widths = np.asarray(w.widths, dtype=np.int32)
+    out = np.empty(widths.size, dtype=np.float64)
+    if nout is None:
+        nout = geometry(w)["nout"][r]
+    if _load().aaor_snr_at(d.ctypes.data, d_first, d.size, nout, mu, sigma, widths.ctypes.data,
+                           widths.size, tau, out.ctypes.data) != 0:
+        raise ValueError("row segment does not cover tau")
+    return out
+
+
+def pack_candidates(dm_index: int, bin_: int, tau, ww, sn) -> np.ndarray:
+    """Step 8 output record: global dm index, raw-sample start and width, float S/N (A14)."""
+    out = np.empty(len(tau), dtype=CAND_DTYPE)
+    out["dm_index"] = dm_index
+    out["t_start"] = (np.asarray(tau, dtype=np.uint64) * bin_).astype(np.uint32)
+    out["width"] = (np.asarray(ww, dtype=np.int64) * bin_).astype(np.uint32)
+    out["snr"] = np.asarray(sn, dtype=np.float64).astype(np.float32)
+    return out
+
+
+def run(x: np.ndarray, w, *, keep_dense: bool = False, row_subset: Optional[Dict[int, Sequence[int]]] = None,
+        threads: Optional[int] = None):
+    """Whole observation at once: candidates sorted by (dm_index, t_start) [+ dense D per range].
+
+    `row_subset` {range: [rows]} restricts the DM trials (rows are independent).
+    """
+    geo = geometry(w)
+    cands: List[np.ndarray] = []
+    dense = {}
+    base = 0
+    for r, rg in enumerate(w.ranges):
+        rows = list(range(rg.ndms)) if row_subset is None else list(row_subset.get(r, []))
+        if rows:
+            D = dedisperse(x, w, r, rows=rows, geo=geo)
+            if keep_dense:
+                dense[r] = D
+
+            def one(k, D=D, r=r, rows=rows, base=base, rg=rg):
+                tau, ww, sn = sps_row(D[k], w, r, geo=geo)
+                return pack_candidates(base + rows[k], rg.bin, tau, ww, sn)
+
+            with ThreadPoolExecutor(max_workers=threads or os.cpu_count() or 1) as ex:
+                cands.extend(ex.map(one, range(len(rows))))
+        base += rg.ndms
+    allc = np.concatenate(cands) if cands else np.empty(0, dtype=CAND_DTYPE)
+    order = np.lexsort((allc["t_start"], allc["dm_index"]))
+    allc = allc[order]
+    return (allc, dense, geo) if keep_dense else (allc, geo)

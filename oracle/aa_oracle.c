@@ -1,0 +1,217 @@
+/*
+ * ORACLE -- TEST INFRASTRUCTURE ONLY.
+ *
+ * Plain, slow, obviously-correct CPU statement of what the hot path computes:
+ * brute-force incoherent dedispersion of 8-bit filterbank data followed by the
+ * single-pulse search (boxcar S/N over a width list, robust per-block mean and
+ * sigma, threshold, one candidate per (DM, time)).  Only tests/,
+ * __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs
+ * may call it.  It shares no code, header, table or helper with the CUDA path
+ * (paper_2101_00941_b200/csrc) and knows nothing of chunks, streams or tiles:
+ * it works on the whole observation (or on a plain sub-range of output
+ * samples) exactly in the order of SURVEY.md §8(c) steps 1-8.
+ *
+ * What defines each step.  The paper names the two phases --
+ * "dedispersion of data and single pulse searching" --
+ * but gives no formula; the arithmetic is fixed by BASELINE.json:north_star
+ * (delay formula, exact integer sums, S/N tolerances) and by the readings
+ * A1-A16 of SURVEY.md §8(c), restated in DESIGN.md "Readings".
+ *
+ * Parity pins (tests/test_oracle_pins.py): delay closed forms and spot values;
+ * DM=0 row == plain channel sum; constant input; single-impulse brute force;
+ * python-loop brute force on tiny inputs; statistics vs numpy on un-clipped
+ * data and vs a python restatement of the clipping; S/N of an injected boxcar
+ * vs its closed form; candidate rule vs python loops.
+ * Parity unpinned against the paper (the paper fixes none of them): the choice
+ * of estimator (A8), the norm-block length (A9), the candidate definition
+ * (A11).  They are conventions of this build, pinned only to their own written
+ * definition by brute force.
+ *
+ * Floating point: double everywhere, no FMA contraction (compile with
+ * -ffp-contract=off), statistics from exact integer sums so that the only
+ * roundings are the ones written below.
+ */
+#include <math.h>
+#include <stdint.h>
+#include <stdlib.h>
+#include <string.h>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+/* ---- steps 1-2: channel frequencies and integer delays --------------------
+ * f_c = f_top + c*foff  (channel centres, A2);  DM_i = dm_low + i*dm_step;
+ * delta(c,i) = floor(v + 0.5),
+ *   v = ((4.148808e3*DM_i) * (1/(f_c*f_c) - 1/(f_top*f_top))) / (tsamp*bin)
+ * (north_star: "delay(c,DM) = round(4.148808e3*DM*(f_c^-2 - f_top^-2)/tsamp) in
+ * double"; binned ranges measure the delay in binned samples, A6).
+ * out[i*nchans + c]. */
+void aaor_delays(int nchans, double f_top, double foff, double tsamp, int bin,
+                 double dm_low, double dm_step, int ndms, int64_t *out)
+{
+    double ts = tsamp * (double)bin;
+    for (int i = 0; i < ndms; ++i) {
+        double dm = dm_low + (double)i * dm_step;
+        for (int c = 0; c < nchans; ++c) {
+            double f = f_top + (double)c * foff;
+            double g = 1.0 / (f * f) - 1.0 / (f_top * f_top);
+            double v = ((4.148808e3 * dm) * g) / ts;
+            out[(size_t)i * nchans + c] = (int64_t)floor(v + 0.5);
+        }
+    }
+}
+
+/* ---- step 4: binned, channel-major input ----------------------------------
+ * y[c][k] = sum_{i<bin} x[(bin*(tau_first+k) + i)][c],  k = 0..ntau-1,
+ * x time-major [nsamp][nchans] (A1), integer sum before delaying (A6).
+ * Samples past the end of the observation must not be asked for. */
+int aaor_bin(const uint8_t *x, uint64_t nsamp, int nchans, int bin,
+             uint64_t tau_first, uint64_t ntau, uint32_t *y)
+{
+    if ((tau_first + ntau) * (uint64_t)bin > nsamp) return -1;
+    #pragma omp parallel for schedule(static)
+    for (int c = 0; c < nchans; ++c)
+        for (uint64_t k = 0; k < ntau; ++k) {
+            uint32_t s = 0;
+            for (int i = 0; i < bin; ++i)
+                s += x[((tau_first + k) * (uint64_t)bin + (uint64_t)i) * (uint64_t)nchans + (uint64_t)c];
+            y[(size_t)c * ntau + k] = s;
+        }
+    return 0;
+}
+
+/* ---- step 5: dedispersion ---------------------------------------------------
+ * D[i][k] = sum_c y[c][(tau_first + k) + delta(c,i) - y_first],  k = 0..ntau-1,
+ * where row c of y holds binned samples y_first .. y_first+ny-1.
+ * Exact integer sums (A7: 255*nchans*bin < 2^32 is checked by the caller). */
+int aaor_dedisperse(const uint32_t *y, int nchans, uint64_t y_first, uint64_t ny,
+                    const int64_t *delays, int ndms,
+                    uint64_t tau_first, uint64_t ntau, uint32_t *D)
+{
+    int bad = 0;
+    #pragma omp parallel for schedule(dynamic, 1)
+    for (int i = 0; i < ndms; ++i) {
+        uint32_t *row = D + (size_t)i * ntau;
+        memset(row, 0, ntau * sizeof(uint32_t));
+        for (int c = 0; c < nchans; ++c) {
+            int64_t dl = delays[(size_t)i * nchans + c];
+            int64_t first = (int64_t)tau_first + dl - (int64_t)y_first;
+            if (first < 0 || (uint64_t)first + ntau > ny) { bad = 1; continue; }
+            const uint32_t *src = y + (size_t)c * ny + (size_t)first;
+            for (uint64_t k = 0; k < ntau; ++k) row[k] += src[k];
+        }
+    }
+    return bad ? -1 : 0;
+}
+
+/* ---- step 6: robust mean and sigma of one norm block ----------------------
+ * Plain pass over all n samples, then exactly three passes that keep the
+ * samples with |x - mu| <= 3 sigma (latest mu, sigma; chosen among ALL n samples
+ * each time) and recompute.  Population sigma, no bias correction (A8).
+ * Each (mu, sigma) comes from exact integer sums m = #, S1 = sum x, S2 = sum x^2:
+ *     mu = S1/m,   sigma = sqrt( (m*S2 - S1^2) / (m*m) )
+ * with m*S2 - S1^2 formed exactly in 128-bit integers and rounded once. */
+static void moments(uint64_t m, uint64_t S1, uint64_t S2, double *mu, double *sigma)
+{
+    unsigned __int128 N = (unsigned __int128)m * S2 - (unsigned __int128)S1 * S1;
+    double dm = (double)m;
+    *mu = (double)S1 / dm;
+    *sigma = sqrt((double)N / (dm * dm));
+}
+
+void aaor_block_stats(const uint32_t *d, uint64_t n, double *mu_out, double *sigma_out,
+                      uint64_t *nsel_out)
+{
+    uint64_t m = 0, S1 = 0, S2 = 0;
+    double mu = 0.0, sigma = 0.0;
+    for (uint64_t k = 0; k < n; ++k) { m++; S1 += d[k]; S2 += (uint64_t)d[k] * d[k]; }
+    if (m) moments(m, S1, S2, &mu, &sigma);
+    for (int pass = 0; pass < 3 && m; ++pass) {
+        double lim = 3.0 * sigma;
+        m = 0; S1 = 0; S2 = 0;
+        for (uint64_t k = 0; k < n; ++k)
+            if (fabs((double)d[k] - mu) <= lim) { m++; S1 += d[k]; S2 += (uint64_t)d[k] * d[k]; }
+        if (m) moments(m, S1, S2, &mu, &sigma);
+    }
+    *mu_out = mu; *sigma_out = sigma; *nsel_out = m;
+}
+
+/* ---- steps 6-8 for one dedispersed row --------------------------------------
+ * d[0..d_count) holds D[row][d_first .. d_first+d_count).  nout = number of valid
+ * output samples of the row's range, L = norm-block length in binned samples.
+ * Emits one candidate per tau in [tau_a, tau_b) (tau_a on a block boundary):
+ *   for every width w with tau + w <= nout:  B_w = sum_{i<w} D[tau+i],
+ *   S_w = (B_w - w*mu_k) / (sigma_k*sqrt(w)),  k = block containing tau   (A9, A10)
+ *   w* = argmax_w S_w (ties -> smallest w);  emit iff S_{w*} >= thr, sigma_k > 0
+ *   and the block has n_k >= 32 samples                                    (A11, A13)
+ * Returns the number found (may exceed max_out; only max_out are stored) or -1
+ * if d does not cover what is needed. */
+int64_t aaor_sps_row(const uint32_t *d, uint64_t d_first, uint64_t d_count,
+                     uint64_t nout, uint64_t L,
+                     const int32_t *widths, int nwidths, double thr,
+                     uint64_t tau_a, uint64_t tau_b,
+                     uint64_t *out_tau, int32_t *out_w, double *out_snr, int64_t max_out)
+{
+    int64_t found = 0;
+    if (tau_b > nout) tau_b = nout;
+    if (tau_a % L != 0) return -1;
+    for (uint64_t b0 = tau_a; b0 < tau_b; b0 += L) {
+        uint64_t b1 = b0 + L < nout ? b0 + L : nout;       /* block [b0, b1) */
+        uint64_t n_k = b1 - b0, nsel;
+        double mu, sigma;
+        if (b0 < d_first || b1 > d_first + d_count) return -1;
+        aaor_block_stats(d + (b0 - d_first), n_k, &mu, &sigma, &nsel);
+        if (!(sigma > 0.0) || n_k < 32) continue;
+        uint64_t e = b1 < tau_b ? b1 : tau_b;
+        for (uint64_t tau = b0; tau < e; ++tau) {
+            double best = 0.0; int32_t best_w = 0;
+            for (int j = 0; j < nwidths; ++j) {
+                uint64_t w = (uint64_t)widths[j];
+                if (tau + w > nout) continue;
+                if (tau + w > d_first + d_count) return -1;
+                int64_t B = 0;
+                for (uint64_t i = 0; i < w; ++i) B += d[tau + i - d_first];
+                double S = ((double)B - (double)w * mu) / (sigma * sqrt((double)w));
+                if (best_w == 0 || S > best) { best = S; best_w = (int32_t)w; }
+            }
+            if (best_w != 0 && best >= thr) {
+                if (found < max_out) { out_tau[found] = tau; out_w[found] = best_w; out_snr[found] = best; }
+                found++;
+            }
+        }
+    }
+    return found;
+}
+
+/* S/N of every width at one tau (for tolerance-aware comparisons in tests). */
+int aaor_snr_at(const uint32_t *d, uint64_t d_first, uint64_t d_count, uint64_t nout,
+                double mu, double sigma, const int32_t *widths, int nwidths,
+                uint64_t tau, double *snr_out)
+{
+    for (int j = 0; j < nwidths; ++j) {
+        uint64_t w = (uint64_t)widths[j];
+        snr_out[j] = -INFINITY;
+        if (tau + w > nout) continue;
+        if (tau < d_first || tau + w > d_first + d_count) return -1;
+        int64_t B = 0;
+        for (uint64_t i = 0; i < w; ++i) B += d[tau + i - d_first];
+        snr_out[j] = ((double)B - (double)w * mu) / (sigma * sqrt((double)w));
+    }
+    return 0;
+}
+
+int aaor_num_threads(void)
+{
+    int n = 1;
+    #pragma omp parallel
+    {
+        #pragma omp single
+        n =
+#ifdef _OPENMP
+            omp_get_num_threads();
+#else
+            1;
+#endif
+    }
+    return n;
+}
