@@ -1,0 +1,179 @@
+/*
+ * aa.h -- C ABI of the B200-native streamed dedispersion + single-pulse search.
+ *
+ * The hot path of "Implementing CUDA Streams into AstroAccelerate - A Case Study"
+ * (arXiv 2101.00941): time chunks split into per-stream sub-chunks (PAPER.md:33,
+ * Fig. 2), pinned host memory and asynchronous copies (PAPER.md:41 steps 1-5,
+ * :49-51), dedispersion then single-pulse search per sub-chunk (PAPER.md:19, :43,
+ * :71), one host thread per stream for the host-side output copy.
+ * The paper states no interface (AstroAccelerate is a program); the three calls
+ * and their arguments follow BASELINE.json:north_star, the arithmetic follows
+ * SURVEY.md section 8(c) as restated in DESIGN.md.
+ *
+ * Conventions
+ *   - plain C, no exceptions, no global state; every function returns an aa_status
+ *     (0 = AA_OK, negative = error) unless stated otherwise.
+ *   - "host" pointers are ordinary process memory; "pinned" means page-locked
+ *     (cudaHostAlloc / cudaHostRegister / aa_host_alloc); "device" means CUDA
+ *     device memory of the current device.
+ *   - the caller owns every buffer it passes; aa_plan_create copies the arrays in
+ *     the descriptor; the library owns what it allocates and frees it in aa_destroy.
+ *   - one aa_plan may be used by one thread at a time; different plans are independent.
+ */
+#ifndef AA_H_
+#define AA_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    AA_OK = 0,
+    AA_ERR_INVALID = -1,     /* bad argument / inconsistent descriptor */
+    AA_ERR_NOT_PINNED = -2,  /* aa_run input is pageable host memory (never staged silently) */
+    AA_ERR_OOM = -3,         /* device or pinned allocation failed */
+    AA_ERR_CUDA = -4,        /* a CUDA call failed; see aa_last_cuda_error() */
+    AA_ERR_OVERFLOW = -5     /* more candidates than the output / per-sub-chunk buffers hold;
+                                the run is otherwise valid and *n_cands is the true total */
+} aa_status;
+
+/* One DM range of the plan: DM_i = dm_low + i*dm_step (double), i = 0..ndms-1, searched on
+ * the input summed over `bin` consecutive raw samples (time decimation). */
+typedef struct {
+    double  dm_low;      /* pc cm^-3 */
+    double  dm_step;     /* pc cm^-3, >= 0 */
+    int32_t ndms;        /* > 0 */
+    int32_t bin;         /* >= 1, divides norm_block */
+} aa_dm_range;
+
+/* One detection. 16 bytes. */
+typedef struct {
+    uint32_t dm_index;   /* global trial index: ranges concatenated in plan order */
+    uint32_t t_start;    /* first raw input sample of the boxcar (= tau*bin) */
+    uint32_t width;      /* boxcar width in raw samples (= w*bin) */
+    float    snr;        /* (B_w - w*mu)/(sigma*sqrt(w)), computed in double, stored as float */
+} aa_candidate;
+
+typedef struct {
+    /* filterbank: x[t][c] uint8, time-major, channel 0 centred on f_top, foff < 0 (A1, A2) */
+    int32_t  nchans;
+    uint64_t nsamp;
+    double   tsamp;            /* seconds */
+    double   f_top;            /* MHz */
+    double   foff;             /* MHz, negative */
+    /* search plan */
+    int32_t  nranges;
+    const aa_dm_range *ranges;
+    int32_t  nwidths;
+    const int32_t *widths;     /* boxcar widths in BINNED samples of each range, ascending, >= 1 */
+    double   snr_threshold;
+    /* streaming: each time chunk of chunk_len raw samples is split into n_streams
+     * sub-chunks; chunk_len/n_streams must be a multiple of norm_block and at least the halo
+     * (DM sweep + longest boxcar) reported by aa_plan_query. */
+    int32_t  n_streams;        /* 1..64 */
+    uint64_t chunk_len;        /* raw samples */
+    uint32_t norm_block;       /* raw samples per normalisation block; 0 -> 65536 (A9) */
+    /* optional resources owned by the caller (e.g. a torch tensor and torch streams);
+     * NULL/0 -> the library allocates with cudaMalloc and creates non-blocking streams. */
+    void    *device_arena;       /* device */
+    uint64_t device_arena_bytes; /* must be >= aa_plan_arena_bytes(desc) */
+    void *const *streams;        /* cudaStream_t[n_streams] or NULL */
+    /* dense rows to hand back for parity checks: global dm indices, ascending */
+    int32_t  ntap;
+    const uint32_t *tap_dm_indices;
+    /* capacity of each stream's device candidate list per sub-chunk; 0 -> 1<<21 */
+    uint64_t max_cands_per_subchunk;
+} aa_plan_desc;
+
+typedef struct {
+    uint64_t maxshift;          /* raw samples, multiple of every bin */
+    uint64_t t_valid;           /* nsamp - maxshift */
+    uint64_t halo;              /* raw samples a sub-chunk reads past its own span */
+    uint64_t subchunk_len;      /* chunk_len / n_streams */
+    uint64_t n_subchunks;
+    uint64_t ndms_total;
+    uint64_t dm_trial_samples;  /* sum_r ndms_r * nout_r : the work unit of the metric */
+    uint64_t arena_bytes;       /* device memory the plan uses */
+    uint64_t pinned_bytes;      /* pinned staging the plan owns */
+    uint64_t tap_row_len;       /* uint32 elements per tapped row in aa_run's tap_out
+                                   (= max over ranges of nout_r); 0 if ntap == 0 */
+} aa_plan_info;
+
+typedef struct {
+    double   wall_ms;           /* aa_run call -> return */
+    double   sort_ms;           /* final host sort, inside wall_ms */
+    uint64_t h2d_bytes, d2h_bytes;
+    double   h2d_ms, d2h_ms;    /* sum of copy durations (CUDA events on their streams) */
+    double   prep_ms;           /* corner turn + binning kernels, summed */
+    double   dedisp_ms;         /* dedispersion kernels, summed over launches */
+    double   sps_ms;            /* statistics + boxcar/candidate kernels, summed */
+    uint64_t dedisp_launches, sps_launches, prep_launches;
+    uint64_t n_candidates;      /* true total found */
+    uint64_t n_stored;          /* records written to `out` (< n_candidates only on overflow) */
+    int32_t  overflow;          /* 1 if any list was truncated */
+    int32_t  n_streams;
+} aa_stats;
+
+typedef struct aa_plan aa_plan;
+
+/* Device bytes a plan built from `d` needs (for callers that bring their own arena).
+ * Returns 0 if the descriptor is invalid. */
+uint64_t aa_plan_arena_bytes(const aa_plan_desc *d);
+
+/* Allocation phase (PAPER.md:19 part 2, :41 steps 1-2, :71): validates the descriptor, builds
+ * the delay tables in double (north_star formula), creates streams and events, allocates the
+ * device ring, per-stream work buffers, candidate lists and pinned staging.  Nothing is
+ * allocated later.  *out is NULL on error. */
+int aa_plan_create(aa_plan **out, const aa_plan_desc *d);
+
+int aa_plan_query(const aa_plan *p, aa_plan_info *out);
+
+/* nout_r (valid output samples, binned) of range r, or 0 if r is out of range. */
+uint64_t aa_plan_nout(const aa_plan *p, int32_t r);
+
+/* Copies the integer delay table of range r ([ndms_r][nchans] int32, binned samples) to host
+ * memory `out`; used by tests to compare with the oracle entry by entry. */
+int aa_plan_delays(const aa_plan *p, int32_t r, int32_t *out);
+
+/*
+ * The hot path: for every sub-chunk, on its stream:
+ * async H2D of the new input rows -> corner turn into the device ring -> per range: (binning,)
+ * dedispersion, block statistics + boxcar S/N + candidate compaction -> D2H of the candidate
+ * list into pinned staging; one host thread per stream copies staging into `out`.
+ *   host_input : PINNED host, uint8 [nsamp][nchans]           (AA_ERR_NOT_PINNED otherwise)
+ *   out        : host (pageable ok), room for max_cands records; sorted by (dm_index, t_start)
+ *   n_cands    : host, receives the true number found; if it exceeds max_cands or a sub-chunk's
+ *                device list overflowed the call returns AA_ERR_OVERFLOW and aa_stats.n_stored
+ *                says how many (sorted) records `out` holds
+ *   tap_out    : host (pageable ok) uint32 [ntap][tap_row_len] or NULL; row k receives the
+ *                dedispersed series of tap_dm_indices[k], nout_r values, rest untouched
+ * No allocation, no pageable copy and no device-wide synchronisation happen inside.
+ */
+int aa_run(aa_plan *p, const uint8_t *host_input, aa_candidate *out, uint64_t max_cands,
+           uint64_t *n_cands, uint32_t *tap_out);
+
+/* Same path with the observation already in device memory (uint8 [nsamp][nchans], device):
+ * the H2D step is skipped, everything else is identical.  Used for kernel-only timing. */
+int aa_run_resident(aa_plan *p, const uint8_t *device_input, aa_candidate *out, uint64_t max_cands,
+                    uint64_t *n_cands, uint32_t *tap_out);
+
+/* Timings and counters of the last aa_run / aa_run_resident on this plan. */
+int aa_get_stats(const aa_plan *p, aa_stats *out);
+
+/* NULL-safe.  Frees everything the plan allocated (not a caller-owned arena or streams). */
+void aa_destroy(aa_plan *p);
+
+/* Pinned host allocation helpers (cudaHostAlloc / cudaFreeHost). */
+int  aa_host_alloc(void **p, uint64_t bytes);
+void aa_host_free(void *p);
+
+const char *aa_strerror(int status);
+/* cudaError_t of the last failing CUDA call in this thread's last aa_* call (0 if none). */
+int aa_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* AA_H_ */

@@ -1,0 +1,224 @@
+"""Thin ctypes binding of the C-ABI library (include/aa.h): argument marshalling only.
+
+Every step of the path runs in libaa's CUDA kernels.  PyTorch supplies device memory (the plan's
+arena is a torch uint8 tensor), streams and pinned host tensors; there is no CPU fallback: if
+libaa.so is missing or no CUDA device is present the calls raise.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libaa.so")
+
+AA_OK, AA_ERR_INVALID, AA_ERR_NOT_PINNED, AA_ERR_OOM, AA_ERR_CUDA, AA_ERR_OVERFLOW = 0, -1, -2, -3, -4, -5
+
+CAND_DTYPE = np.dtype([("dm_index", np.uint32), ("t_start", np.uint32),
+                       ("width", np.uint32), ("snr", np.float32)])
+
+EXPORTS = ["aa_plan_arena_bytes", "aa_plan_create", "aa_plan_query", "aa_plan_nout", "aa_plan_delays",
+           "aa_run", "aa_run_resident", "aa_get_stats", "aa_destroy", "aa_host_alloc", "aa_host_free",
+           "aa_strerror", "aa_last_cuda_error"]
+
+
+class DMRangeC(ctypes.Structure):
+    _fields_ = [("dm_low", ctypes.c_double), ("dm_step", ctypes.c_double),
+                ("ndms", ctypes.c_int32), ("bin", ctypes.c_int32)]
+
+
+class PlanDescC(ctypes.Structure):
+    _fields_ = [("nchans", ctypes.c_int32), ("nsamp", ctypes.c_uint64), ("tsamp", ctypes.c_double),
+                ("f_top", ctypes.c_double), ("foff", ctypes.c_double),
+                ("nranges", ctypes.c_int32), ("ranges", ctypes.POINTER(DMRangeC)),
+                ("nwidths", ctypes.c_int32), ("widths", ctypes.POINTER(ctypes.c_int32)),
+                ("snr_threshold", ctypes.c_double),
+                ("n_streams", ctypes.c_int32), ("chunk_len", ctypes.c_uint64), ("norm_block", ctypes.c_uint32),
+                ("device_arena", ctypes.c_void_p), ("device_arena_bytes", ctypes.c_uint64),
+                ("streams", ctypes.POINTER(ctypes.c_void_p)),
+                ("ntap", ctypes.c_int32), ("tap_dm_indices", ctypes.POINTER(ctypes.c_uint32)),
+                ("max_cands_per_subchunk", ctypes.c_uint64)]
+
+
+class PlanInfoC(ctypes.Structure):
+    _fields_ = [(n, ctypes.c_uint64) for n in
+                ("maxshift", "t_valid", "halo", "subchunk_len", "n_subchunks", "ndms_total",
+                 "dm_trial_samples", "arena_bytes", "pinned_bytes", "tap_row_len")]
+
+
+class StatsC(ctypes.Structure):
+    _fields_ = [("wall_ms", ctypes.c_double), ("sort_ms", ctypes.c_double),
+                ("h2d_bytes", ctypes.c_uint64), ("d2h_bytes", ctypes.c_uint64),
+                ("h2d_ms", ctypes.c_double), ("d2h_ms", ctypes.c_double), ("prep_ms", ctypes.c_double),
+                ("dedisp_ms", ctypes.c_double), ("sps_ms", ctypes.c_double),
+                ("dedisp_launches", ctypes.c_uint64), ("sps_launches", ctypes.c_uint64),
+                ("prep_launches", ctypes.c_uint64), ("n_candidates", ctypes.c_uint64), ("n_stored", ctypes.c_uint64),
+                ("overflow", ctypes.c_int32), ("n_streams", ctypes.c_int32)]
+
+
+class AAError(RuntimeError):
+    def __init__(self, status: int, msg: str):
+        super().__init__(f"libaa status {status}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def load_library() -> ctypes.CDLL:
+    """dlopen libaa.so and declare every symbol of include/aa.h.  Raises if it is missing."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2101_00941_b200.build` "
+                          "(there is no CPU fallback)")
+    lib = ctypes.CDLL(LIB_PATH)
+    vp, u64, i32 = ctypes.c_void_p, ctypes.c_uint64, ctypes.c_int32
+    lib.aa_plan_arena_bytes.restype = u64
+    lib.aa_plan_arena_bytes.argtypes = [ctypes.POINTER(PlanDescC)]
+    lib.aa_plan_create.restype = ctypes.c_int
+    lib.aa_plan_create.argtypes = [ctypes.POINTER(vp), ctypes.POINTER(PlanDescC)]
+    lib.aa_plan_query.restype = ctypes.c_int
+    lib.aa_plan_query.argtypes = [vp, ctypes.POINTER(PlanInfoC)]
+    lib.aa_plan_nout.restype = u64
+    lib.aa_plan_nout.argtypes = [vp, i32]
+    lib.aa_plan_delays.restype = ctypes.c_int
+    lib.aa_plan_delays.argtypes = [vp, i32, vp]
+    for f in (lib.aa_run, lib.aa_run_resident):
+        f.restype = ctypes.c_int
+        f.argtypes = [vp, vp, vp, u64, ctypes.POINTER(u64), vp]
+    lib.aa_get_stats.restype = ctypes.c_int
+    lib.aa_get_stats.argtypes = [vp, ctypes.POINTER(StatsC)]
+    lib.aa_destroy.restype = None
+    lib.aa_destroy.argtypes = [vp]
+    lib.aa_host_alloc.restype = ctypes.c_int
+    lib.aa_host_alloc.argtypes = [ctypes.POINTER(vp), u64]
+    lib.aa_host_free.restype = None
+    lib.aa_host_free.argtypes = [vp]
+    lib.aa_strerror.restype = ctypes.c_char_p
+    lib.aa_strerror.argtypes = [ctypes.c_int]
+    lib.aa_last_cuda_error.restype = ctypes.c_int
+    lib.aa_last_cuda_error.argtypes = []
+    _lib = lib
+    return lib
+
+
+def _check(lib, rc: int, allow_overflow: bool = False) -> int:
+    if rc == AA_OK or (allow_overflow and rc == AA_ERR_OVERFLOW):
+        return rc
+    msg = lib.aa_strerror(rc).decode()
+    if rc == AA_ERR_CUDA:
+        msg += f" (cudaError {lib.aa_last_cuda_error()})"
+    raise AAError(rc, msg)
+
+
+def pinned_empty(nbytes: int):
+    """Pinned host uint8 tensor (torch owns it)."""
+    import torch
+    return torch.empty(int(nbytes), dtype=torch.uint8, pin_memory=True)
+
+
+class Plan:
+    """aa_plan_create / aa_run / aa_destroy with torch-owned device memory and streams."""
+
+    def __init__(self, w, *, n_streams: Optional[int] = None, chunk_len: Optional[int] = None,
+                 taps: Optional[Sequence[int]] = None, max_cands_per_subchunk: int = 0,
+                 torch_resources: bool = True):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: the path has no CPU fallback")
+        self.lib = load_library()
+        self.w = w
+        self._ranges = (DMRangeC * len(w.ranges))(*[DMRangeC(r.dm_low, r.dm_step, r.ndms, r.bin) for r in w.ranges])
+        self._widths = (ctypes.c_int32 * len(w.widths))(*w.widths)
+        taps = sorted(int(t) for t in (taps or []))
+        self._taps = (ctypes.c_uint32 * max(1, len(taps)))(*taps)
+        self.taps = taps
+        d = PlanDescC()
+        d.nchans, d.nsamp, d.tsamp, d.f_top, d.foff = w.nchans, w.nsamp, w.tsamp, w.f_top, w.foff
+        d.nranges, d.ranges = len(w.ranges), self._ranges
+        d.nwidths, d.widths = len(w.widths), self._widths
+        d.snr_threshold = float(w.snr_threshold)
+        d.n_streams = int(n_streams if n_streams is not None else w.n_streams)
+        d.chunk_len = int(chunk_len if chunk_len is not None else w.chunk_len)
+        d.norm_block = int(getattr(w, "norm_block", 65536))
+        d.ntap = len(taps)
+        d.tap_dm_indices = self._taps if taps else None
+        d.max_cands_per_subchunk = int(max_cands_per_subchunk)
+        self._arena = None
+        self._streams = None
+        if torch_resources:
+            need = self.lib.aa_plan_arena_bytes(ctypes.byref(d))
+            if need == 0:
+                raise AAError(AA_ERR_INVALID, "invalid plan descriptor")
+            self._arena = torch.empty(int(need) + 256, dtype=torch.uint8, device="cuda")
+            base = (self._arena.data_ptr() + 255) & ~255
+            d.device_arena = base
+            d.device_arena_bytes = need
+            self._streams = [torch.cuda.Stream() for _ in range(d.n_streams)]
+            self._stream_arr = (ctypes.c_void_p * d.n_streams)(*[s.cuda_stream for s in self._streams])
+            d.streams = self._stream_arr
+        self.desc = d
+        self.handle = ctypes.c_void_p()
+        _check(self.lib, self.lib.aa_plan_create(ctypes.byref(self.handle), ctypes.byref(d)))
+        info = PlanInfoC()
+        _check(self.lib, self.lib.aa_plan_query(self.handle, ctypes.byref(info)))
+        self.info = {n: int(getattr(info, n)) for n, _ in PlanInfoC._fields_}
+        self.nout = [int(self.lib.aa_plan_nout(self.handle, r)) for r in range(len(w.ranges))]
+        self.overflow = False
+
+    # ------------------------------------------------------------------
+    def delays(self, r: int) -> np.ndarray:
+        out = np.empty((self.w.ranges[r].ndms, self.w.nchans), dtype=np.int32)
+        _check(self.lib, self.lib.aa_plan_delays(self.handle, r, out.ctypes.data))
+        return out
+
+    def _run(self, fn, ptr: int, max_cands: int, want_taps: bool):
+        out = np.empty(int(max_cands), dtype=CAND_DTYPE)
+        n = ctypes.c_uint64(0)
+        tap = None
+        if want_taps and self.taps:
+            tap = np.zeros((len(self.taps), self.info["tap_row_len"]), dtype=np.uint32)
+        rc = fn(self.handle, ptr, out.ctypes.data, int(max_cands), ctypes.byref(n),
+                tap.ctypes.data if tap is not None else None)
+        _check(self.lib, rc, allow_overflow=True)
+        self.overflow = rc == AA_ERR_OVERFLOW
+        self.n_found = int(n.value)
+        return out[:int(self.stats()["n_stored"])], tap
+
+    def run(self, host_input, max_cands: int = 1 << 22, want_taps: bool = True):
+        """aa_run on a pinned host buffer (torch pinned tensor or its numpy view)."""
+        ptr = host_input.data_ptr() if hasattr(host_input, "data_ptr") else host_input.ctypes.data
+        return self._run(self.lib.aa_run, ptr, max_cands, want_taps)
+
+    def run_resident(self, device_input, max_cands: int = 1 << 22, want_taps: bool = True):
+        """aa_run_resident on a torch CUDA uint8 tensor holding the whole observation."""
+        return self._run(self.lib.aa_run_resident, device_input.data_ptr(), max_cands, want_taps)
+
+    def stats(self) -> dict:
+        s = StatsC()
+        _check(self.lib, self.lib.aa_get_stats(self.handle, ctypes.byref(s)))
+        return {n: getattr(s, n) for n, _ in StatsC._fields_}
+
+    def close(self):
+        if getattr(self, "handle", None) is not None and self.handle:
+            self.lib.aa_destroy(self.handle)
+            self.handle = ctypes.c_void_p()
+        self._arena = None
+        self._streams = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def __enter__(self):
+        return self
+
+    def __exit__(self, *exc):
+        self.close()

@@ -1,0 +1,684 @@
+// Host side of libaa: plan (allocation phase), stream/event scheduler, output stage.
+//
+// Paper mapping: all allocation happens in aa_plan_create (PAPER.md:19 part 2, :71 "moved memory
+// allocations ... to the Preparation/Memory allocation phase"); aa_run only issues asynchronous
+// copies and kernels on per-sub-chunk streams with event dependencies (PAPER.md:41 steps 3-5) and
+// uses one host thread per stream for the host-side copies.  Every stream owns a
+// private candidate list and counter (the paper's atomics / cudaStreamWaitEvent trouble,
+// PAPER.md:73, came from state shared across streams; nothing is shared here).
+#include <algorithm>
+#include <atomic>
+#include <chrono>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <memory>
+#include <mutex>
+#include <new>
+#include <thread>
+#include <vector>
+
+#include "aa_internal.h"
+
+using namespace aa;
+
+namespace {
+
+thread_local int g_last_cuda_error = 0;
+
+inline uint64_t round_up(uint64_t v, uint64_t m) { return (v + m - 1) / m * m; }
+inline uint64_t gcd64(uint64_t a, uint64_t b) { while (b) { uint64_t t = a % b; a = b; b = t; } return a; }
+
+struct Range {
+    aa_dm_range r{};
+    uint64_t nout = 0;          // valid output samples (binned)
+    int32_t maxdelay = 0;       // binned samples
+    uint32_t dm_base = 0;
+    std::vector<int32_t> h_delays;   // [ndms][nchans]
+    int32_t *d_delays = nullptr;
+    int row = 0;                // staged row length (elements)
+    int dpw = 4;                // DM trials per warp in the dedispersion kernel
+    bool in16 = false;
+    int flush_ch = 2;
+    bool wide = false;          // 64-bit boxcar sums
+    int bin_slot = -1;          // index into the per-stream binned buffers
+    std::vector<std::pair<int, int>> taps;   // (local dm, tap row)
+};
+
+constexpr int kEvFixed = 7;     // h2d0 h2d1 ct1 bin0 bin1 list0 list1
+
+struct Stream {
+    cudaStream_t st = nullptr;
+    bool own = false;
+    uint8_t *d_raw = nullptr;
+    std::vector<uint16_t *> d_binned;
+    uint32_t *d_D = nullptr;
+    aa_candidate *d_cands = nullptr;
+    uint32_t *d_count = nullptr;
+    uint32_t *h_count = nullptr;      // pinned
+    aa_candidate *h_cands = nullptr;  // pinned
+    uint32_t *h_tap = nullptr;        // pinned
+    std::vector<cudaEvent_t> ev;      // timing events
+    // per-run accumulators
+    double h2d_ms = 0, d2h_ms = 0, prep_ms = 0, dedisp_ms = 0, sps_ms = 0;
+    uint64_t h2d_bytes = 0, d2h_bytes = 0, dedisp_launches = 0, sps_launches = 0, prep_launches = 0;
+};
+
+}  // namespace
+
+struct aa_plan {
+    aa_plan_desc desc{};
+    std::vector<aa_dm_range> ranges_in;
+    std::vector<int32_t> widths;
+    std::vector<uint32_t> taps_in;
+    std::vector<Range> ranges;
+    std::vector<int> bins;            // distinct bins > 1
+    WidthTable wt{};
+    int wmax = 1;
+    uint64_t maxshift = 0, t_valid = 0, halo = 0, L = 0, n_sub = 0, ring_len = 0, ring_pitch = 0;
+    uint64_t pitchD = 0, d_rows = 0, cap = 0, tap_row_len = 0, tap_stage_elems = 0;
+    std::vector<uint64_t> pitch_b;
+    uint32_t norm_block = 65536;
+    int n_streams = 1;
+    uint64_t arena_bytes = 0, pinned_bytes = 0;
+    void *arena = nullptr;
+    bool own_arena = false;
+    uint8_t *d_ring = nullptr;
+    std::vector<Stream> streams;
+    std::vector<cudaEvent_t> ev_loaded;
+    std::unique_ptr<std::atomic<int>[]> loaded, done;
+    std::atomic<int> error{0};
+    std::atomic<uint64_t> out_pos{0}, total{0};
+    std::atomic<int> overflow{0};
+    aa_stats stats{};
+};
+
+namespace {
+
+#define AA_CUDA(call)                                   \
+    do {                                                \
+        cudaError_t e_ = (call);                        \
+        if (e_ != cudaSuccess) {                        \
+            g_last_cuda_error = (int)e_;                \
+            return AA_ERR_CUDA;                         \
+        }                                               \
+    } while (0)
+
+// Builds everything that depends only on the descriptor: validation, delay tables, geometry,
+// buffer sizes.  Fills `p` (no CUDA calls).  Returns aa_status.
+int build_geometry(aa_plan &p, const aa_plan_desc *d)
+{
+    if (!d || d->nchans < 1 || d->nsamp < 1 || !(d->tsamp > 0) || !(d->f_top > 0) || !(d->foff < 0))
+        return AA_ERR_INVALID;
+    if (!(d->f_top + (d->nchans - 1) * d->foff > 0)) return AA_ERR_INVALID;
+    if (d->nranges < 1 || !d->ranges || d->nwidths < 1 || d->nwidths > kMaxWidths || !d->widths)
+        return AA_ERR_INVALID;
+    if (d->n_streams < 1 || d->n_streams > 64 || d->chunk_len < 1) return AA_ERR_INVALID;
+    if (d->ntap < 0 || (d->ntap > 0 && !d->tap_dm_indices)) return AA_ERR_INVALID;
+    if (d->nsamp > 0xFFFFFFFFull) return AA_ERR_INVALID;       // candidates carry 32-bit sample indices
+
+    p.desc = *d;
+    p.ranges_in.assign(d->ranges, d->ranges + d->nranges);
+    p.widths.assign(d->widths, d->widths + d->nwidths);
+    p.taps_in.assign(d->tap_dm_indices, d->tap_dm_indices + d->ntap);
+    p.desc.ranges = p.ranges_in.data();
+    p.desc.widths = p.widths.data();
+    p.desc.tap_dm_indices = p.taps_in.data();
+    p.n_streams = d->n_streams;
+    p.norm_block = d->norm_block ? d->norm_block : 65536u;
+
+    for (int j = 0; j < d->nwidths; ++j) {
+        if (p.widths[j] < 1 || (j && p.widths[j] <= p.widths[j - 1])) return AA_ERR_INVALID;
+        p.wt.w[j] = p.widths[j];
+    }
+    p.wmax = p.widths.back();
+    if (p.wmax > 4096) return AA_ERR_INVALID;
+
+    uint64_t lcm = 1;
+    int bin_max = 1;
+    for (auto &r : p.ranges_in) {
+        if (r.ndms < 1 || r.ndms > 65535 || r.bin < 1 || r.bin > 128 || !(r.dm_step >= 0) || !(r.dm_low >= 0))
+            return AA_ERR_INVALID;
+        if (p.norm_block % r.bin) return AA_ERR_INVALID;
+        if (255ull * d->nchans * r.bin >= (1ull << 32)) return AA_ERR_INVALID;
+        lcm = lcm / gcd64(lcm, r.bin) * r.bin;
+        bin_max = std::max(bin_max, r.bin);
+    }
+    if (p.norm_block % kAlign || p.norm_block % lcm) return AA_ERR_INVALID;
+    // exact 64-bit sum of squares per block: norm_block*bin*(255*nchans)^2 < 2^63
+    {
+        long double bound = (long double)p.norm_block * bin_max * 255.0L * 255.0L * d->nchans * d->nchans;
+        if (bound >= 9.2e18L) return AA_ERR_INVALID;
+    }
+
+    // delay tables: delta(c,i) = floor(((4.148808e3*DM_i)*(1/f_c^2 - 1/f_top^2))/(tsamp*bin) + 0.5)
+    // in double, each operation rounded separately (north_star).
+    p.ranges.resize(d->nranges);
+    uint32_t base = 0;
+    p.maxshift = 0;
+    std::vector<double> g(d->nchans);
+    for (int c = 0; c < d->nchans; ++c) {
+        const double f = d->f_top + (double)c * d->foff;
+        const double a = 1.0 / (f * f);
+        const double b = 1.0 / (d->f_top * d->f_top);
+        g[c] = a - b;
+    }
+    for (int ri = 0; ri < d->nranges; ++ri) {
+        Range &R = p.ranges[ri];
+        R.r = p.ranges_in[ri];
+        R.dm_base = base;
+        base += (uint32_t)R.r.ndms;
+        R.h_delays.resize((size_t)R.r.ndms * d->nchans);
+        const double ts = d->tsamp * (double)R.r.bin;
+        int64_t mx = 0;
+        for (int i = 0; i < R.r.ndms; ++i) {
+            const double prod = (double)i * R.r.dm_step;
+            const double dm = R.r.dm_low + prod;
+            const double kdm = 4.148808e3 * dm;
+            for (int c = 0; c < d->nchans; ++c) {
+                const double num = kdm * g[c];
+                const double v = num / ts;
+                const double rounded = std::floor(v + 0.5);
+                if (!(rounded >= 0) || rounded > 1.0e9) return AA_ERR_INVALID;
+                R.h_delays[(size_t)i * d->nchans + c] = (int32_t)rounded;
+                mx = std::max<int64_t>(mx, (int64_t)rounded);
+            }
+        }
+        R.maxdelay = (int32_t)mx;
+        p.maxshift = std::max<uint64_t>(p.maxshift, (uint64_t)mx * R.r.bin);
+    }
+    p.maxshift = round_up(p.maxshift, lcm);
+    if (p.maxshift >= d->nsamp) return AA_ERR_INVALID;
+    p.t_valid = d->nsamp - p.maxshift;
+
+    p.halo = round_up(p.maxshift + (uint64_t)(p.wmax - 1) * bin_max, std::max<uint64_t>(lcm, kAlign));
+    if (d->chunk_len % d->n_streams) return AA_ERR_INVALID;
+    p.L = d->chunk_len / d->n_streams;
+    if (p.L % p.norm_block || p.L < p.halo) return AA_ERR_INVALID;
+    p.n_sub = (p.t_valid + p.L - 1) / p.L;
+    const uint64_t n_slots = std::min<uint64_t>((uint64_t)p.n_streams + 1, p.n_sub + 1);
+    p.ring_len = n_slots * p.L;
+
+    // taps
+    for (int k = 0; k < d->ntap; ++k) {
+        const uint32_t gi = p.taps_in[k];
+        if (k && gi <= p.taps_in[k - 1]) return AA_ERR_INVALID;
+        bool found = false;
+        for (auto &R : p.ranges)
+            if (gi >= R.dm_base && gi < R.dm_base + (uint32_t)R.r.ndms) {
+                R.taps.emplace_back((int)(gi - R.dm_base), k);
+                found = true;
+            }
+        if (!found) return AA_ERR_INVALID;
+    }
+
+    // per-range kernel configuration
+    p.bins.clear();
+    int max_row_u8 = 0;
+    p.d_rows = 0;
+    uint64_t max_cols = 0;
+    p.tap_row_len = 0;
+    p.tap_stage_elems = 0;
+    for (auto &R : p.ranges) {
+        R.nout = p.t_valid / R.r.bin;
+        R.in16 = R.r.bin > 1;
+        R.flush_ch = (int)((65535 / (255 * R.r.bin)) & ~1);
+        if (R.flush_ch < 2) return AA_ERR_INVALID;
+        R.wide = 255ull * d->nchans * R.r.bin * p.wmax >= (1ull << 32);
+        if (R.in16) {
+            auto it = std::find(p.bins.begin(), p.bins.end(), R.r.bin);
+            if (it == p.bins.end()) { p.bins.push_back(R.r.bin); R.bin_slot = (int)p.bins.size() - 1; }
+            else R.bin_slot = (int)(it - p.bins.begin());
+        }
+        // largest delay spread inside a block of DB trials decides the staged row length
+        bool ok = false;
+        for (int dpw : {4, 2, 1}) {
+            const int DB = dpw * (kDedispThreads / 32);
+            int spread = 0;
+            for (int d0 = 0; d0 < R.r.ndms; d0 += DB) {
+                const int d1 = std::min(d0 + DB, R.r.ndms) - 1;
+                const int32_t *a = &R.h_delays[(size_t)d0 * d->nchans];
+                const int32_t *b = &R.h_delays[(size_t)d1 * d->nchans];
+                for (int c = 0; c < d->nchans; ++c) spread = std::max(spread, b[c] - a[c]);
+            }
+            const int row = (int)round_up((uint64_t)kDedispTB + spread + kAlign + 1, 16);
+            if (dedisp_smem_bytes(R.in16, dpw, row) <= 110 * 1024 || (dpw == 1 && dedisp_smem_bytes(R.in16, dpw, row) <= 227 * 1024)) {
+                R.dpw = dpw; R.row = row; ok = true;
+                break;
+            }
+        }
+        if (!ok) return AA_ERR_INVALID;     // DM step too coarse for the staged window
+        if (!R.in16) max_row_u8 = std::max(max_row_u8, R.row);
+        p.d_rows = std::max<uint64_t>(p.d_rows, (uint64_t)R.r.ndms);
+        max_cols = std::max<uint64_t>(max_cols, p.L / R.r.bin + p.wmax - 1);
+        if (!R.taps.empty()) {
+            p.tap_row_len = std::max<uint64_t>(p.tap_row_len, R.nout);
+            p.tap_stage_elems += (uint64_t)R.taps.size() * (p.L / R.r.bin);
+        }
+    }
+    p.pitchD = round_up(max_cols + 8, 64);
+    p.ring_pitch = round_up(p.ring_len + p.halo + (uint64_t)max_row_u8 + kDedispTB + 64, 256);
+    p.pitch_b.resize(p.bins.size());
+    for (size_t k = 0; k < p.bins.size(); ++k) {
+        int max_row = 0;
+        for (auto &R : p.ranges) if (R.bin_slot == (int)k) max_row = std::max(max_row, R.row);
+        p.pitch_b[k] = round_up((p.L + p.halo) / p.bins[k] + max_row + kDedispTB + 64, 128);
+    }
+    p.cap = d->max_cands_per_subchunk ? d->max_cands_per_subchunk : (1ull << 21);
+    if (p.cap > (1ull << 30)) return AA_ERR_INVALID;
+
+    // arena layout (256-byte aligned bump allocation, computed identically in carve())
+    uint64_t off = 0;
+    auto take = [&](uint64_t bytes) { off = round_up(off, 256) + bytes; };
+    take((uint64_t)d->nchans * p.ring_pitch);
+    for (auto &R : p.ranges) take((uint64_t)R.r.ndms * d->nchans * 4);
+    for (int s = 0; s < p.n_streams; ++s) {
+        take((p.L + p.halo) * (uint64_t)d->nchans);
+        for (size_t k = 0; k < p.bins.size(); ++k) take((uint64_t)d->nchans * p.pitch_b[k] * 2);
+        take(p.d_rows * p.pitchD * 4);
+        take(p.cap * sizeof(aa_candidate));
+        take(256);
+    }
+    p.arena_bytes = round_up(off, 256);
+    p.pinned_bytes = (uint64_t)p.n_streams * (256 + p.cap * sizeof(aa_candidate) + p.tap_stage_elems * 4);
+    return AA_OK;
+}
+
+void carve(aa_plan &p)
+{
+    uint8_t *base = static_cast<uint8_t *>(p.arena);
+    uint64_t off = 0;
+    auto take = [&](uint64_t bytes) { off = round_up(off, 256); uint8_t *q = base + off; off += bytes; return q; };
+    const int nchans = p.desc.nchans;
+    p.d_ring = take((uint64_t)nchans * p.ring_pitch);
+    for (auto &R : p.ranges) R.d_delays = reinterpret_cast<int32_t *>(take((uint64_t)R.r.ndms * nchans * 4));
+    for (auto &S : p.streams) {
+        S.d_raw = take((p.L + p.halo) * (uint64_t)nchans);
+        S.d_binned.resize(p.bins.size());
+        for (size_t k = 0; k < p.bins.size(); ++k)
+            S.d_binned[k] = reinterpret_cast<uint16_t *>(take((uint64_t)nchans * p.pitch_b[k] * 2));
+        S.d_D = reinterpret_cast<uint32_t *>(take(p.d_rows * p.pitchD * 4));
+        S.d_cands = reinterpret_cast<aa_candidate *>(take(p.cap * sizeof(aa_candidate)));
+        S.d_count = reinterpret_cast<uint32_t *>(take(256));
+    }
+}
+
+void destroy_plan(aa_plan *p)
+{
+    if (!p) return;
+    for (auto &S : p->streams) {
+        if (S.st) cudaStreamSynchronize(S.st);
+        for (auto e : S.ev) if (e) cudaEventDestroy(e);
+        if (S.h_count) cudaFreeHost(S.h_count);
+        if (S.h_cands) cudaFreeHost(S.h_cands);
+        if (S.h_tap) cudaFreeHost(S.h_tap);
+        if (S.own && S.st) cudaStreamDestroy(S.st);
+    }
+    for (auto e : p->ev_loaded) if (e) cudaEventDestroy(e);
+    if (p->own_arena && p->arena) cudaFree(p->arena);
+    delete p;
+}
+
+inline bool wait_flag(aa_plan *p, std::atomic<int> &f)
+{
+    int spins = 0;
+    while (!f.load(std::memory_order_acquire)) {
+        if (p->error.load(std::memory_order_relaxed)) return false;
+        if (++spins < 200) std::this_thread::yield();
+        else std::this_thread::sleep_for(std::chrono::microseconds(20));
+    }
+    return true;
+}
+
+#define AA_W(call)                                                       \
+    do {                                                                 \
+        cudaError_t e_ = (call);                                         \
+        if (e_ != cudaSuccess) {                                         \
+            int z_ = 0;                                                  \
+            p->error.compare_exchange_strong(z_, (int)e_);               \
+            return;                                                      \
+        }                                                                \
+    } while (0)
+
+// One stream's host thread: issues every sub-chunk j = s, s+n_streams, ... and copies its results out.
+void worker(aa_plan *p, int s, const uint8_t *input, bool resident, aa_candidate *out, uint64_t max_cands,
+            uint32_t *tap_out)
+{
+    Stream &S = p->streams[s];
+    cudaStream_t st = S.st;
+    const uint64_t L = p->L, halo = p->halo, R = p->ring_len, nsamp = p->desc.nsamp;
+    const int nchans = p->desc.nchans;
+    const int nr = (int)p->ranges.size();
+
+    for (uint64_t j = (uint64_t)s; j < p->n_sub; j += (uint64_t)p->n_streams) {
+        // the new rows overwrite ring columns last read by sub-chunks j-n_streams-1 and j-n_streams
+        if (j >= (uint64_t)p->n_streams + 1 && !wait_flag(p, p->done[j - p->n_streams - 1])) return;
+
+        const uint64_t t_first = j == 0 ? 0 : j * L + halo;
+        const uint64_t t_last = std::min<uint64_t>((j + 1) * L + halo, nsamp);
+        const uint64_t nt = t_last > t_first ? t_last - t_first : 0;
+        const uint8_t *src = input + t_first * (uint64_t)nchans;
+
+        AA_W(cudaEventRecord(S.ev[0], st));
+        if (!resident && nt) {
+            AA_W(cudaMemcpyAsync(S.d_raw, src, nt * (uint64_t)nchans, cudaMemcpyHostToDevice, st));
+            S.h2d_bytes += nt * (uint64_t)nchans;
+            src = S.d_raw;
+        }
+        AA_W(cudaEventRecord(S.ev[1], st));
+        AA_W(launch_corner_turn(src, (int64_t)nt, nchans, (int64_t)t_first, p->d_ring, (int64_t)p->ring_pitch,
+                                (int64_t)R, (int64_t)halo, st));
+        S.prep_launches += nt ? 1 : 0;
+        AA_W(cudaEventRecord(S.ev[2], st));
+        AA_W(cudaEventRecord(p->ev_loaded[j], st));
+        p->loaded[j].store(1, std::memory_order_release);
+
+        // the window [jL, (j+1)L + halo) also needs the rows loaded by sub-chunk j-1's stream
+        if (j > 0) {
+            if (!wait_flag(p, p->loaded[j - 1])) return;
+            AA_W(cudaStreamWaitEvent(st, p->ev_loaded[j - 1], 0));
+        }
+        const uint64_t col0 = (j * L) % R;
+        const uint64_t in_len = std::min<uint64_t>(L + halo, nsamp - j * L);
+
+        AA_W(cudaEventRecord(S.ev[3], st));
+        for (size_t k = 0; k < p->bins.size(); ++k) {
+            AA_W(launch_bin(p->d_ring, (int64_t)p->ring_pitch, (int64_t)col0, nchans, p->bins[k],
+                            (int64_t)(in_len / p->bins[k]), S.d_binned[k], (int64_t)p->pitch_b[k], st));
+            S.prep_launches++;
+        }
+        AA_W(cudaEventRecord(S.ev[4], st));
+        AA_W(cudaMemsetAsync(S.d_count, 0, sizeof(uint32_t), st));
+
+        uint64_t tap_off = 0;
+        struct TapCopy { int row; uint64_t tau0, n, off; };
+        std::vector<TapCopy> tapcopies;
+        for (int ri = 0; ri < nr; ++ri) {
+            Range &Rg = p->ranges[ri];
+            const uint64_t b = (uint64_t)Rg.r.bin;
+            const uint64_t tau0 = j * L / b;
+            cudaEvent_t e0 = S.ev[kEvFixed + 3 * ri], e1 = S.ev[kEvFixed + 3 * ri + 1], e2 = S.ev[kEvFixed + 3 * ri + 2];
+            AA_W(cudaEventRecord(e0, st));
+            if (tau0 < Rg.nout) {
+                const uint64_t left = Rg.nout - tau0;
+                const uint64_t nemit = std::min<uint64_t>(L / b, left);
+                const uint64_t ncols = std::min<uint64_t>(L / b + p->wmax - 1, left);
+                DedispArgs da{};
+                da.in = Rg.in16 ? (const void *)S.d_binned[Rg.bin_slot] : (const void *)p->d_ring;
+                da.pitch_in = Rg.in16 ? (int64_t)p->pitch_b[Rg.bin_slot] : (int64_t)p->ring_pitch;
+                da.col0 = Rg.in16 ? 0 : (int64_t)col0;
+                da.delays = Rg.d_delays;
+                da.nchans = nchans;
+                da.ndms = Rg.r.ndms;
+                da.ncols = (int32_t)ncols;
+                da.out = S.d_D;
+                da.pitch_out = (int64_t)p->pitchD;
+                da.row = Rg.row;
+                da.flush_ch = Rg.flush_ch;
+                AA_W(launch_dedisp(da, Rg.in16, Rg.dpw, st));
+                S.dedisp_launches++;
+                AA_W(cudaEventRecord(e1, st));
+                SpsArgs sa{};
+                sa.D = S.d_D;
+                sa.pitch = (int64_t)p->pitchD;
+                sa.ndms = Rg.r.ndms;
+                sa.ncols = (int32_t)ncols;
+                sa.nemit = (int32_t)nemit;
+                sa.nout_left = (int64_t)left;
+                sa.block_len = (int32_t)(p->norm_block / b);
+                sa.nwidths = (int32_t)p->widths.size();
+                sa.wmax = p->wmax;
+                sa.thr = p->desc.snr_threshold;
+                sa.dm_base = Rg.dm_base;
+                sa.tau0 = (uint32_t)tau0;
+                sa.bin = (uint32_t)b;
+                sa.cands = S.d_cands;
+                sa.count = S.d_count;
+                sa.cap = (uint32_t)p->cap;
+                AA_W(launch_sps(sa, p->wt, Rg.wide, st));
+                S.sps_launches++;
+                AA_W(cudaEventRecord(e2, st));
+                for (auto &tp : Rg.taps) {
+                    AA_W(cudaMemcpyAsync(S.h_tap + tap_off, S.d_D + (uint64_t)tp.first * p->pitchD, nemit * 4,
+                                         cudaMemcpyDeviceToHost, st));
+                    tapcopies.push_back({tp.second, tau0, nemit, tap_off});
+                    tap_off += nemit;
+                    S.d2h_bytes += nemit * 4;
+                }
+            } else {
+                AA_W(cudaEventRecord(e1, st));
+                AA_W(cudaEventRecord(e2, st));
+            }
+        }
+        AA_W(cudaMemcpyAsync(S.h_count, S.d_count, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+        AA_W(cudaStreamSynchronize(st));           // stream-scoped wait, never device-wide
+        p->done[j].store(1, std::memory_order_release);
+
+        const uint64_t found = *S.h_count;
+        const uint64_t n = std::min<uint64_t>(found, p->cap);
+        if (found > p->cap) p->overflow.store(1);
+        AA_W(cudaEventRecord(S.ev[5], st));
+        if (n) AA_W(cudaMemcpyAsync(S.h_cands, S.d_cands, n * sizeof(aa_candidate), cudaMemcpyDeviceToHost, st));
+        AA_W(cudaEventRecord(S.ev[6], st));
+        AA_W(cudaStreamSynchronize(st));
+        S.d2h_bytes += 4 + n * sizeof(aa_candidate);
+
+        // host-to-host output stage of this stream
+        p->total.fetch_add(found);
+        const uint64_t pos = p->out_pos.fetch_add(n);
+        if (pos < max_cands) {
+            const uint64_t m = std::min<uint64_t>(n, max_cands - pos);
+            if (m) std::memcpy(out + pos, S.h_cands, m * sizeof(aa_candidate));
+        }
+        if (tap_out)
+            for (auto &tc : tapcopies)
+                std::memcpy(tap_out + (uint64_t)tc.row * p->tap_row_len + tc.tau0, S.h_tap + tc.off, tc.n * 4);
+
+        float ms = 0;
+        if (!resident && nt) { cudaEventElapsedTime(&ms, S.ev[0], S.ev[1]); S.h2d_ms += ms; }
+        cudaEventElapsedTime(&ms, S.ev[1], S.ev[2]); S.prep_ms += ms;
+        cudaEventElapsedTime(&ms, S.ev[3], S.ev[4]); S.prep_ms += ms;
+        for (int ri = 0; ri < nr; ++ri) {
+            cudaEventElapsedTime(&ms, S.ev[kEvFixed + 3 * ri], S.ev[kEvFixed + 3 * ri + 1]); S.dedisp_ms += ms;
+            cudaEventElapsedTime(&ms, S.ev[kEvFixed + 3 * ri + 1], S.ev[kEvFixed + 3 * ri + 2]); S.sps_ms += ms;
+        }
+        cudaEventElapsedTime(&ms, S.ev[5], S.ev[6]); S.d2h_ms += ms;
+    }
+}
+
+int run_impl(aa_plan *p, const uint8_t *input, bool resident, aa_candidate *out, uint64_t max_cands,
+             uint64_t *n_cands, uint32_t *tap_out)
+{
+    if (!p || !input || !n_cands || (!out && max_cands)) return AA_ERR_INVALID;
+    if (tap_out && p->taps_in.empty()) return AA_ERR_INVALID;
+    g_last_cuda_error = 0;
+    cudaPointerAttributes at{};
+    cudaError_t pe = cudaPointerGetAttributes(&at, input);
+    if (pe != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
+    if (resident) {
+        if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) return AA_ERR_INVALID;
+    } else if (at.type != cudaMemoryTypeHost) {
+        return AA_ERR_NOT_PINNED;                   // never staged through pageable memory silently
+    }
+
+    const auto t0 = std::chrono::steady_clock::now();
+    for (uint64_t j = 0; j < p->n_sub; ++j) { p->loaded[j].store(0); p->done[j].store(0); }
+    p->error.store(0); p->out_pos.store(0); p->total.store(0); p->overflow.store(0);
+    for (auto &S : p->streams) {
+        S.h2d_ms = S.d2h_ms = S.prep_ms = S.dedisp_ms = S.sps_ms = 0;
+        S.h2d_bytes = S.d2h_bytes = S.dedisp_launches = S.sps_launches = S.prep_launches = 0;
+    }
+    const int nthreads = (int)std::min<uint64_t>((uint64_t)p->n_streams, p->n_sub);
+    std::vector<std::thread> th;
+    for (int s = 1; s < nthreads; ++s) th.emplace_back(worker, p, s, input, resident, out, max_cands, tap_out);
+    worker(p, 0, input, resident, out, max_cands, tap_out);
+    for (auto &t : th) t.join();
+    if (p->error.load()) {
+        for (auto &S : p->streams) cudaStreamSynchronize(S.st);
+        g_last_cuda_error = p->error.load();
+        return AA_ERR_CUDA;
+    }
+
+    const uint64_t total = p->total.load();
+    const uint64_t stored = std::min<uint64_t>(p->out_pos.load(), max_cands);
+    const auto t1 = std::chrono::steady_clock::now();
+    std::sort(out, out + stored, [](const aa_candidate &a, const aa_candidate &b) {
+        return a.dm_index != b.dm_index ? a.dm_index < b.dm_index : a.t_start < b.t_start;
+    });
+    const auto t2 = std::chrono::steady_clock::now();
+    *n_cands = total;
+
+    aa_stats &st = p->stats;
+    st = aa_stats{};
+    st.wall_ms = std::chrono::duration<double, std::milli>(t2 - t0).count();
+    st.sort_ms = std::chrono::duration<double, std::milli>(t2 - t1).count();
+    for (auto &S : p->streams) {
+        st.h2d_bytes += S.h2d_bytes; st.d2h_bytes += S.d2h_bytes;
+        st.h2d_ms += S.h2d_ms; st.d2h_ms += S.d2h_ms; st.prep_ms += S.prep_ms;
+        st.dedisp_ms += S.dedisp_ms; st.sps_ms += S.sps_ms;
+        st.dedisp_launches += S.dedisp_launches; st.sps_launches += S.sps_launches;
+        st.prep_launches += S.prep_launches;
+    }
+    st.n_candidates = total;
+    st.n_stored = stored;
+    st.overflow = (p->overflow.load() || total > max_cands) ? 1 : 0;
+    st.n_streams = p->n_streams;
+    return st.overflow ? AA_ERR_OVERFLOW : AA_OK;
+}
+
+}  // namespace
+
+// ---------------------------------------------------------------------------------------------
+extern "C" {
+
+uint64_t aa_plan_arena_bytes(const aa_plan_desc *d)
+{
+    aa_plan tmp;
+    if (build_geometry(tmp, d) != AA_OK) return 0;
+    return tmp.arena_bytes;
+}
+
+int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
+{
+    if (!out) return AA_ERR_INVALID;
+    *out = nullptr;
+    g_last_cuda_error = 0;
+    aa_plan *p = new (std::nothrow) aa_plan;
+    if (!p) return AA_ERR_OOM;
+    int rc = build_geometry(*p, d);
+    if (rc != AA_OK) { delete p; return rc; }
+
+    auto fail = [&](int code, cudaError_t e) { g_last_cuda_error = (int)e; destroy_plan(p); return code; };
+    cudaError_t e;
+    if ((e = dedisp_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
+    if ((e = sps_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
+
+    if (d->device_arena) {
+        if (d->device_arena_bytes < p->arena_bytes || ((uintptr_t)d->device_arena & 255)) return fail(AA_ERR_INVALID, cudaSuccess);
+        p->arena = d->device_arena;
+    } else {
+        if ((e = cudaMalloc(&p->arena, p->arena_bytes)) != cudaSuccess) { cudaGetLastError(); return fail(AA_ERR_OOM, e); }
+        p->own_arena = true;
+    }
+    p->streams.resize(p->n_streams);
+    for (int s = 0; s < p->n_streams; ++s) {
+        Stream &S = p->streams[s];
+        if (d->streams) S.st = static_cast<cudaStream_t>(d->streams[s]);
+        else {
+            if ((e = cudaStreamCreateWithFlags(&S.st, cudaStreamNonBlocking)) != cudaSuccess) return fail(AA_ERR_CUDA, e);
+            S.own = true;
+        }
+        S.ev.assign(kEvFixed + 3 * p->ranges.size(), nullptr);
+        for (auto &ev : S.ev) if ((e = cudaEventCreate(&ev)) != cudaSuccess) return fail(AA_ERR_CUDA, e);
+        if ((e = cudaHostAlloc((void **)&S.h_count, 256, cudaHostAllocDefault)) != cudaSuccess) { cudaGetLastError(); return fail(AA_ERR_OOM, e); }
+        if ((e = cudaHostAlloc((void **)&S.h_cands, p->cap * sizeof(aa_candidate), cudaHostAllocDefault)) != cudaSuccess) { cudaGetLastError(); return fail(AA_ERR_OOM, e); }
+        if (p->tap_stage_elems)
+            if ((e = cudaHostAlloc((void **)&S.h_tap, p->tap_stage_elems * 4, cudaHostAllocDefault)) != cudaSuccess) { cudaGetLastError(); return fail(AA_ERR_OOM, e); }
+    }
+    carve(*p);
+    p->ev_loaded.assign(p->n_sub, nullptr);
+    for (auto &ev : p->ev_loaded)
+        if ((e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess) return fail(AA_ERR_CUDA, e);
+    p->loaded.reset(new std::atomic<int>[p->n_sub]);
+    p->done.reset(new std::atomic<int>[p->n_sub]);
+    for (auto &R : p->ranges) {
+        if ((e = cudaMemcpy(R.d_delays, R.h_delays.data(), R.h_delays.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess)
+            return fail(AA_ERR_CUDA, e);
+    }
+    *out = p;
+    return AA_OK;
+}
+
+int aa_plan_query(const aa_plan *p, aa_plan_info *o)
+{
+    if (!p || !o) return AA_ERR_INVALID;
+    o->maxshift = p->maxshift; o->t_valid = p->t_valid; o->halo = p->halo; o->subchunk_len = p->L;
+    o->n_subchunks = p->n_sub;
+    o->ndms_total = 0; o->dm_trial_samples = 0;
+    for (auto &R : p->ranges) { o->ndms_total += (uint64_t)R.r.ndms; o->dm_trial_samples += (uint64_t)R.r.ndms * R.nout; }
+    o->arena_bytes = p->arena_bytes; o->pinned_bytes = p->pinned_bytes; o->tap_row_len = p->tap_row_len;
+    return AA_OK;
+}
+
+uint64_t aa_plan_nout(const aa_plan *p, int32_t r)
+{
+    if (!p || r < 0 || r >= (int32_t)p->ranges.size()) return 0;
+    return p->ranges[r].nout;
+}
+
+int aa_plan_delays(const aa_plan *p, int32_t r, int32_t *out)
+{
+    if (!p || !out || r < 0 || r >= (int32_t)p->ranges.size()) return AA_ERR_INVALID;
+    const Range &R = p->ranges[r];
+    AA_CUDA(cudaMemcpy(out, R.d_delays, R.h_delays.size() * 4, cudaMemcpyDeviceToHost));
+    return AA_OK;
+}
+
+int aa_run(aa_plan *p, const uint8_t *host_input, aa_candidate *out, uint64_t max_cands, uint64_t *n_cands,
+           uint32_t *tap_out)
+{
+    return run_impl(p, host_input, false, out, max_cands, n_cands, tap_out);
+}
+
+int aa_run_resident(aa_plan *p, const uint8_t *device_input, aa_candidate *out, uint64_t max_cands,
+                    uint64_t *n_cands, uint32_t *tap_out)
+{
+    return run_impl(p, device_input, true, out, max_cands, n_cands, tap_out);
+}
+
+int aa_get_stats(const aa_plan *p, aa_stats *out)
+{
+    if (!p || !out) return AA_ERR_INVALID;
+    *out = p->stats;
+    return AA_OK;
+}
+
+void aa_destroy(aa_plan *p) { destroy_plan(p); }
+
+int aa_host_alloc(void **ptr, uint64_t bytes)
+{
+    if (!ptr) return AA_ERR_INVALID;
+    *ptr = nullptr;
+    cudaError_t e = cudaHostAlloc(ptr, bytes, cudaHostAllocDefault);
+    if (e != cudaSuccess) { cudaGetLastError(); g_last_cuda_error = (int)e; return AA_ERR_OOM; }
+    return AA_OK;
+}
+
+void aa_host_free(void *ptr) { if (ptr) cudaFreeHost(ptr); }
+
+const char *aa_strerror(int s)
+{
+    switch (s) {
+        case AA_OK: return "ok";
+        case AA_ERR_INVALID: return "invalid argument or inconsistent plan descriptor";
+        case AA_ERR_NOT_PINNED: return "input buffer is not pinned host memory";
+        case AA_ERR_OOM: return "out of device or pinned memory";
+        case AA_ERR_CUDA: return "CUDA call failed (see aa_last_cuda_error)";
+        case AA_ERR_OVERFLOW: return "candidate buffer overflow (list truncated)";
+        default: return "unknown status";
+    }
+}
+
+int aa_last_cuda_error(void) { return g_last_cuda_error; }
+
+}  // extern "C"

@@ -1,0 +1,131 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element."""
+import numpy as np
+import pytest
+
+import oracle
+from paper_2101_00941_b200 import inputs as I
+from _compare import compare_candidates
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2101_00941_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def _pinned_fill(B, w):
+    buf = B.pinned_empty(w.nbytes)
+    x = buf.numpy().reshape(w.nsamp, w.nchans)
+    I.fill(w, x)
+    return buf, x
+
+
+def _run_gpu(B, w, buf, *, taps="all", **kw):
+    tap_list = list(range(w.ndms_total)) if taps == "all" else taps
+    with B.Plan(w, taps=tap_list, **kw) as plan:
+        cands, tap = plan.run(buf)
+        assert not plan.overflow
+        return cands, tap, plan.info, plan.nout, plan.stats()
+
+
+def _check_against_oracle(B, w, **kw):
+    buf, x = _pinned_fill(B, w)
+    cands, tap, info, nout, _ = _run_gpu(B, w, buf, **kw)
+    ref, dense, geo = oracle.run(x, w, keep_dense=True)
+    assert info["maxshift"] == geo["maxshift"] and nout == geo["nout"]
+    base = 0
+    for r, rg in enumerate(w.ranges):
+        got = tap[base:base + rg.ndms, :geo["nout"][r]]
+        assert np.array_equal(got, dense[r]), f"dedispersed series differ in range {r}"
+        base += rg.ndms
+    res = compare_candidates(cands, ref, w.snr_threshold)
+    return cands, ref, res
+
+
+def _tiny(nchans=16, nsamp=20000, bins=(1,), ndms=40, dm_step=3.0, widths=(1, 2, 4, 8), thr=5.0,
+          norm_block=1024, n_streams=1, chunk_len=4096, seed=0, f_top=1500.0, foff=-4.0):
+    ranges, lo = [], 0.0
+    for b in bins:
+        ranges.append(I.DMRange(lo, dm_step, ndms, b))
+        lo += dm_step * ndms
+    w = I.Workload(name="tiny", nchans=nchans, nsamp=nsamp, tsamp=64e-6, f_top=f_top, foff=foff,
+                   ranges=tuple(ranges), widths=tuple(widths), snr_threshold=thr, n_streams=n_streams,
+                   chunk_len=chunk_len, noise_seed=99 + seed,
+                   pulses=(I.Pulse(dm=dm_step * ndms * 0.4, t0=nsamp // 3, width=4, amp=4.0),
+                           I.Pulse(dm=dm_step * ndms * len(bins) * 0.8, t0=nsamp // 2, width=16, amp=2.0)),
+                   norm_block=norm_block)
+    return w
+
+
+def test_delay_tables_match_oracle_entry_by_entry(B):
+    for k in (1, 2, 4):
+        w = I.scaled(I.workload(k), nsamp=1 << 17, chunk_len=1 << 17, n_streams=1, pulses=())
+        with B.Plan(w) as plan:
+            for r in range(len(w.ranges)):
+                assert np.array_equal(plan.delays(r), oracle.delays(w, r).astype(np.int32))
+
+
+@pytest.mark.parametrize("case", [
+    dict(),                                                     # one range, several sub-chunks
+    dict(nchans=24, ndms=37, nsamp=15001),                      # ragged channels / trials / tail
+    dict(bins=(1, 2, 4), nsamp=40000, chunk_len=8192),          # time decimation
+    dict(bins=(8,), nsamp=60000, chunk_len=16384, ndms=20),
+    dict(n_streams=3, chunk_len=3 * 2048, nsamp=30000),         # streams
+    dict(widths=(1, 3, 5, 32), thr=4.0),                        # arbitrary widths
+    dict(nchans=300, nsamp=12000, foff=-0.3, dm_step=4.0, chunk_len=4096, norm_block=2048),  # flushes of the 16-bit lanes
+])
+def test_small_cases_bit_exact(B, case):
+    w = _tiny(**case)
+    cands, ref, res = _check_against_oracle(B, w)
+    assert res["only_gpu"] == 0 and res["only_oracle"] == 0 and res["width_ties"] == 0
+    assert len(ref) > 0
+
+
+def test_cfg1_full(B):
+    w = I.workload(1)
+    cands, ref, res = _check_against_oracle(B, w)
+    top = cands[np.argmax(cands["snr"])]
+    assert (top["dm_index"], top["t_start"], top["width"]) == (50, 40000, 8)
+    assert np.array_equal(cands, ref) or res["max_rel"] <= 1e-5
+
+
+def test_stream_and_chunk_invariance(B):
+    w = I.scaled(I.workload(2), nsamp=1 << 18, name="cfg2_short")
+    buf, x = _pinned_fill(B, w)
+    outs = []
+    for ns, cl in [(1, 1 << 18), (1, 1 << 16), (2, 1 << 17), (4, 1 << 18), (4, 1 << 19)]:
+        cands, tap, _, nout, _ = _run_gpu(B, w, buf, taps=[0, 7, 300, 511], n_streams=ns, chunk_len=cl)
+        outs.append((cands.tobytes(), tap.tobytes()))
+    assert all(o == outs[0] for o in outs[1:])
+
+
+def test_saturated_input_and_constant_input(B):
+    w = _tiny(nchans=300, nsamp=9000, foff=-0.3, dm_step=4.0, chunk_len=4096, norm_block=2048)
+    buf = B.pinned_empty(w.nbytes)
+    x = buf.numpy().reshape(w.nsamp, w.nchans)
+    x[:] = 255                                       # 16-bit lanes at their limit before every flush
+    with B.Plan(w, taps=list(range(w.ndms_total))) as plan:
+        cands, tap = plan.run(buf)
+        assert len(cands) == 0                       # sigma = 0 everywhere
+        assert np.all(tap[:, :plan.nout[0]] == 255 * w.nchans)
+
+
+def test_errors(B):
+    w = _tiny()
+    x = I.fill(w)                                    # pageable
+    with B.Plan(w) as plan:
+        with pytest.raises(B.AAError) as e:
+            plan.run(x)
+        assert e.value.status == B.AA_ERR_NOT_PINNED
+    with pytest.raises(B.AAError):
+        B.Plan(I.scaled(w, chunk_len=1000))          # not a multiple of norm_block
+    with pytest.raises(B.AAError):
+        B.Plan(I.scaled(w, widths=(4, 2)))
+    # candidate overflow is reported, not fatal
+    buf, _ = _pinned_fill(B, I.scaled(w, snr_threshold=1.0))
+    with B.Plan(I.scaled(w, snr_threshold=1.0), max_cands_per_subchunk=64) as plan:
+        cands, _ = plan.run(buf, max_cands=1 << 20)
+        assert plan.overflow and plan.n_found > len(cands)
