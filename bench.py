@@ -1,0 +1,336 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the streamed dedispersion + single-pulse-search path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload 1..5] [--impl ours|reference]
+
+A "step" is one pass of the whole hot path (H2D, corner turn, binning, dedispersion, SPS,
+candidate D2H, host merge) over one synthetic observation.  The default workload is the one
+BASELINE.json's north_star quotes its targets on, configs[2] (SKA-like 4096 channels x 2^23
+samples x 2048 DM trials); the metric is DM-trial*samples/s (plan.dm_trial_samples / time).
+
+  value : inputs already resident in HBM (aa_run_resident), one stream
+  e2e   : aa_run on the pinned HOST buffer, H2D/D2H inside the timed region, n_streams streams
+  roofline : dedispersion kernel, CUDA-event duration of each launch (stream of the launch)
+  cpu_baseline : the oracle, as it stands, on a bounded sample of the same workload
+
+Prints one JSON line (rank 0).  Under torchrun each rank processes its own observation (weak
+scaling, no collective on the data path); the time is the max over ranks.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+from paper_2101_00941_b200 import inputs as I  # noqa: E402
+
+METRIC = "end-to-end DM-trial*samples/s"
+UNIT = "DM-trial*samples/s"
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return p, "measured (MEASURED_PEAKS.json)"
+    return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
+
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.rows = []
+        self.proc = None
+        self.index = index
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(
+                ["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "200"],
+                stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+            self.thread = threading.Thread(target=self._read, daemon=True)
+            self.thread.start()
+        except OSError:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([c.strip() for c in line.split(",")])
+
+    def stop(self):
+        if not self.proc:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.proc.terminate()
+        try:
+            self.proc.wait(timeout=5)
+        except Exception:
+            self.proc.kill()
+        sm, mx, reasons = [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx.append(float(r[1]))
+            except (ValueError, IndexError):
+                continue
+            for n, v in zip(names, r[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+def dist_env():
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    return rank, world, local
+
+
+def pick_workload(k: int, world: int):
+    w = I.workload(k)
+    note = None
+    if world > 1:
+        # weak scaling: every rank searches its own observation; keep N pinned copies within host RAM
+        try:
+            avail = os.sysconf("SC_PHYS_PAGES") * os.sysconf("SC_PAGE_SIZE")
+        except (ValueError, OSError):
+            avail = 0
+        ns = w.nsamp
+        while avail and world * w.nchans * ns * 1.15 > 0.8 * avail and ns > (1 << 21):
+            ns //= 2
+        if ns != w.nsamp:
+            w = I.scaled(w, nsamp=ns, name=w.name + f"_nsamp{ns}")
+            note = f"observation shortened to {ns} samples per rank to fit {world} pinned copies in host RAM"
+    return w, note
+
+
+def cpu_baseline(w, x, budget_rows=48):
+    """The oracle on a bounded sample: `budget_rows` DM trials x one normalisation block."""
+    import oracle
+    geo = oracle.geometry(w)
+    r = 0
+    rg = w.ranges[r]
+    rows = sorted(set(np.linspace(0, rg.ndms - 1, budget_rows).astype(int).tolist()))
+    L = w.norm_block // rg.bin
+    ntau = min(L + max(w.widths) - 1, geo["nout"][r])
+    t0 = time.perf_counter()
+    D = oracle.dedisperse(x, w, r, rows=rows, tau_first=0, ntau=ntau, geo=geo)
+    ncand = 0
+    for k in range(len(rows)):
+        tau, _, _ = oracle.sps_row(D[k], w, r, d_first=0, tau_a=0, tau_b=min(L, geo["nout"][r]), nout=geo["nout"][r])
+        ncand += len(tau)
+    dt = time.perf_counter() - t0
+    units = len(rows) * min(L, geo["nout"][r])
+    return {"value": units / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+            "sample": f"{len(rows)} DM trials x {min(L, geo['nout'][r])} output samples (one normalisation block) "
+                      f"of {w.name}, dedispersion + SPS, {dt:.1f} s", "seconds": dt}
+
+
+def run_reference(args):
+    rank, world, local = dist_env()
+    if rank != 0:
+        return 0
+    w = I.workload(args.workload)
+    # the oracle needs only the rows its sample touches: a short prefix of the observation
+    import oracle
+    geo_full = oracle.geometry(w)
+    need = w.norm_block + max(w.widths) * max(r.bin for r in w.ranges) + geo_full["maxshift"] + 64
+    ws = I.scaled(w, nsamp=min(w.nsamp, int(need)), pulses=w.pulses)
+    x = I.fill(ws)
+    times, val = [], None
+    for i in range(args.warmup + args.steps):
+        cb = cpu_baseline(ws, x, budget_rows=args.ref_rows)
+        if i >= args.warmup:
+            times.append(cb["seconds"]); val = cb
+    units = val["value"] * val["seconds"]
+    v = units * len(times) / sum(times)
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * sum(times) / len(times),
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "u8->u32 sums, f64 S/N",
+            "data": "synthetic", "config": {"workload": w.name, "sample": val["sample"]},
+            "cpu_baseline": {"value": v, "unit": UNIT, "cores": val["cores"], "kind": "oracle", "sample": val["sample"]},
+            "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+    return 0
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=3)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--workload", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--streams", type=int, default=0, help="n_streams of the e2e leg (0: the workload's)")
+    ap.add_argument("--ref-rows", type=int, default=48)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--nsamp", type=int, default=0,
+                    help="shorten the observation (profiling runs under ncu only; not a bench line)")
+    args = ap.parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+
+    import torch
+    from paper_2101_00941_b200 import binding as B
+
+    rank, world, local = dist_env()
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    B.load_library()
+
+    w, note = pick_workload(args.workload, world)
+    if args.nsamp:
+        w = I.scaled(w, nsamp=args.nsamp, name=w.name + f"_nsamp{args.nsamp}")
+        note = "shortened observation for profiling; not a bench line"
+    if world > 1:
+        w = I.scaled(w, noise_seed=w.noise_seed + 1000 * rank)
+    n_streams = args.streams or w.n_streams
+    L = w.chunk_len // w.n_streams                     # sub-chunk length of both legs
+
+    t_gen0 = time.perf_counter()
+    host = B.pinned_empty(w.nbytes)
+    t_pin = time.perf_counter() - t_gen0
+    x = host.numpy().reshape(w.nsamp, w.nchans)
+    I.fill(w, x)
+    t_gen = time.perf_counter() - t_gen0 - t_pin
+
+    def barrier():
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    def timed(fn, steps, warmup):
+        for _ in range(warmup):
+            fn()
+        barrier()
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        e0.record()
+        t0 = time.perf_counter()
+        acc = []
+        for _ in range(steps):
+            fn()
+            acc.append(plan_stats())
+        e1.record()
+        barrier()
+        wall = time.perf_counter() - t0
+        dev = e0.elapsed_time(e1) / 1e3
+        t = max(wall, dev)
+        if world > 1:
+            tt = torch.tensor([t], dtype=torch.float64, device="cuda")
+            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
+            t = float(tt.item())
+        return t, acc
+
+    max_cands = 1 << 24
+    sampler = ClockSampler(local)
+
+    # ---- leg 1: end to end from pinned host memory -------------------------------------------
+    plan = B.Plan(w, n_streams=n_streams, chunk_len=L * n_streams)
+    plan_stats = plan.stats
+    info = plan.info
+    units = info["dm_trial_samples"]
+    last = {}
+
+    def step_e2e():
+        c, _ = plan.run(host, max_cands=max_cands, want_taps=False)
+        last["n"] = len(c)
+
+    sampler.start()
+    t_e2e, st_e2e = timed(step_e2e, args.steps, args.warmup)
+    h2d = st_e2e[-1]["h2d_bytes"]; d2h = st_e2e[-1]["d2h_bytes"]
+    launches_e2e = sum(s["dedisp_launches"] + s["sps_launches"] + s["prep_launches"] for s in st_e2e)
+    n_cands = last["n"]
+    plan.close()
+
+    # ---- leg 2: observation resident in HBM, one stream (kernel-only; per-launch event times) --
+    dev_in = torch.empty(w.nbytes, dtype=torch.uint8, device="cuda")
+    torch.cuda.synchronize()
+    tc0 = time.perf_counter()
+    dev_in.copy_(host, non_blocking=True)
+    torch.cuda.synchronize()
+    t_copy = time.perf_counter() - tc0                 # the transfers alone
+    plan = B.Plan(w, n_streams=1, chunk_len=L)
+    plan_stats = plan.stats
+
+    def step_res():
+        c, _ = plan.run_resident(dev_in, max_cands=max_cands, want_taps=False)
+        last["n_res"] = len(c)
+
+    t_res, st_res = timed(step_res, args.steps, args.warmup)
+    clocks = sampler.stop()
+    plan.close()
+    del dev_in
+
+    # ---- roofline of the dominant kernel (dedispersion) ---------------------------------------
+    pk, pk_src = peaks()
+    d_ms = sum(s["dedisp_ms"] for s in st_res); d_n = sum(s["dedisp_launches"] for s in st_res)
+    s_ms = sum(s["sps_ms"] for s in st_res); p_ms = sum(s["prep_ms"] for s in st_res)
+    wall_ms = sum(s["wall_ms"] for s in st_res)
+    adds_per_step = sum(r.ndms * (info["t_valid"] // r.bin) for r in w.ranges) * w.nchans
+    adds_per_launch = adds_per_step * args.steps / max(d_n, 1)
+    avg_launch_s = d_ms / 1e3 / max(d_n, 1)
+    achieved = adds_per_launch / avg_launch_s / 1e12              # T adds/s
+    sm_mhz = pk.get("sm_max_mhz", 1965.0)
+    peak = 148 * 128 * sm_mhz * 1e6 / 1e12                        # T lane-ops/s
+    roofline = {"kernel": "dedisp_kernel", "bound": "alu", "achieved": achieved, "peak": peak,
+                "unit": "T integer adds/s", "frac": achieved / peak, "traffic": None,
+                "peak_source": f"148 SMs x 128 lanes x {sm_mhz:.0f} MHz ({pk_src}); one add per lane-op",
+                "avg_launch_ms": avg_launch_s * 1e3, "launches": d_n,
+                "share_of_step": {"dedisp": d_ms / wall_ms, "sps": s_ms / wall_ms, "prep": p_ms / wall_ms}}
+
+    if rank == 0:
+        value = world * units * args.steps / t_res
+        e2e_v = world * units * args.steps / t_e2e
+        step_s = t_e2e / args.steps
+        line = {
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": 1e3 * t_res / args.steps, "higher_is_better": True,
+            "scaling": "weak", "vs_baseline": None, "dtype": "u8 input, u32 exact sums, f64 S/N",
+            "data": "synthetic",
+            "config": {"workload": w.name, "nchans": w.nchans, "nsamp": w.nsamp, "ndms": w.ndms_total,
+                       "widths": list(w.widths), "n_streams_e2e": n_streams, "subchunk_len": L,
+                       "chunk_len_e2e": L * n_streams, "l2": "inputs (34 GB) >> L2; no flush needed",
+                       "note": note},
+            "e2e": {"value": e2e_v, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": 1e3 * step_s, "n_streams": n_streams,
+                    "real_time_factor": w.nsamp * w.tsamp / step_s,
+                    "h2d_gbs_effective": h2d / step_s / 1e9,
+                    "transfer_alone_s": t_copy, "kernels_alone_s": t_res / args.steps,
+                    "overlap_efficiency": max(t_copy, t_res / args.steps) / step_s},
+            "gpu_launches": int(launches_e2e),
+            "candidates": n_cands, "clocks": clocks, "roofline": roofline,
+            "setup": {"pin_s": t_pin, "generate_s": t_gen},
+        }
+        if not args.no_cpu_baseline:
+            cb = cpu_baseline(w, x, budget_rows=args.ref_rows)
+            cb.pop("seconds", None)
+            line["cpu_baseline"] = cb
+        print(json.dumps(line))
+    if world > 1:
+        dist.barrier()
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -47,6 +47,7 @@ struct Shared {
     long long bthr[kMaxWidths];
     double den[kMaxWidths];
     unsigned long long warp_tot[NT / 32];
+    int w[kMaxWidths];        // widths (a dynamically indexed kernel parameter would go through the ADU pipe)
 };
 
 template <typename ACC>
@@ -58,6 +59,7 @@ __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const WidthTab
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int d = blockIdx.y;
+    if (tid < kMaxWidths) sh.w[tid] = wt.w[tid];
     const int64_t b0 = (int64_t)blockIdx.x * a.block_len;
     int64_t b1 = b0 + a.block_len;
     if (b1 > a.nout_left) b1 = a.nout_left;
@@ -103,7 +105,7 @@ __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const WidthTab
 
     // ---- 2. per-width constants ---------------------------------------------------------
     if (tid < a.nwidths) {
-        const double w = (double)wt.w[tid];
+        const double w = (double)sh.w[tid];
         const double den = __dmul_rn(sigma, __dsqrt_rn(w));
         sh.den[tid] = den;
         sh.bthr[tid] = __double2ll_rd(w * mu + a.thr * den) - 1;
@@ -155,7 +157,7 @@ __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const WidthTab
                 const ACC p0 = P[tl];
                 bool any = false;
                 for (int j = 0; j < a.nwidths; ++j) {
-                    const int w = wt.w[j];
+                    const int w = sh.w[j];
                     if (tau + w <= a.nout_left) {
                         const long long B = (long long)(ACC)(P[tl + w] - p0);
                         any |= (B >= sh.bthr[j]);
@@ -163,7 +165,7 @@ __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const WidthTab
                 }
                 if (any) {
                     for (int j = 0; j < a.nwidths; ++j) {
-                        const int w = wt.w[j];
+                        const int w = sh.w[j];
                         if (tau + w > a.nout_left) continue;
                         const long long B = (long long)(ACC)(P[tl + w] - p0);
                         const double num = __dsub_rn((double)B, __dmul_rn((double)w, mu));
