@@ -96,10 +96,8 @@ class ClockSampler:
 
 
 def dist_env():
-    rank = int(os.environ.get("RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    return rank, world, local
+    from paper_2101_00941_b200 import dist_util
+    return dist_util.env()
 
 
 def pick_workload(k: int, world: int):
@@ -193,17 +191,15 @@ def main():
     if not torch.cuda.is_available():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    from paper_2101_00941_b200 import dist_util
+    dist_util.init("nccl", device=torch.device("cuda", local))
     B.load_library()
 
     w, note = pick_workload(args.workload, world)
     if args.nsamp:
         w = I.scaled(w, nsamp=args.nsamp, name=w.name + f"_nsamp{args.nsamp}")
         note = "shortened observation for profiling; not a bench line"
-    if world > 1:
-        w = I.scaled(w, noise_seed=w.noise_seed + 1000 * rank)
+    w = dist_util.rank_workload(w, rank)
     n_streams = args.streams or w.n_streams
     L = w.chunk_len // w.n_streams                     # sub-chunk length of both legs
 
@@ -215,8 +211,7 @@ def main():
     t_gen = time.perf_counter() - t_gen0 - t_pin
 
     def barrier():
-        if world > 1:
-            dist.barrier()
+        dist_util.barrier()
         torch.cuda.synchronize()
 
     def timed(fn, steps, warmup):
@@ -234,11 +229,7 @@ def main():
         barrier()
         wall = time.perf_counter() - t0
         dev = e0.elapsed_time(e1) / 1e3
-        t = max(wall, dev)
-        if world > 1:
-            tt = torch.tensor([t], dtype=torch.float64, device="cuda")
-            dist.all_reduce(tt, op=dist.ReduceOp.MAX)
-            t = float(tt.item())
+        t = dist_util.max_over_ranks(max(wall, dev))
         return t, acc
 
     max_cands = 1 << 24
@@ -326,9 +317,7 @@ def main():
             cb.pop("seconds", None)
             line["cpu_baseline"] = cb
         print(json.dumps(line))
-    if world > 1:
-        dist.barrier()
-        dist.destroy_process_group()
+    dist_util.shutdown()
     return 0
 
 

@@ -36,6 +36,8 @@ struct Range {
     uint32_t dm_base = 0;
     std::vector<int32_t> h_delays;   // [ndms][nchans]
     int32_t *d_delays = nullptr;
+    std::vector<int32_t> h_dtiles;   // [nblk][nstages][DB][CS]: per (DM block, channel stage) delay tiles
+    int32_t *d_dtiles = nullptr;
     int row = 0;                // staged row length (elements)
     int dpw = 4;                // DM trials per warp in the dedispersion kernel
     bool in16 = false;
@@ -248,6 +250,23 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
             }
         }
         if (!ok) return AA_ERR_INVALID;     // DM step too coarse for the staged window
+        {
+            // tiled copy of the delay table: one contiguous [DB][CS] tile per (DM block, channel stage),
+            // trials clamped to the last one, channels past nchans zero -> one bulk copy per stage
+            const int DB = R.dpw * (kDedispThreads / 32), CS = dedisp_stage_channels(R.in16);
+            const int nblk = (R.r.ndms + DB - 1) / DB, nst = (d->nchans + CS - 1) / CS;
+            R.h_dtiles.assign((size_t)nblk * nst * DB * CS, 0);
+            for (int b = 0; b < nblk; ++b)
+                for (int st = 0; st < nst; ++st)
+                    for (int dl = 0; dl < DB; ++dl) {
+                        const int dd = std::min(b * DB + dl, R.r.ndms - 1);
+                        for (int cl = 0; cl < CS; ++cl) {
+                            const int c = st * CS + cl;
+                            if (c < d->nchans)
+                                R.h_dtiles[(((size_t)b * nst + st) * DB + dl) * CS + cl] = R.h_delays[(size_t)dd * d->nchans + c];
+                        }
+                    }
+        }
         if (!R.in16) max_row_u8 = std::max(max_row_u8, R.row);
         p.d_rows = std::max<uint64_t>(p.d_rows, (uint64_t)R.r.ndms);
         max_cols = std::max<uint64_t>(max_cols, p.L / R.r.bin + p.wmax - 1);
@@ -271,7 +290,7 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
     uint64_t off = 0;
     auto take = [&](uint64_t bytes) { off = round_up(off, 256) + bytes; };
     take((uint64_t)d->nchans * p.ring_pitch);
-    for (auto &R : p.ranges) take((uint64_t)R.r.ndms * d->nchans * 4);
+    for (auto &R : p.ranges) { take((uint64_t)R.r.ndms * d->nchans * 4); take((uint64_t)R.h_dtiles.size() * 4); }
     for (int s = 0; s < p.n_streams; ++s) {
         take((p.L + p.halo) * (uint64_t)d->nchans);
         for (size_t k = 0; k < p.bins.size(); ++k) take((uint64_t)d->nchans * p.pitch_b[k] * 2);
@@ -291,7 +310,10 @@ void carve(aa_plan &p)
     auto take = [&](uint64_t bytes) { off = round_up(off, 256); uint8_t *q = base + off; off += bytes; return q; };
     const int nchans = p.desc.nchans;
     p.d_ring = take((uint64_t)nchans * p.ring_pitch);
-    for (auto &R : p.ranges) R.d_delays = reinterpret_cast<int32_t *>(take((uint64_t)R.r.ndms * nchans * 4));
+    for (auto &R : p.ranges) {
+        R.d_delays = reinterpret_cast<int32_t *>(take((uint64_t)R.r.ndms * nchans * 4));
+        R.d_dtiles = reinterpret_cast<int32_t *>(take((uint64_t)R.h_dtiles.size() * 4));
+    }
     for (auto &S : p.streams) {
         S.d_raw = take((p.L + p.halo) * (uint64_t)nchans);
         S.d_binned.resize(p.bins.size());
@@ -408,6 +430,7 @@ void worker(aa_plan *p, int s, const uint8_t *input, bool resident, aa_candidate
                 da.pitch_in = Rg.in16 ? (int64_t)p->pitch_b[Rg.bin_slot] : (int64_t)p->ring_pitch;
                 da.col0 = Rg.in16 ? 0 : (int64_t)col0;
                 da.delays = Rg.d_delays;
+                da.dtiles = Rg.d_dtiles;
                 da.nchans = nchans;
                 da.ndms = Rg.r.ndms;
                 da.ncols = (int32_t)ncols;
@@ -603,6 +626,8 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
     p->done.reset(new std::atomic<int>[p->n_sub]);
     for (auto &R : p->ranges) {
         if ((e = cudaMemcpy(R.d_delays, R.h_delays.data(), R.h_delays.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess)
+            return fail(AA_ERR_CUDA, e);
+        if ((e = cudaMemcpy(R.d_dtiles, R.h_dtiles.data(), R.h_dtiles.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess)
             return fail(AA_ERR_CUDA, e);
     }
     *out = p;

@@ -17,6 +17,7 @@ struct DedispArgs {
     int64_t pitch_in;      // elements
     int64_t col0;          // element column of output sample 0 with zero delay
     const int32_t *delays; // [ndms][nchans] binned samples (device)
+    const int32_t *dtiles; // [nblk][nstages][DB][CS] the same delays tiled per (DM block, channel stage)
     int32_t nchans, ndms;
     int32_t ncols;         // output columns to produce
     uint32_t *out;         // [ndms][pitch_out]

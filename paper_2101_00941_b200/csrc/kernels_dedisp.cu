@@ -59,6 +59,13 @@ __device__ __forceinline__ void bulk_g2s(void *dst, const void *src, uint32_t by
         : "memory");
 }
 
+// acc += x on the FMA pipe: IMAD acc = x * one + acc with a run-time multiplier of 1.  The ALU pipe
+// (64 lanes/clk/SM) is busy with the byte unpacking; integer multiply-add issues on the other pipe.
+__device__ __forceinline__ void fma_add(uint32_t &acc, uint32_t x, uint32_t one)
+{
+    asm("mad.lo.u32 %0, %1, %2, %0;" : "+r"(acc) : "r"(x), "r"(one));
+}
+
 template <int N>
 struct OffVec;
 template <>
@@ -250,6 +257,224 @@ __global__ void __launch_bounds__(NT, 2) dedisp_kernel(const DedispArgs a)
     }
 }
 
+// ---------------------------------------------------------------------------------------------
+// uint8 input, 8-bit staging ("U8" path).  The 16-bit-lane kernel above is bound by shared-memory
+// bandwidth (2 B of LDS per sample-add, 86 % of the pipe in profiles/r1_dedisp_ncu.txt).  Here a
+// row stays 1 B per sample in shared memory: the staged row itself is "copy 0" and the expand step
+// writes three more copies shifted by 1, 2 and 3 bytes, so a word-aligned 32-bit LDS returns four
+// consecutive samples for ANY delay (copy = delay & 3, word = delay >> 2).  A thread owns quads
+// of output samples; each loaded word is split into its even bytes (LOP3) and odd bytes (PRMT),
+// i.e. two registers of two 16-bit lanes, and added to the quad's two accumulators.  That is 1 B
+// of LDS and 1.25 issue slots per sample-add instead of 2 B and 0.75: the bound moves from the
+// shared-memory pipe to instruction issue, with the adds shared between the ALU and FMA pipes.
+template <int DPW, int CS>
+__global__ void __launch_bounds__(NT, 2) dedisp_u8_kernel(const DedispArgs a)
+{
+    constexpr int DB = DPW * NW;
+    constexpr int NQ = TB / 4 / 32;               // quads per lane (4)
+    static_assert(DB <= 32 && CS == 16, "one delay-tile row per lane of warp 0; two staged rows per warp");
+    extern __shared__ __align__(128) uint8_t smem[];
+    const int ROW = a.row;
+    const size_t stg_bytes = (size_t)CS * ROW + 16;
+    uint8_t *stg0 = smem;                                           // [2][CS][ROW] (+16): copy 0
+    uint8_t *cpy = smem + 2 * stg_bytes;                            // [3][CS][ROW]: copies 1..3
+    uint32_t *soff = reinterpret_cast<uint32_t *>(cpy + (size_t)3 * CS * ROW);   // [CS][DB]
+    int32_t *dtile = reinterpret_cast<int32_t *>(soff + CS * DB);   // [3][DB][CS] delays of a stage
+    uint64_t *bar = reinterpret_cast<uint64_t *>(dtile + 3 * DB * CS);           // [3]
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int d0 = blockIdx.x * DB;
+    const int64_t t0 = (int64_t)blockIdx.y * TB;
+    const int nchans = a.nchans;
+    const int nstages = (nchans + CS - 1) / CS;
+    const uint8_t *in = static_cast<const uint8_t *>(a.in);
+
+    if (tid == 0) {
+        mbar_init(&bar[0], 1);
+        mbar_init(&bar[1], 1);
+        mbar_init(&bar[2], 1);
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    // Delay tile of stage s: one contiguous [DB][CS] block of the tiled delay table (trials clamped,
+    // channels past nchans zero): a single 2 KB bulk copy.
+    const int32_t *tiles = a.dtiles + (size_t)blockIdx.x * nstages * (DB * CS);
+    // Rows of stage s (window base from the tile's first trial): every warp issues its own CS/NW rows,
+    // so no warp serialises 16 copies; thread 0 arms the barrier and adds the delay tile of stage s+1.
+    auto issue_rows = [&](int s, int buf) {
+        if (tid == 0) {
+            int nvalid = nchans - s * CS;
+            if (nvalid > CS) nvalid = CS;
+            const bool next_tile = s + 1 < nstages;
+            mbar_expect_tx(&bar[buf], (uint32_t)(nvalid * ROW) + (next_tile ? DB * CS * 4 : 0));
+            if (next_tile) bulk_g2s(dtile + ((s + 1) % 3) * DB * CS, tiles + (size_t)(s + 1) * DB * CS, DB * CS * 4, &bar[buf]);
+        }
+        if (lane < CS / NW) {
+            const int cl = warp * (CS / NW) + lane, c = s * CS + cl;
+            if (c < nchans) {
+                const int base = dtile[(s % 3) * DB * CS + cl] & ~(kAlign - 1);
+                const uint8_t *src = in + (size_t)c * a.pitch_in + a.col0 + t0 + base;
+                bulk_g2s(stg0 + buf * stg_bytes + (size_t)cl * ROW, src, (uint32_t)ROW, &bar[buf]);
+            }
+        }
+    };
+
+    uint32_t acc_e[DPW][NQ], acc_o[DPW][NQ];      // 16-bit lanes: samples (4q, 4q+2) and (4q+1, 4q+3)
+    uint32_t acc32[DPW][4 * NQ];
+#pragma unroll
+    for (int k = 0; k < DPW; ++k) {
+#pragma unroll
+        for (int i = 0; i < NQ; ++i) acc_e[k][i] = acc_o[k][i] = 0;
+#pragma unroll
+        for (int i = 0; i < 4 * NQ; ++i) acc32[k][i] = 0;
+    }
+    int since_flush = 0;
+    const uint32_t one = a.flush_ch > 0 ? 1u : 0u;     // always 1; opaque to the compiler
+    auto flush = [&]() {
+#pragma unroll
+        for (int k = 0; k < DPW; ++k)
+#pragma unroll
+            for (int i = 0; i < NQ; ++i) {
+                acc32[k][4 * i + 0] += acc_e[k][i] & 0xFFFFu;
+                acc32[k][4 * i + 1] += acc_o[k][i] & 0xFFFFu;
+                acc32[k][4 * i + 2] += acc_e[k][i] >> 16;
+                acc32[k][4 * i + 3] += acc_o[k][i] >> 16;
+                acc_e[k][i] = acc_o[k][i] = 0;
+            }
+    };
+
+    // prologue: tile 0 (own barrier), then rows 0 + tile 1
+    if (tid == 0) {
+        mbar_expect_tx(&bar[2], DB * CS * 4);
+        bulk_g2s(dtile, tiles, DB * CS * 4, &bar[2]);
+    }
+    mbar_wait(&bar[2], 0);
+    issue_rows(0, 0);
+
+    for (int s = 0; s < nstages; ++s) {
+        const int buf = s & 1;
+        uint8_t *stg = stg0 + buf * stg_bytes;
+
+        mbar_wait(&bar[buf], (uint32_t)((s >> 1) & 1));              // rows(s) and tile(s+1) have landed
+        if (s + 1 < nstages) issue_rows(s + 1, buf ^ 1);
+
+        // shared-memory byte offset of (channel, trial): copy (delay & 3), word (delay >> 2)
+        {
+            const uint32_t stg_off = (uint32_t)(stg - smem), cpy_off = (uint32_t)(cpy - smem);
+            const int32_t *dt = dtile + (s % 3) * DB * CS;
+            for (int e = tid; e < CS * DB; e += NT) {
+                const int cl = e % CS, dl = e / CS;
+                uint32_t off = cpy_off + (uint32_t)(cl * ROW);      // rows past nchans: zero-filled copy 1
+                if (s * CS + cl < nchans) {
+                    const int rel = dt[dl * CS + cl] - (dt[cl] & ~(kAlign - 1));
+                    const int sh = rel & 3;
+                    off = (sh == 0 ? stg_off + (uint32_t)(cl * ROW)
+                                   : cpy_off + (uint32_t)(((sh - 1) * CS + cl) * ROW)) + (uint32_t)(rel >> 2) * 4u;
+                }
+                soff[cl * DB + dl] = off;
+            }
+        }
+
+        // expand: copies shifted by 1, 2, 3 bytes; warp w owns rows 2w and 2w+1, 16 samples per task
+        {
+            const int tasks_per_row = ROW / 16;
+#pragma unroll
+            for (int rr = 0; rr < CS / NW; ++rr) {
+                const int cl = warp * (CS / NW) + rr;
+                const bool live = s * CS + cl < nchans;
+                for (int k = lane; k < tasks_per_row; k += 32) {
+                    uint4 c1, c2, c3;
+                    if (live) {
+                        const uint8_t *src = stg + (size_t)cl * ROW + k * 16;
+                        const uint4 v = *reinterpret_cast<const uint4 *>(src);
+                        const uint32_t nx = *reinterpret_cast<const uint32_t *>(src + 16);
+                        c1 = make_uint4(__funnelshift_r(v.x, v.y, 8), __funnelshift_r(v.y, v.z, 8),
+                                        __funnelshift_r(v.z, v.w, 8), __funnelshift_r(v.w, nx, 8));
+                        c2 = make_uint4(__funnelshift_r(v.x, v.y, 16), __funnelshift_r(v.y, v.z, 16),
+                                        __funnelshift_r(v.z, v.w, 16), __funnelshift_r(v.w, nx, 16));
+                        c3 = make_uint4(__funnelshift_r(v.x, v.y, 24), __funnelshift_r(v.y, v.z, 24),
+                                        __funnelshift_r(v.z, v.w, 24), __funnelshift_r(v.w, nx, 24));
+                    } else {
+                        c1 = c2 = c3 = make_uint4(0, 0, 0, 0);
+                    }
+                    uint8_t *dst = cpy + (size_t)cl * ROW + k * 16;
+                    *reinterpret_cast<uint4 *>(dst) = c1;
+                    *reinterpret_cast<uint4 *>(dst + (size_t)CS * ROW) = c2;
+                    *reinterpret_cast<uint4 *>(dst + (size_t)2 * CS * ROW) = c3;
+                }
+            }
+        }
+        __syncthreads();
+
+        {
+            const uint8_t *sb = smem + lane * 4;
+#pragma unroll 2
+            for (int cp = 0; cp < CS; cp += 2) {
+                uint32_t o0[DPW], o1[DPW];
+                load_offsets<DPW>(soff + cp * DB + warp * DPW, o0);
+                load_offsets<DPW>(soff + (cp + 1) * DB + warp * DPW, o1);
+#pragma unroll
+                for (int k = 0; k < DPW; ++k) {
+                    const uint32_t *p0 = reinterpret_cast<const uint32_t *>(sb + o0[k]);
+                    const uint32_t *p1 = reinterpret_cast<const uint32_t *>(sb + o1[k]);
+#pragma unroll
+                    for (int i = 0; i < NQ; ++i) {
+                        const uint32_t w0 = p0[i * 32], w1 = p1[i * 32];
+                        // unpack on the ALU pipe (LOP3, PRMT); accumulate on the FMA pipe (IMAD by a
+                        // run-time 1) so the two pipes and the LSU each carry 1/3 of the instructions
+                        fma_add(acc_e[k][i], w0 & 0x00FF00FFu, one);
+                        fma_add(acc_o[k][i], __byte_perm(w0, 0, 0x4341), one);
+                        fma_add(acc_e[k][i], w1 & 0x00FF00FFu, one);
+                        fma_add(acc_o[k][i], __byte_perm(w1, 0, 0x4341), one);
+                    }
+                }
+                since_flush += 2;
+                if (since_flush >= a.flush_ch) {
+                    flush();
+                    since_flush = 0;
+                }
+            }
+        }
+        __syncthreads();
+    }
+    flush();
+
+#pragma unroll
+    for (int k = 0; k < DPW; ++k) {
+        const int d = d0 + warp * DPW + k;
+        if (d >= a.ndms) continue;
+        uint32_t *orow = a.out + (size_t)d * a.pitch_out;
+#pragma unroll
+        for (int i = 0; i < NQ; ++i) {
+            const int64_t t = t0 + 4 * (lane + 32 * i);
+            if (t + 3 < a.ncols) {
+                *reinterpret_cast<uint4 *>(orow + t) =
+                    make_uint4(acc32[k][4 * i], acc32[k][4 * i + 1], acc32[k][4 * i + 2], acc32[k][4 * i + 3]);
+            } else {
+#pragma unroll
+                for (int j = 0; j < 4; ++j)
+                    if (t + j < a.ncols) orow[t + j] = acc32[k][4 * i + j];
+            }
+        }
+    }
+}
+
+template <int DPW, int CS>
+size_t smem_bytes_u8(int row)
+{
+    return 2 * ((size_t)CS * row + 16) + (size_t)3 * CS * row + (size_t)CS * DPW * NW * 4 * 4 + 32;
+}
+
+template <int DPW, int CS>
+cudaError_t launch_u8(const DedispArgs &a, cudaStream_t st)
+{
+    constexpr int DB = DPW * NW;
+    dim3 grid((unsigned)((a.ndms + DB - 1) / DB), (unsigned)((a.ncols + TB - 1) / TB));
+    dedisp_u8_kernel<DPW, CS><<<grid, NT, smem_bytes_u8<DPW, CS>(a.row), st>>>(a);
+    return cudaGetLastError();
+}
+
 template <typename IN_T, int DPW, int CS>
 size_t smem_bytes_t(int row)
 {
@@ -279,9 +504,9 @@ size_t dedisp_smem_bytes(bool in16, int dpw, int row)
                : dpw == 2 ? smem_bytes_t<uint16_t, 2, CS16>(row)
                           : smem_bytes_t<uint16_t, 1, CS16>(row);
     }
-    return dpw == 4 ? smem_bytes_t<uint8_t, 4, CS8>(row)
-           : dpw == 2 ? smem_bytes_t<uint8_t, 2, CS8>(row)
-                      : smem_bytes_t<uint8_t, 1, CS8>(row);
+    return dpw == 4 ? smem_bytes_u8<4, CS8>(row)
+           : dpw == 2 ? smem_bytes_u8<2, CS8>(row)
+                      : smem_bytes_u8<1, CS8>(row);
 }
 
 cudaError_t dedisp_configure()
@@ -291,9 +516,13 @@ cudaError_t dedisp_configure()
 #define AA_CFG(T, D, C)                                                                                    \
     e = cudaFuncSetAttribute(dedisp_kernel<T, D, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxb); \
     if (e != cudaSuccess) return e;
-    AA_CFG(uint8_t, 4, CS8) AA_CFG(uint8_t, 2, CS8) AA_CFG(uint8_t, 1, CS8)
     AA_CFG(uint16_t, 4, CS16) AA_CFG(uint16_t, 2, CS16) AA_CFG(uint16_t, 1, CS16)
 #undef AA_CFG
+#define AA_CFG8(D, C)                                                                                    \
+    e = cudaFuncSetAttribute(dedisp_u8_kernel<D, C>, cudaFuncAttributeMaxDynamicSharedMemorySize, maxb); \
+    if (e != cudaSuccess) return e;
+    AA_CFG8(4, CS8) AA_CFG8(2, CS8) AA_CFG8(1, CS8)
+#undef AA_CFG8
     return cudaSuccess;
 }
 
@@ -305,9 +534,9 @@ cudaError_t launch_dedisp(const DedispArgs &a, bool in16, int dpw, cudaStream_t 
                : dpw == 2 ? launch_t<uint16_t, 2, CS16>(a, st)
                           : launch_t<uint16_t, 1, CS16>(a, st);
     }
-    return dpw == 4 ? launch_t<uint8_t, 4, CS8>(a, st)
-           : dpw == 2 ? launch_t<uint8_t, 2, CS8>(a, st)
-                      : launch_t<uint8_t, 1, CS8>(a, st);
+    return dpw == 4 ? launch_u8<4, CS8>(a, st)
+           : dpw == 2 ? launch_u8<2, CS8>(a, st)
+                      : launch_u8<1, CS8>(a, st);
 }
 
 }  // namespace aa
