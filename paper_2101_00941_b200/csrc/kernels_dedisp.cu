@@ -320,29 +320,12 @@ __global__ void __launch_bounds__(NT, 2) dedisp_u8_kernel(const DedispArgs a)
         }
     };
 
-    uint32_t acc_e[DPW][NQ], acc_o[DPW][NQ];      // 16-bit lanes: samples (4q, 4q+2) and (4q+1, 4q+3)
-    uint32_t acc32[DPW][4 * NQ];
+    // one exact 32-bit accumulator per output sample: no 16-bit lanes, no flush, any channel count
+    uint32_t acc[DPW][4 * NQ];
 #pragma unroll
-    for (int k = 0; k < DPW; ++k) {
+    for (int k = 0; k < DPW; ++k)
 #pragma unroll
-        for (int i = 0; i < NQ; ++i) acc_e[k][i] = acc_o[k][i] = 0;
-#pragma unroll
-        for (int i = 0; i < 4 * NQ; ++i) acc32[k][i] = 0;
-    }
-    int since_flush = 0;
-    const uint32_t one = a.flush_ch > 0 ? 1u : 0u;     // always 1; opaque to the compiler
-    auto flush = [&]() {
-#pragma unroll
-        for (int k = 0; k < DPW; ++k)
-#pragma unroll
-            for (int i = 0; i < NQ; ++i) {
-                acc32[k][4 * i + 0] += acc_e[k][i] & 0xFFFFu;
-                acc32[k][4 * i + 1] += acc_o[k][i] & 0xFFFFu;
-                acc32[k][4 * i + 2] += acc_e[k][i] >> 16;
-                acc32[k][4 * i + 3] += acc_o[k][i] >> 16;
-                acc_e[k][i] = acc_o[k][i] = 0;
-            }
-    };
+        for (int i = 0; i < 4 * NQ; ++i) acc[k][i] = 0;
 
     // prologue: tile 0 (own barrier), then rows 0 + tile 1
     if (tid == 0) {
@@ -421,24 +404,21 @@ __global__ void __launch_bounds__(NT, 2) dedisp_u8_kernel(const DedispArgs a)
 #pragma unroll
                     for (int i = 0; i < NQ; ++i) {
                         const uint32_t w0 = p0[i * 32], w1 = p1[i * 32];
-                        // unpack on the ALU pipe (LOP3, PRMT); accumulate on the FMA pipe (IMAD by a
-                        // run-time 1) so the two pipes and the LSU each carry 1/3 of the instructions
-                        fma_add(acc_e[k][i], w0 & 0x00FF00FFu, one);
-                        fma_add(acc_o[k][i], __byte_perm(w0, 0, 0x4341), one);
-                        fma_add(acc_e[k][i], w1 & 0x00FF00FFu, one);
-                        fma_add(acc_o[k][i], __byte_perm(w1, 0, 0x4341), one);
+                        // interleave the two channels' bytes (PRMT, ALU pipe), then one dp4a per output
+                        // sample adds both channels into its 32-bit accumulator (IDP4A, FMA pipe):
+                        // 2 LDS + 2 PRMT + 4 IDP4A per 8 sample-adds
+                        const uint32_t lo = __byte_perm(w0, w1, 0x5140);   // (a0, b0, a1, b1)
+                        const uint32_t hi = __byte_perm(w0, w1, 0x7362);   // (a2, b2, a3, b3)
+                        acc[k][4 * i + 0] = __dp4a(lo, 0x00000101u, acc[k][4 * i + 0]);
+                        acc[k][4 * i + 1] = __dp4a(lo, 0x01010000u, acc[k][4 * i + 1]);
+                        acc[k][4 * i + 2] = __dp4a(hi, 0x00000101u, acc[k][4 * i + 2]);
+                        acc[k][4 * i + 3] = __dp4a(hi, 0x01010000u, acc[k][4 * i + 3]);
                     }
-                }
-                since_flush += 2;
-                if (since_flush >= a.flush_ch) {
-                    flush();
-                    since_flush = 0;
                 }
             }
         }
         __syncthreads();
     }
-    flush();
 
 #pragma unroll
     for (int k = 0; k < DPW; ++k) {
@@ -450,11 +430,11 @@ __global__ void __launch_bounds__(NT, 2) dedisp_u8_kernel(const DedispArgs a)
             const int64_t t = t0 + 4 * (lane + 32 * i);
             if (t + 3 < a.ncols) {
                 *reinterpret_cast<uint4 *>(orow + t) =
-                    make_uint4(acc32[k][4 * i], acc32[k][4 * i + 1], acc32[k][4 * i + 2], acc32[k][4 * i + 3]);
+                    make_uint4(acc[k][4 * i], acc[k][4 * i + 1], acc[k][4 * i + 2], acc[k][4 * i + 3]);
             } else {
 #pragma unroll
                 for (int j = 0; j < 4; ++j)
-                    if (t + j < a.ncols) orow[t + j] = acc32[k][4 * i + j];
+                    if (t + j < a.ncols) orow[t + j] = acc[k][4 * i + j];
             }
         }
     }
