@@ -11,6 +11,7 @@
 #include <chrono>
 #include <cmath>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <memory>
 #include <mutex>
@@ -44,6 +45,10 @@ struct Range {
     int flush_ch = 2;
     bool wide = false;          // 64-bit boxcar sums
     int bin_slot = -1;          // index into the per-stream binned buffers
+    int sp_tb = 0;              // shared-pattern kernel: time tile (1024 or 512); 0 = plain kernel
+    std::vector<SpRecord> h_sp;
+    SpRecord *d_sp = nullptr;
+    int32_t sp_rows = 0, sp_pbytes = 0, sp_flush = 1;
     std::vector<std::pair<int, int>> taps;   // (local dm, tap row)
 };
 
@@ -267,7 +272,27 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
                         }
                     }
         }
-        if (!R.in16) max_row_u8 = std::max(max_row_u8, R.row);
+        // shared-pattern kernel: uint8 input, tables within limits, rows within shared memory.
+        // AA_DEDISP=plain forces the plain kernels, =sp512 / =sp1024 one tile size (A/B timing, tests).
+        R.sp_tb = 0;
+        if (!R.in16) {
+            const char *env = std::getenv("AA_DEDISP");
+            const bool plain = env && std::strcmp(env, "plain") == 0;
+            const bool only512 = env && std::strcmp(env, "sp512") == 0;
+            const bool only1024 = env && std::strcmp(env, "sp1024") == 0;
+            for (int tb : {1024, 512}) {
+                if (plain || (tb == 1024 && only512) || (tb == 512 && only1024)) continue;
+                const size_t limit = tb == 1024 ? 227 * 1024 : 113 * 1024;
+                if (sp_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, R.h_sp, R.sp_rows, R.sp_pbytes) &&
+                    dedisp_sp_smem_bytes(R.sp_rows, R.sp_pbytes) + 1024 <= limit) {
+                    R.sp_tb = tb;
+                    R.sp_flush = 65535 / (255 * R.r.bin * kSpG);
+                    break;
+                }
+            }
+            if (!R.sp_tb) { R.h_sp.clear(); R.h_sp.shrink_to_fit(); }
+        }
+        if (!R.in16) max_row_u8 = std::max(max_row_u8, std::max(R.row, R.sp_tb ? R.sp_rows + R.sp_tb : 0));
         p.d_rows = std::max<uint64_t>(p.d_rows, (uint64_t)R.r.ndms);
         max_cols = std::max<uint64_t>(max_cols, p.L / R.r.bin + p.wmax - 1);
         if (!R.taps.empty()) {
@@ -289,8 +314,12 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
     // arena layout (256-byte aligned bump allocation, computed identically in carve())
     uint64_t off = 0;
     auto take = [&](uint64_t bytes) { off = round_up(off, 256) + bytes; };
-    take((uint64_t)d->nchans * p.ring_pitch);
-    for (auto &R : p.ranges) { take((uint64_t)R.r.ndms * d->nchans * 4); take((uint64_t)R.h_dtiles.size() * 4); }
+    take(round_up((uint64_t)d->nchans, kSpG) * p.ring_pitch);   // zero rows pad the channels to a multiple of kSpG
+    for (auto &R : p.ranges) {
+        take((uint64_t)R.r.ndms * d->nchans * 4);
+        take((uint64_t)R.h_dtiles.size() * 4);
+        take((uint64_t)R.h_sp.size() * sizeof(SpRecord));
+    }
     for (int s = 0; s < p.n_streams; ++s) {
         take((p.L + p.halo) * (uint64_t)d->nchans);
         for (size_t k = 0; k < p.bins.size(); ++k) take((uint64_t)d->nchans * p.pitch_b[k] * 2);
@@ -309,10 +338,11 @@ void carve(aa_plan &p)
     uint64_t off = 0;
     auto take = [&](uint64_t bytes) { off = round_up(off, 256); uint8_t *q = base + off; off += bytes; return q; };
     const int nchans = p.desc.nchans;
-    p.d_ring = take((uint64_t)nchans * p.ring_pitch);
+    p.d_ring = take(round_up((uint64_t)nchans, kSpG) * p.ring_pitch);
     for (auto &R : p.ranges) {
         R.d_delays = reinterpret_cast<int32_t *>(take((uint64_t)R.r.ndms * nchans * 4));
         R.d_dtiles = reinterpret_cast<int32_t *>(take((uint64_t)R.h_dtiles.size() * 4));
+        R.d_sp = reinterpret_cast<SpRecord *>(take((uint64_t)R.h_sp.size() * sizeof(SpRecord)));
     }
     for (auto &S : p.streams) {
         S.d_raw = take((p.L + p.halo) * (uint64_t)nchans);
@@ -438,7 +468,12 @@ void worker(aa_plan *p, int s, const uint8_t *input, bool resident, aa_candidate
                 da.pitch_out = (int64_t)p->pitchD;
                 da.row = Rg.row;
                 da.flush_ch = Rg.flush_ch;
-                AA_W(launch_dedisp(da, Rg.in16, Rg.dpw, st));
+                da.sp_tab = Rg.d_sp;
+                da.sp_rows = Rg.sp_rows;
+                da.sp_pbytes = Rg.sp_pbytes;
+                da.sp_flush = Rg.sp_flush;
+                if (Rg.sp_tb) AA_W(launch_dedisp_sp(da, Rg.sp_tb, st));
+                else AA_W(launch_dedisp(da, Rg.in16, Rg.dpw, st));
                 S.dedisp_launches++;
                 AA_W(cudaEventRecord(e1, st));
                 SpsArgs sa{};
@@ -594,6 +629,7 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
     auto fail = [&](int code, cudaError_t e) { g_last_cuda_error = (int)e; destroy_plan(p); return code; };
     cudaError_t e;
     if ((e = dedisp_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
+    if ((e = dedisp_sp_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
     if ((e = sps_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
 
     if (d->device_arena) {
@@ -619,6 +655,11 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
             if ((e = cudaHostAlloc((void **)&S.h_tap, p->tap_stage_elems * 4, cudaHostAllocDefault)) != cudaSuccess) { cudaGetLastError(); return fail(AA_ERR_OOM, e); }
     }
     carve(*p);
+    {
+        const uint64_t pad_rows = round_up((uint64_t)d->nchans, kSpG) - (uint64_t)d->nchans;
+        if (pad_rows && (e = cudaMemset(p->d_ring + (uint64_t)d->nchans * p->ring_pitch, 0, pad_rows * p->ring_pitch)) != cudaSuccess)
+            return fail(AA_ERR_CUDA, e);
+    }
     p->ev_loaded.assign(p->n_sub, nullptr);
     for (auto &ev : p->ev_loaded)
         if ((e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess) return fail(AA_ERR_CUDA, e);
@@ -628,6 +669,8 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
         if ((e = cudaMemcpy(R.d_delays, R.h_delays.data(), R.h_delays.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess)
             return fail(AA_ERR_CUDA, e);
         if ((e = cudaMemcpy(R.d_dtiles, R.h_dtiles.data(), R.h_dtiles.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess)
+            return fail(AA_ERR_CUDA, e);
+        if (R.sp_tb && (e = cudaMemcpy(R.d_sp, R.h_sp.data(), R.h_sp.size() * sizeof(SpRecord), cudaMemcpyHostToDevice)) != cudaSuccess)
             return fail(AA_ERR_CUDA, e);
     }
     *out = p;

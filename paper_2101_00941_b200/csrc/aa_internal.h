@@ -3,6 +3,8 @@
 #include <cuda_runtime.h>
 #include <stdint.h>
 
+#include <vector>
+
 #include "../../include/aa.h"
 
 namespace aa {
@@ -24,7 +26,45 @@ struct DedispArgs {
     int64_t pitch_out;     // elements (even)
     int32_t row;           // staged row length in elements (multiple of 16)
     int32_t flush_ch;      // channels between 16->32 bit flushes (even, >= 2)
+    // shared-pattern kernel (kernels_dedisp_shared.cu) only:
+    const void *sp_tab;    // SpRecord [nblk][ngroups] (device)
+    int32_t sp_rows;       // shared-memory bytes reserved per staged channel row (multiple of 16)
+    int32_t sp_pbytes;     // bytes of one pattern-row buffer (multiple of 16)
+    int32_t sp_flush;      // channel groups between 16-bit -> 32-bit flushes
 };
+
+// ---- shared-pattern dedispersion: plan-time record per (DM block, channel group) ---------------
+// Within a block of kSpDB consecutive trials the rounded delays of kSpG adjacent channels, taken
+// relative to the group's first channel, form only a few distinct vectors ("patterns": each delay
+// is rounded on its own, so the differences jitter between floor and ceil).  The kernel sums the
+// group's channels once per pattern into a 16-bit row and every trial then adds ONE row sample per
+// group instead of kSpG channel samples.  Exact: the same integers are added, in another order.
+constexpr int kSpG = 4;             // channels per group
+constexpr int kSpDB = 64;           // DM trials per CTA
+constexpr int kSpMaxPat = 8;        // pattern rows per record
+struct SpRecord {
+    int32_t rbase[kSpG];            // first staged sample of each channel row relative to col0 + t0 (multiple of 16)
+    uint16_t rbytes[kSpG];          // staged bytes of each channel row (multiple of 16)
+    uint16_t npat;                  // pattern rows
+    uint16_t nchunk;                // 8-sample chunks per pattern row
+    uint16_t nbatch;                // warp-sized batches of chunks per pattern row
+    uint16_t inv;                   // ceil(65536 / nbatch): item / nbatch == (item * inv) >> 16
+    // pattern k, channel i: row sample u is byte u + sh of the staged channel row.  bits 0-15:
+    // i * sp_rows + (sh & ~7), the 8-byte-aligned load offset inside the staging buffer; bits 16-21: (sh & 7) * 8
+    uint32_t win[kSpMaxPat][kSpG];
+    uint32_t poff[kSpDB];           // byte offset, inside the pattern-row buffer, of trial d's word (tau 0, tau 1)
+};
+static_assert(sizeof(SpRecord) % 16 == 0, "records are fetched with 16-byte bulk copies");
+
+// Builds the records of one range for time tiles of `tb` samples (host, plan time).  Returns false
+// if the range does not fit the scheme (too many patterns, delays not monotone); the caller then
+// uses the plain kernels.  rows / pbytes: see DedispArgs.
+bool sp_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t tb, std::vector<SpRecord> &out,
+                     int32_t &rows, int32_t &pbytes);
+// tb = 1024 (512 threads, one CTA per SM) or 512 (256 threads, two CTAs per SM)
+cudaError_t launch_dedisp_sp(const DedispArgs &a, int tb, cudaStream_t st);
+size_t dedisp_sp_smem_bytes(int rows, int pbytes);
+cudaError_t dedisp_sp_configure();
 
 struct SpsArgs {
     const uint32_t *D;     // [ndms][pitch] dedispersed sub-chunk
