@@ -137,6 +137,12 @@ uint64_t aa_plan_nout(const aa_plan *p, int32_t r);
  * memory `out`; used by tests to compare with the oracle entry by entry. */
 int aa_plan_delays(const aa_plan *p, int32_t r, int32_t *out);
 
+/* Which dedispersion kernel the plan chose for range r (the choice depends only on the delay table):
+ * 0 = plain tiled kernel, 1 / 2 = shared-pattern kernel with 512 / 1024-sample tiles, 3 / 4 =
+ * warp-specialised shared-pattern kernel with 512 / 1024-sample tiles; AA_ERR_INVALID if r is out
+ * of range.  Used by tests to make sure every kernel is covered. */
+int aa_plan_dedisp_variant(const aa_plan *p, int32_t r);
+
 /*
  * The hot path: for every sub-chunk, on its stream:
  * async H2D of the new input rows -> corner turn into the device ring -> per range: (binning,)

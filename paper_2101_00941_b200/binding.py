@@ -21,6 +21,7 @@ CAND_DTYPE = np.dtype([("dm_index", np.uint32), ("t_start", np.uint32),
                        ("width", np.uint32), ("snr", np.float32)])
 
 EXPORTS = ["aa_plan_arena_bytes", "aa_plan_create", "aa_plan_query", "aa_plan_nout", "aa_plan_delays",
+           "aa_plan_dedisp_variant",
            "aa_run", "aa_run_resident", "aa_get_stats", "aa_destroy", "aa_host_alloc", "aa_host_free",
            "aa_strerror", "aa_last_cuda_error"]
 
@@ -88,6 +89,8 @@ def load_library() -> ctypes.CDLL:
     lib.aa_plan_nout.argtypes = [vp, i32]
     lib.aa_plan_delays.restype = ctypes.c_int
     lib.aa_plan_delays.argtypes = [vp, i32, vp]
+    lib.aa_plan_dedisp_variant.restype = ctypes.c_int
+    lib.aa_plan_dedisp_variant.argtypes = [vp, i32]
     for f in (lib.aa_run, lib.aa_run_resident):
         f.restype = ctypes.c_int
         f.argtypes = [vp, vp, vp, u64, ctypes.POINTER(u64), vp]
@@ -176,6 +179,13 @@ class Plan:
         out = np.empty((self.w.ranges[r].ndms, self.w.nchans), dtype=np.int32)
         _check(self.lib, self.lib.aa_plan_delays(self.handle, r, out.ctypes.data))
         return out
+
+    def dedisp_variant(self, r: int) -> int:
+        """0 plain, 1/2 shared-pattern 512/1024, 3/4 warp-specialised shared-pattern 512/1024."""
+        v = self.lib.aa_plan_dedisp_variant(self.handle, r)
+        if v < 0:
+            _check(self.lib, v)
+        return v
 
     def _run(self, fn, ptr: int, max_cands: int, want_taps: bool):
         out = np.empty(int(max_cands), dtype=CAND_DTYPE)

@@ -46,8 +46,12 @@ struct Range {
     bool wide = false;          // 64-bit boxcar sums
     int bin_slot = -1;          // index into the per-stream binned buffers
     int sp_tb = 0;              // shared-pattern kernel: time tile (1024 or 512); 0 = plain kernel
+    bool ws = false;            // warp-specialised variant of the shared-pattern kernel
     std::vector<SpRecord> h_sp;
-    SpRecord *d_sp = nullptr;
+    std::vector<WsRecord> h_ws;
+    void *d_sp = nullptr;
+    size_t sp_table_bytes() const { return ws ? h_ws.size() * sizeof(WsRecord) : h_sp.size() * sizeof(SpRecord); }
+    const void *sp_table() const { return ws ? (const void *)h_ws.data() : (const void *)h_sp.data(); }
     int32_t sp_rows = 0, sp_pbytes = 0, sp_flush = 1;
     std::vector<std::pair<int, int>> taps;   // (local dm, tap row)
 };
@@ -272,25 +276,31 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
                         }
                     }
         }
-        // shared-pattern kernel: uint8 input, tables within limits, rows within shared memory.
-        // AA_DEDISP=plain forces the plain kernels, =sp512 / =sp1024 one tile size (A/B timing, tests).
+        // shared-pattern kernels: uint8 input, tables within limits, rows within shared memory.
+        // AA_DEDISP=plain forces the plain kernels, =ws1024 / ws512 / sp1024 / sp512 one variant (A/B timing, tests).
         R.sp_tb = 0;
+        R.ws = false;
         if (!R.in16) {
             const char *env = std::getenv("AA_DEDISP");
-            const bool plain = env && std::strcmp(env, "plain") == 0;
-            const bool only512 = env && std::strcmp(env, "sp512") == 0;
-            const bool only1024 = env && std::strcmp(env, "sp1024") == 0;
+            auto allowed = [&](const char *name) { return !env || !*env || std::strcmp(env, name) == 0; };
             for (int tb : {1024, 512}) {
-                if (plain || (tb == 1024 && only512) || (tb == 512 && only1024)) continue;
-                const size_t limit = tb == 1024 ? 227 * 1024 : 113 * 1024;
-                if (sp_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, R.h_sp, R.sp_rows, R.sp_pbytes) &&
-                    dedisp_sp_smem_bytes(R.sp_rows, R.sp_pbytes) + 1024 <= limit) {
+                if (R.sp_tb || !allowed(tb == 1024 ? "ws1024" : "ws512")) continue;
+                if (ws_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, R.h_ws, R.sp_rows, R.sp_pbytes) &&
+                    dedisp_ws_smem_bytes(R.sp_rows, R.sp_pbytes) + 1024 <= 227 * 1024) {
                     R.sp_tb = tb;
-                    R.sp_flush = 65535 / (255 * R.r.bin * kSpG);
-                    break;
+                    R.ws = true;
                 }
             }
-            if (!R.sp_tb) { R.h_sp.clear(); R.h_sp.shrink_to_fit(); }
+            if (!R.ws) { R.h_ws.clear(); R.h_ws.shrink_to_fit(); }
+            for (int tb : {1024, 512}) {
+                if (R.sp_tb || !allowed(tb == 1024 ? "sp1024" : "sp512")) continue;
+                const size_t limit = tb == 1024 ? 227 * 1024 : 113 * 1024;
+                if (sp_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, R.h_sp, R.sp_rows, R.sp_pbytes) &&
+                    dedisp_sp_smem_bytes(R.sp_rows, R.sp_pbytes) + 1024 <= limit)
+                    R.sp_tb = tb;
+            }
+            if (!R.sp_tb || R.ws) { R.h_sp.clear(); R.h_sp.shrink_to_fit(); }
+            if (R.sp_tb) R.sp_flush = 65535 / (255 * R.r.bin * kSpG);
         }
         if (!R.in16) max_row_u8 = std::max(max_row_u8, std::max(R.row, R.sp_tb ? R.sp_rows + R.sp_tb : 0));
         p.d_rows = std::max<uint64_t>(p.d_rows, (uint64_t)R.r.ndms);
@@ -318,7 +328,7 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
     for (auto &R : p.ranges) {
         take((uint64_t)R.r.ndms * d->nchans * 4);
         take((uint64_t)R.h_dtiles.size() * 4);
-        take((uint64_t)R.h_sp.size() * sizeof(SpRecord));
+        take((uint64_t)R.sp_table_bytes());
     }
     for (int s = 0; s < p.n_streams; ++s) {
         take((p.L + p.halo) * (uint64_t)d->nchans);
@@ -342,7 +352,7 @@ void carve(aa_plan &p)
     for (auto &R : p.ranges) {
         R.d_delays = reinterpret_cast<int32_t *>(take((uint64_t)R.r.ndms * nchans * 4));
         R.d_dtiles = reinterpret_cast<int32_t *>(take((uint64_t)R.h_dtiles.size() * 4));
-        R.d_sp = reinterpret_cast<SpRecord *>(take((uint64_t)R.h_sp.size() * sizeof(SpRecord)));
+        R.d_sp = take((uint64_t)R.sp_table_bytes());
     }
     for (auto &S : p.streams) {
         S.d_raw = take((p.L + p.halo) * (uint64_t)nchans);
@@ -472,7 +482,8 @@ void worker(aa_plan *p, int s, const uint8_t *input, bool resident, aa_candidate
                 da.sp_rows = Rg.sp_rows;
                 da.sp_pbytes = Rg.sp_pbytes;
                 da.sp_flush = Rg.sp_flush;
-                if (Rg.sp_tb) AA_W(launch_dedisp_sp(da, Rg.sp_tb, st));
+                if (Rg.ws) AA_W(launch_dedisp_ws(da, Rg.sp_tb, st));
+                else if (Rg.sp_tb) AA_W(launch_dedisp_sp(da, Rg.sp_tb, st));
                 else AA_W(launch_dedisp(da, Rg.in16, Rg.dpw, st));
                 S.dedisp_launches++;
                 AA_W(cudaEventRecord(e1, st));
@@ -630,6 +641,7 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
     cudaError_t e;
     if ((e = dedisp_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
     if ((e = dedisp_sp_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
+    if ((e = dedisp_ws_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
     if ((e = sps_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
 
     if (d->device_arena) {
@@ -670,7 +682,7 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
             return fail(AA_ERR_CUDA, e);
         if ((e = cudaMemcpy(R.d_dtiles, R.h_dtiles.data(), R.h_dtiles.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess)
             return fail(AA_ERR_CUDA, e);
-        if (R.sp_tb && (e = cudaMemcpy(R.d_sp, R.h_sp.data(), R.h_sp.size() * sizeof(SpRecord), cudaMemcpyHostToDevice)) != cudaSuccess)
+        if (R.sp_tb && (e = cudaMemcpy(R.d_sp, R.sp_table(), R.sp_table_bytes(), cudaMemcpyHostToDevice)) != cudaSuccess)
             return fail(AA_ERR_CUDA, e);
     }
     *out = p;
@@ -700,6 +712,14 @@ int aa_plan_delays(const aa_plan *p, int32_t r, int32_t *out)
     const Range &R = p->ranges[r];
     AA_CUDA(cudaMemcpy(out, R.d_delays, R.h_delays.size() * 4, cudaMemcpyDeviceToHost));
     return AA_OK;
+}
+
+int aa_plan_dedisp_variant(const aa_plan *p, int32_t r)
+{
+    if (!p || r < 0 || r >= (int32_t)p->ranges.size()) return AA_ERR_INVALID;
+    const Range &R = p->ranges[r];
+    if (!R.sp_tb) return 0;
+    return (R.ws ? 3 : 1) + (R.sp_tb == 1024 ? 1 : 0);
 }
 
 int aa_run(aa_plan *p, const uint8_t *host_input, aa_candidate *out, uint64_t max_cands, uint64_t *n_cands,

@@ -63,6 +63,29 @@ bool sp_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_
                      int32_t &rows, int32_t &pbytes);
 // tb = 1024 (512 threads, one CTA per SM) or 512 (256 threads, two CTAs per SM)
 cudaError_t launch_dedisp_sp(const DedispArgs &a, int tb, cudaStream_t st);
+
+// ---- warp-specialised shared-pattern kernel (kernels_dedisp_ws.cu): record per (DM block, channel group) ----
+// Pattern k, channel i: row sample u is byte u + m_i + e_{k,i} of the staged channel row, m_i the
+// smallest shift of the channel over the block's patterns and 0 <= e_{k,i} <= 3.
+struct WsRecord {
+    int32_t rbase[kSpG];            // first staged sample of each channel row relative to col0 + t0 (multiple of 16)
+    uint16_t rbytes[kSpG];          // staged bytes of each channel row (multiple of 16)
+    uint16_t npat;                  // pattern rows (1..kSpMaxPat)
+    uint16_t nchunk;                // 8-sample chunks per pattern row
+    uint16_t nbatch;                // warp-sized batches of 31 chunks per pattern row
+    uint16_t pad;
+    // bits 0-15: i * sp_rows + (m_i & ~7), the 8-byte-aligned load offset of chunk 0 inside the staging
+    // slot; bits 16-20: 8 * (m_i & 3); bit 21: (m_i & 4) != 0
+    uint32_t chdesc[kSpG];
+    uint32_t esh[kSpG][2];          // byte k of the pair: 8 * e_{k,i}
+    uint32_t poff[kSpDB];           // byte offset, inside the pattern-row buffer, of trial d's word (tau 0, tau 1)
+};
+static_assert(sizeof(WsRecord) % 16 == 0, "records are fetched with 16-byte bulk copies");
+bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t tb, std::vector<WsRecord> &out,
+                     int32_t &rows, int32_t &pbytes);
+cudaError_t launch_dedisp_ws(const DedispArgs &a, int tb, cudaStream_t st);
+size_t dedisp_ws_smem_bytes(int rows, int pbytes);
+cudaError_t dedisp_ws_configure();
 size_t dedisp_sp_smem_bytes(int rows, int pbytes);
 cudaError_t dedisp_sp_configure();
 

@@ -1,0 +1,424 @@
+// Brute-force incoherent dedispersion, warp-specialised shared-pattern kernel
+// (BASELINE.json north_star):  D[d][tau] = sum_c y[c][tau + delta(c,d)], exact.
+//
+// Channels are taken in groups of kSpG = 4.  Inside a block of 64 consecutive trials the group's
+// rounded delays, relative to its first channel, form only a few distinct vectors ("patterns",
+// ws_tables.cu); the CTA sums the 4 channels once per pattern into a row of 16-bit sums and each
+// trial then adds ONE row sample per group.  Same integers, same sums, a quarter of the adds.
+//
+// CTA = 16 consumer warps + NPW producer warps, tile = 64 trials x TB samples, one stage per group:
+//   TMA       one producer lane issues cp.async.bulk (1-D, mbarrier complete_tx) for the 4 channel
+//             windows of stage s+2 and the plan-time record of stage s+4.
+//   producers a lane owns 8 consecutive row samples of EVERY pattern: per channel it loads one
+//             20-byte window, aligns it to the smallest shift with funnel shifts, and per pattern
+//             adds it with IDP.2A (dp2a: two byte adds into two 15-bit lanes, FMA pipe).  Rows are
+//             stored twice, as (s[2j], s[2j+1]) and (s[2j+1], s[2j+2]) pairs, so that any integer
+//             offset is one aligned 32-bit load (the 9th sample comes from the next lane by SHFL).
+//   consumers a warp owns 4 trials, a lane TB/64 words of 2 samples: acc16 += row word (SWAR).
+//             Every sp_flush groups the 16-bit lanes are added into the uint32 output tile (L2).
+//   full[] / empty[] mbarriers hand the three pattern-row buffers back and forth; nothing in the
+//   loop is CTA-wide.
+// No tensor cores: a gather-add, not a dense contraction.
+#include "aa_internal.h"
+
+namespace aa {
+
+namespace {
+
+constexpr int G = kSpG;
+constexpr int DB = kSpDB;
+constexpr int NCW = 16;                // consumer warps
+constexpr int NPW = 8;                 // producer warps
+constexpr int DPW = DB / NCW;          // trials per consumer warp
+constexpr int NBUF = 3;                // pattern-row buffers
+constexpr int NRAW = 6;                // staged channel-window slots
+constexpr int DIST = 4;                // windows are requested DIST stages ahead
+constexpr int NREC = 16;               // record ring
+constexpr int REC = (int)sizeof(WsRecord);
+constexpr int NT = 32 * (NCW + NPW);
+// Registers: the CTA is launched with 80 per thread (768 * 80 = 61440); the consumer warpgroups
+// then take 88 (64 accumulators + loads in flight) and the producer warpgroups drop to 64.
+constexpr int REG_CONS = 88, REG_PROD = 64;
+static_assert(DPW == 4, "trial offsets are fetched four at a time");
+static_assert(NCW % 4 == 0 && NPW % 4 == 0, "setmaxnreg works on warpgroups");
+static_assert(NCW * REG_CONS + NPW * REG_PROD <= (NCW + NPW) * 80, "register budget");
+
+__device__ __forceinline__ uint32_t smem_u32(const void *p)
+{
+    return (uint32_t)__cvta_generic_to_shared(p);
+}
+// mbarriers are addressed by their 32-bit shared-window address
+__device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
+{
+    asm volatile("mbarrier.init.shared::cta.b64 [%0], %1;" ::"r"(bar), "r"(count));
+}
+__device__ __forceinline__ void mbar_expect_tx(uint32_t bar, uint32_t bytes)
+{
+    asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+}
+__device__ __forceinline__ void mbar_arrive(uint32_t bar)
+{
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(bar) : "memory");
+}
+__device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity)
+{
+    uint32_t ok;
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "selp.u32 %0, 1, 0, p;\n\t}"
+        : "=r"(ok)
+        : "r"(bar), "r"(parity)
+        : "memory");
+    return ok != 0;
+}
+// Whole-warp wait: every lane observes the completed phase itself (acquire), and the lanes leave the
+// loop together, so the warp stays converged (lanes leaving one by one would split it for good).
+__device__ __forceinline__ void mbar_wait(uint32_t bar, uint32_t parity)
+{
+    while (!__all_sync(0xFFFFFFFFu, mbar_try(bar, parity))) {
+    }
+}
+// single-lane wait (inside a lane-0 section)
+__device__ __forceinline__ void mbar_wait_lane(uint32_t bar, uint32_t parity)
+{
+    while (!mbar_try(bar, parity)) {
+    }
+}
+__device__ __forceinline__ void sts128_if(uint32_t addr, uint32_t x, uint32_t y, uint32_t z, uint32_t w, uint32_t pred)
+{
+    asm volatile(
+        "{\n\t.reg .pred p;\n\t"
+        "setp.ne.u32 p, %5, 0;\n\t"
+        "@p st.shared.v4.u32 [%0], {%1, %2, %3, %4};\n\t}" ::"r"(addr),
+        "r"(x), "r"(y), "r"(z), "r"(w), "r"(pred)
+        : "memory");
+}
+__device__ __forceinline__ void bulk_g2s(uint32_t dst, const void *src, uint32_t bytes, uint32_t bar)
+{
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(dst),
+                 "l"(src), "r"(bytes), "r"(bar)
+                 : "memory");
+}
+
+// byte 0 / 2 of x times 1 plus byte 1 / 3 times 2^15: two samples into two 15-bit lanes (IDP.2A)
+__device__ __forceinline__ void dp2a_lo(uint32_t &acc, uint32_t x)
+{
+    asm("dp2a.lo.u32.u32 %0, %1, %2, %0;" : "+r"(acc) : "r"(0x80000001u), "r"(x));
+}
+__device__ __forceinline__ void dp2a_hi(uint32_t &acc, uint32_t x)
+{
+    asm("dp2a.hi.u32.u32 %0, %1, %2, %0;" : "+r"(acc) : "r"(0x80000001u), "r"(x));
+}
+
+// Pattern rows K0 .. K0+NPAT-1 of one batch (31 row chunks of 8 samples; lane 31 only feeds lane 30
+// its first word).  q: this lane's first window byte of channel 0, chunk offset included; dst: shared
+// address of this lane's four words of pattern 0's even copy; st: this lane stores; rowbytes: bytes per copy.
+template <int NPAT, int K0>
+__device__ __forceinline__ void build_batch(const WsRecord *R, const uint8_t *q, uint32_t dst, uint32_t st, uint32_t rowbytes)
+{
+    uint32_t acc[NPAT][4];
+#pragma unroll
+    for (int k = 0; k < NPAT; ++k)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[k][j] = 0;
+
+#pragma unroll
+    for (int i = 0; i < G; ++i) {
+        const uint32_t cd = R->chdesc[i];
+        const uint8_t *qi = q + (cd & 0xFFFFu);
+        const uint2 v0 = *reinterpret_cast<const uint2 *>(qi);
+        const uint2 v1 = *reinterpret_cast<const uint2 *>(qi + 8);
+        const uint32_t w4 = *reinterpret_cast<const uint32_t *>(qi + 16);
+        const bool up = (cd & 0x200000u) != 0;             // smallest shift >= 4 bytes: start one word later
+        const uint32_t t0 = up ? v0.y : v0.x, t1 = up ? v1.x : v0.y, t2 = up ? v1.y : v1.x, t3 = up ? w4 : v1.y;
+        const uint32_t sh = cd >> 16;                      // funnel shifts take the amount modulo 32
+        const uint32_t xs0 = __funnelshift_r(t0, t1, sh), xs1 = __funnelshift_r(t1, t2, sh),
+                       xs2 = __funnelshift_r(t2, t3, sh);
+        uint2 es = make_uint2(0, 0);
+        if (i > 0) es = *reinterpret_cast<const uint2 *>(R->esh[i]);
+#pragma unroll
+        for (int k = 0; k < NPAT; ++k) {
+            uint32_t x0 = xs0, x1 = xs1;
+            if (i > 0) {                                   // channel 0 is the reference: no extra shift
+                const int kk = K0 + k;
+                const uint32_t e8 = (kk < 4 ? es.x : es.y) >> (8 * (kk & 3));   // 8 * extra shift of pattern kk
+                x0 = __funnelshift_r(xs0, xs1, e8);
+                x1 = __funnelshift_r(xs1, xs2, e8);
+            }
+            dp2a_lo(acc[k][0], x0);
+            dp2a_hi(acc[k][1], x0);
+            dp2a_lo(acc[k][2], x1);
+            dp2a_hi(acc[k][3], x1);
+        }
+    }
+
+#pragma unroll
+    for (int k = 0; k < NPAT; ++k) {
+        // 15-bit lanes -> 16-bit lanes: w + (w & ~0x7FFF) moves lane 1 up by one bit
+        uint32_t c[4];
+#pragma unroll
+        for (int j = 0; j < 4; ++j) c[j] = acc[k][j] + (acc[k][j] & 0xFFFF8000u);
+        const uint32_t nx = __shfl_down_sync(0xFFFFFFFFu, c[0], 1);
+        const uint32_t d = dst + (uint32_t)(2 * (K0 + k)) * rowbytes;
+        sts128_if(d, c[0], c[1], c[2], c[3], st);
+        sts128_if(d + rowbytes, __byte_perm(c[0], c[1], 0x5432), __byte_perm(c[1], c[2], 0x5432),
+                  __byte_perm(c[2], c[3], 0x5432), __byte_perm(c[3], nx, 0x5432), st);
+    }
+}
+
+template <int TB>
+__global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
+{
+    constexpr int NP = TB / 64;            // 2-sample words per consumer lane
+
+    extern __shared__ __align__(128) uint8_t smem[];
+    const uint32_t ROWS = (uint32_t)a.sp_rows;
+    const uint32_t raw_bytes = G * ROWS;
+    const uint32_t pbytes = (uint32_t)a.sp_pbytes;
+    uint8_t *P0 = smem;                                     // [NBUF] pattern rows: [pattern][E|O][rowwords] uint32
+    uint8_t *raw0 = P0 + NBUF * pbytes;                     // [NRAW][G][ROWS] staged channel windows
+    uint8_t *rec0 = raw0 + NRAW * raw_bytes;                // [NREC][REC]
+    const uint32_t sm_P = smem_u32(P0), sm_raw = smem_u32(raw0), sm_rec = smem_u32(rec0);
+    const uint32_t rawfull = sm_rec + NREC * REC;           // [NRAW] windows of a stage landed
+    const uint32_t recfull = rawfull + 8 * NRAW;            // [NREC] record landed
+    const uint32_t full = recfull + 8 * NREC;               // [NBUF] every producer warp has built its part
+    const uint32_t empty = full + 8 * NBUF;                 // [NBUF] every consumer warp has used the rows
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int d0 = blockIdx.x * DB;
+    const int64_t t0 = (int64_t)blockIdx.y * TB;
+    const int nstages = (a.nchans + G - 1) / G;
+    const uint8_t *recs = static_cast<const uint8_t *>(a.sp_tab) + (size_t)blockIdx.x * nstages * REC;
+
+    if (tid == 0) {
+#pragma unroll
+        for (int j = 0; j < NRAW; ++j) mbar_init(rawfull + 8 * j, 1);
+#pragma unroll
+        for (int j = 0; j < NREC; ++j) mbar_init(recfull + 8 * j, 1);
+#pragma unroll
+        for (int j = 0; j < NBUF; ++j) {
+            mbar_init(full + 8 * j, NPW);
+            mbar_init(empty + 8 * j, NCW);
+        }
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+
+    if (warp >= NCW) {
+        // ================================ producers ================================================
+        asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REG_PROD));
+        const int pw = warp - NCW;
+        const uint8_t *in = static_cast<const uint8_t *>(a.in) + a.col0 + t0;
+
+        auto fetch_record = [&](int q) {        // one lane
+            const uint32_t bar = recfull + 8 * (q % NREC);
+            mbar_expect_tx(bar, REC);
+            bulk_g2s(sm_rec + (q % NREC) * REC, recs + (size_t)q * REC, REC, bar);
+        };
+        // one lane: the four channel windows of stage q (its record has landed) and the record of stage q+DIST
+        auto issue = [&](int q) {
+            mbar_wait_lane(recfull + 8 * (q % NREC), (uint32_t)((q / NREC) & 1));
+            const WsRecord *R = reinterpret_cast<const WsRecord *>(rec0 + (q % NREC) * REC);
+            uint32_t bytes = 0;
+#pragma unroll
+            for (int i = 0; i < G; ++i) bytes += R->rbytes[i];
+            const uint32_t bar = rawfull + 8 * (q % NRAW);
+            mbar_expect_tx(bar, bytes);
+            const uint32_t dst = sm_raw + (q % NRAW) * raw_bytes;
+#pragma unroll
+            for (int i = 0; i < G; ++i)
+                bulk_g2s(dst + i * ROWS, in + (size_t)(q * G + i) * a.pitch_in + R->rbase[i], R->rbytes[i], bar);
+            if (q + DIST < nstages) fetch_record(q + DIST);
+        };
+
+        if (pw == 0 && lane == 0) {
+            for (int q = 0; q < DIST && q < nstages; ++q) fetch_record(q);
+            for (int q = 0; q < DIST && q < nstages; ++q) issue(q);
+        }
+        __syncwarp();
+
+        uint32_t rot = 0;                       // batch b of a stage goes to producer (b + rot) % NPW
+        int buf = 0, rs = 0, ws = 0, iss = 0;   // s % NBUF, s % NREC, s % NRAW, s % NPW
+        uint32_t bph = 0, rph = 0, wph = 0;     // parities of the current use of those slots
+        for (int s = 0; s < nstages; ++s) {
+            // the producers take turns requesting the windows of stage s + DIST.  Its slot was last read
+            // by stage s + DIST - NRAW: every producer must be done with that one.
+            if (iss == pw && lane == 0 && s + DIST < nstages) {
+                const int f = s + DIST - NRAW;
+                if (f >= 0) mbar_wait_lane(full + 8 * (f % NBUF), (uint32_t)((f / NBUF) & 1));
+                issue(s + DIST);
+            }
+            __syncwarp();
+            mbar_wait(recfull + 8 * rs, rph);
+            mbar_wait(rawfull + 8 * ws, wph);
+            if (s >= NBUF) mbar_wait(empty + 8 * buf, bph ^ 1);
+
+            const WsRecord *R = reinterpret_cast<const WsRecord *>(rec0 + rs * REC);
+            const uint32_t nchunk = R->nchunk, nbatch = R->nbatch, npat = R->npat;
+            const uint32_t rowbytes = 16u * nchunk;
+            const uint8_t *rawslot = raw0 + ws * raw_bytes;
+            const uint32_t P = sm_P + buf * pbytes;
+            for (uint32_t b = ((uint32_t)pw + NPW - rot) % NPW; b < nbatch; b += NPW) {
+                const uint32_t chunk = b * 31u + (uint32_t)lane;
+                // chunk nchunk is read for its first sample only; nothing beyond it is read
+                const uint8_t *q = rawslot + 8u * (chunk < nchunk ? chunk : nchunk);
+                const uint32_t dst = P + 16u * chunk;
+                const uint32_t st = lane < 31 && chunk < nchunk;
+                switch (npat) {
+                    case 1: build_batch<1, 0>(R, q, dst, st, rowbytes); break;
+                    case 2: build_batch<2, 0>(R, q, dst, st, rowbytes); break;
+                    case 3: build_batch<3, 0>(R, q, dst, st, rowbytes); break;
+                    case 4: build_batch<4, 0>(R, q, dst, st, rowbytes); break;
+                    case 5: build_batch<5, 0>(R, q, dst, st, rowbytes); break;
+                    case 6: build_batch<6, 0>(R, q, dst, st, rowbytes); break;
+                    case 7:
+                        build_batch<4, 0>(R, q, dst, st, rowbytes);
+                        build_batch<3, 4>(R, q, dst, st, rowbytes);
+                        break;
+                    default:
+                        build_batch<4, 0>(R, q, dst, st, rowbytes);
+                        build_batch<4, 4>(R, q, dst, st, rowbytes);
+                        break;
+                }
+            }
+            rot = (rot + nbatch) % NPW;
+            __syncwarp();
+            if (lane == 0) mbar_arrive(full + 8 * buf);
+            if (++buf == NBUF) { buf = 0; bph ^= 1; }
+            if (++rs == NREC) { rs = 0; rph ^= 1; }
+            if (++ws == NRAW) { ws = 0; wph ^= 1; }
+            if (++iss == NPW) iss = 0;
+        }
+        return;
+    }
+
+    // ==================================== consumers ================================================
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REG_CONS));
+    uint32_t acc16[DPW][NP];
+#pragma unroll
+    for (int k = 0; k < DPW; ++k)
+#pragma unroll
+        for (int i = 0; i < NP; ++i) acc16[k][i] = 0;
+
+    const bool whole = d0 + DB <= a.ndms && t0 + TB <= (int64_t)a.ncols;   // CTA-uniform: no edge tests
+    uint32_t *otile = a.out + (size_t)(d0 + warp * DPW) * a.pitch_out + t0 + 2 * lane;
+
+    // adds the 16-bit lanes into the uint32 output tile (first time: plain store) and clears them
+    auto flush = [&](bool first) {
+        if (whole) {
+#pragma unroll
+            for (int k = 0; k < DPW; ++k) {
+                uint2 *orow = reinterpret_cast<uint2 *>(otile + (size_t)k * a.pitch_out);
+                if (first) {
+#pragma unroll
+                    for (int i = 0; i < NP; ++i) {
+                        __stcg(orow + 32 * i, make_uint2(acc16[k][i] & 0xFFFFu, acc16[k][i] >> 16));
+                        acc16[k][i] = 0;
+                    }
+                } else {
+#pragma unroll
+                    for (int h = 0; h < NP; h += 8) {
+                        uint2 v[8];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) v[i] = __ldcg(orow + 32 * (h + i));
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            v[i].x += acc16[k][h + i] & 0xFFFFu;
+                            v[i].y += acc16[k][h + i] >> 16;
+                            acc16[k][h + i] = 0;
+                            __stcg(orow + 32 * (h + i), v[i]);
+                        }
+                    }
+                }
+            }
+            return;
+        }
+#pragma unroll
+        for (int k = 0; k < DPW; ++k) {
+            const int d = d0 + warp * DPW + k;
+            uint32_t *orow = otile + (size_t)k * a.pitch_out;
+#pragma unroll
+            for (int i = 0; i < NP; ++i) {
+                const int64_t t = t0 + 2 * (lane + 32 * i);
+                const uint32_t lo = acc16[k][i] & 0xFFFFu, hi = acc16[k][i] >> 16;
+                acc16[k][i] = 0;
+                if (d >= a.ndms) continue;
+                if (t + 1 < a.ncols) {
+                    uint2 v = make_uint2(0, 0);
+                    if (!first) v = __ldcg(reinterpret_cast<const uint2 *>(orow + 64 * i));
+                    v.x += lo;
+                    v.y += hi;
+                    __stcg(reinterpret_cast<uint2 *>(orow + 64 * i), v);
+                } else if (t < a.ncols) {
+                    const uint32_t v = first ? 0u : __ldcg(orow + 64 * i);
+                    __stcg(orow + 64 * i, v + lo);
+                }
+            }
+        }
+    };
+
+    const int FL = a.sp_flush;
+    int since = 0;
+    bool first = true;
+    int buf = 0, rs = 0;
+    uint32_t bph = 0, rph = 0;
+    const uint8_t *Pl = P0 + lane * 4;
+    const uint8_t *poffs = rec0 + offsetof(WsRecord, poff) + warp * (DPW * 4);
+    for (int s = 0; s < nstages; ++s) {
+        mbar_wait(recfull + 8 * rs, rph);
+        mbar_wait(full + 8 * buf, bph);
+
+        // one row word per (trial, group, sample pair)
+        const uint8_t *P = Pl + buf * pbytes;
+        const uint4 po = *reinterpret_cast<const uint4 *>(poffs + rs * REC);
+        const uint32_t pof[4] = {po.x, po.y, po.z, po.w};
+#pragma unroll
+        for (int k = 0; k < DPW; ++k) {
+            const uint32_t *p = reinterpret_cast<const uint32_t *>(P + pof[k]);
+#pragma unroll
+            for (int i = 0; i < NP; ++i) acc16[k][i] += p[i * 32];
+        }
+        __syncwarp();
+        if (lane == 0) mbar_arrive(empty + 8 * buf);
+        if (++buf == NBUF) { buf = 0; bph ^= 1; }
+        if (++rs == NREC) { rs = 0; rph ^= 1; }
+
+        if (++since == FL) {
+            flush(first);
+            first = false;
+            since = 0;
+        }
+    }
+    if (since || first) flush(first);
+}
+
+template <int TB>
+cudaError_t launch_t(const DedispArgs &a, cudaStream_t st)
+{
+    dim3 grid((unsigned)((a.ndms + DB - 1) / DB), (unsigned)((a.ncols + TB - 1) / TB));
+    dedisp_ws_kernel<TB><<<grid, NT, dedisp_ws_smem_bytes(a.sp_rows, a.sp_pbytes), st>>>(a);
+    return cudaGetLastError();
+}
+
+}  // namespace
+
+size_t dedisp_ws_smem_bytes(int rows, int pbytes)
+{
+    return (size_t)NBUF * pbytes + (size_t)NRAW * G * rows + (size_t)NREC * REC + (NRAW + NREC + 2 * NBUF) * 8;
+}
+
+cudaError_t dedisp_ws_configure()
+{
+    cudaError_t e = cudaFuncSetAttribute(dedisp_ws_kernel<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(dedisp_ws_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+}
+
+cudaError_t launch_dedisp_ws(const DedispArgs &a, int tb, cudaStream_t st)
+{
+    if (a.ncols <= 0 || a.ndms <= 0) return cudaSuccess;
+    return tb == 1024 ? launch_t<1024>(a, st) : launch_t<512>(a, st);
+}
+
+}  // namespace aa

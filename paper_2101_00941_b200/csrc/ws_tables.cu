@@ -1,0 +1,111 @@
+// Plan-time tables of the warp-specialised shared-pattern dedispersion kernel
+// (kernels_dedisp_ws.cu).  Host code.
+//
+// For a block of kSpDB consecutive DM trials d and a group of kSpG adjacent channels c0..c0+G-1
+// write   delta(c0+i, d) = ref(d) + rel_i(d),   ref(d) = delta(c0, d).
+// rel(d) is a vector of small integers; because every delay is rounded on its own it jitters
+// between floor and ceil of the exact difference, so a block sees a handful of distinct vectors
+// ("patterns": 4.7 per 64 trials on the 4096-channel workloads).  For pattern k
+//     P_k[u] = sum_i y[c0+i][t0 + ref(d_first) + u + rel_i^k]
+// and then  sum_i y[c0+i][t0 + tau + delta(c0+i,d)] = P_{k(d)}[tau + ref(d) - ref(d_first)]  exactly.
+// The record lists, per (block, group): where each channel row's staged window starts and how long
+// it is, the smallest shift m_i of each channel and every pattern's extra shift e_{k,i} = shift - m_i,
+// and for every trial the position of its first word inside the pattern rows.
+#include <algorithm>
+#include <array>
+
+#include "aa_internal.h"
+
+namespace aa {
+
+bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t tb, std::vector<WsRecord> &out,
+                     int32_t &rows, int32_t &pbytes)
+{
+    constexpr int G = kSpG, DB = kSpDB;
+    const int nblk = (ndms + DB - 1) / DB, ngrp = (nchans + G - 1) / G;
+    out.assign((size_t)nblk * ngrp, WsRecord{});
+    int64_t max_rows = 16, max_pbytes = 16;
+    std::vector<std::array<int, G>> mins((size_t)nblk * ngrp);
+
+    for (int b = 0; b < nblk; ++b) {
+        const int dfirst = b * DB;
+        for (int g = 0; g < ngrp; ++g) {
+            WsRecord &R = out[(size_t)b * ngrp + g];
+            const int c0 = g * G;
+            // trials past ndms repeat the last trial; channels past nchans repeat the last channel's delay
+            // and read the zero rows that pad the input to a multiple of kSpG channels
+            auto dly = [&](int d, int i) {
+                return delays[(size_t)std::min(d, ndms - 1) * nchans + std::min(c0 + i, nchans - 1)];
+            };
+            const int ref0 = dly(dfirst, 0);
+
+            // distinct patterns of the block
+            std::array<int, G> pats[kSpMaxPat];
+            int npat = 0, kd[DB], off[DB];
+            for (int dl = 0; dl < DB; ++dl) {
+                const int d = dfirst + dl, ref = dly(d, 0);
+                std::array<int, G> rel{};
+                for (int i = 0; i < G; ++i) {
+                    rel[i] = dly(d, i) - ref;
+                    if (rel[i] < 0) return false;        // delays must not decrease with channel index
+                }
+                off[dl] = ref - ref0;
+                if (off[dl] < 0 || (dl && off[dl] < off[dl - 1])) return false;   // nor with the trial index
+                int k = 0;
+                while (k < npat && pats[k] != rel) ++k;
+                if (k == npat) {
+                    if (npat == kSpMaxPat) return false;
+                    pats[npat++] = rel;
+                }
+                kd[dl] = k;
+            }
+
+            const int offmax = off[DB - 1];
+            // trial d reads row words [off>>1, off>>1 + tb/2) of the (off&1) copy: samples 0 .. tb + offmax
+            const int nchunk = (tb + offmax + 1 + 7) / 8;
+            if (nchunk > 8000) return false;
+            int maxrb = 0;
+            for (int i = 0; i < G; ++i) {
+                int mn = pats[0][i], mx = pats[0][i];
+                for (int k = 1; k < npat; ++k) {
+                    mn = std::min(mn, pats[k][i]);
+                    mx = std::max(mx, pats[k][i]);
+                }
+                if (mx - mn > 3) return false;           // extra shifts are two bits
+                R.rbase[i] = (ref0 + mn) & ~(kAlign - 1);
+                const int m = ref0 + mn - R.rbase[i];    // smallest shift inside the staged row, 0..15
+                mins[(size_t)b * ngrp + g][i] = m;
+                for (int k = 0; k < npat; ++k) {
+                    const uint32_t e8 = 8u * (uint32_t)(pats[k][i] - mn);
+                    R.esh[i][k >> 2] |= e8 << (8 * (k & 3));
+                }
+                // a producer lane reads 20 bytes from the 8-byte boundary at or below 8*chunk + m, chunk <= nchunk
+                const int need = 8 * nchunk + (m & ~7) + 20;
+                const int rb = (need + 15) / 16 * 16;
+                if (rb > 16368) return false;
+                R.rbytes[i] = (uint16_t)rb;
+                maxrb = std::max(maxrb, rb);
+            }
+            R.npat = (uint16_t)npat;
+            R.nchunk = (uint16_t)nchunk;
+            R.nbatch = (uint16_t)((nchunk + 30) / 31);
+            const int rowwords = nchunk * 4;
+            for (int dl = 0; dl < DB; ++dl)
+                R.poff[dl] = (uint32_t)(((kd[dl] * 2 + (off[dl] & 1)) * rowwords + (off[dl] >> 1)) * 4);
+
+            max_rows = std::max<int64_t>(max_rows, maxrb);
+            max_pbytes = std::max<int64_t>(max_pbytes, (int64_t)npat * 2 * rowwords * 4);
+        }
+    }
+    rows = (int32_t)max_rows;
+    if ((int64_t)G * rows > 65535) return false;
+    for (size_t r = 0; r < out.size(); ++r)
+        for (int i = 0; i < G; ++i) {
+            const uint32_t m = (uint32_t)mins[r][i];
+            out[r].chdesc[i] = ((uint32_t)i * (uint32_t)rows + (m & ~7u)) | (8u * (m & 3u)) << 16 | ((m >> 2) & 1u) << 21;
+        }
+    pbytes = (int32_t)((max_pbytes + 127) / 128 * 128);
+    return true;
+}
+
+}  // namespace aa

@@ -84,6 +84,40 @@ def test_small_cases_bit_exact(B, case):
     assert len(ref) > 0
 
 
+@pytest.mark.parametrize("variant,code", [("ws1024", 4), ("ws512", 3), ("sp1024", 2), ("sp512", 1), ("plain", 0)])
+@pytest.mark.parametrize("case", [
+    dict(nchans=302, ndms=100, nsamp=21000, chunk_len=8192),                 # padded channel group, partial DM block, ragged tile
+    dict(nchans=1024, ndms=64, nsamp=9000, chunk_len=4096, foff=-0.2),      # four flushes of the 16-bit lanes
+])
+def test_every_dedispersion_kernel_bit_exact(B, monkeypatch, variant, code, case):
+    """Fine channels / fine DM steps so that the shared-pattern tables exist; AA_DEDISP picks the kernel."""
+    monkeypatch.setenv("AA_DEDISP", variant)
+    kw = dict(f_top=1500.0, foff=-0.5, dm_step=0.25, norm_block=1024, widths=(1, 2, 4, 8), thr=5.0)
+    kw.update(case)
+    w = _tiny(**kw)
+    buf, x = _pinned_fill(B, w)
+    with B.Plan(w, taps=list(range(w.ndms_total))) as plan:
+        assert plan.dedisp_variant(0) == code
+        cands, tap = plan.run(buf)
+        nout = plan.nout
+    ref, dense, geo = oracle.run(x, w, keep_dense=True)
+    assert np.array_equal(tap[:, :geo["nout"][0]], dense[0])
+    res = compare_candidates(cands, ref, w.snr_threshold)
+    assert res["only_gpu"] == 0 and res["only_oracle"] == 0
+
+
+def test_saturated_input_every_kernel(B, monkeypatch):
+    for variant in ("ws1024", "ws512", "sp1024", "plain"):
+        monkeypatch.setenv("AA_DEDISP", variant)
+        w = _tiny(nchans=1024, ndms=70, nsamp=9000, chunk_len=4096, f_top=1500.0, foff=-0.2, dm_step=0.25, norm_block=1024)
+        buf = B.pinned_empty(w.nbytes)
+        buf.numpy()[:] = 255                         # 16-bit lanes at their limit before every flush
+        with B.Plan(w, taps=list(range(w.ndms_total))) as plan:
+            cands, tap = plan.run(buf)
+            assert len(cands) == 0
+            assert np.all(tap[:, :plan.nout[0]] == 255 * w.nchans)
+
+
 def test_cfg1_full(B):
     w = I.workload(1)
     cands, ref, res = _check_against_oracle(B, w)
