@@ -285,8 +285,7 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
             auto allowed = [&](const char *name) { return !env || !*env || std::strcmp(env, name) == 0; };
             for (int tb : {1024, 512}) {
                 if (R.sp_tb || !allowed(tb == 1024 ? "ws1024" : "ws512")) continue;
-                if (ws_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, R.h_ws, R.sp_rows, R.sp_pbytes) &&
-                    dedisp_ws_smem_bytes(R.sp_rows, R.sp_pbytes) + 1024 <= 227 * 1024) {
+                if (ws_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, 226 * 1024, R.h_ws, R.sp_rows, R.sp_pbytes)) {
                     R.sp_tb = tb;
                     R.ws = true;
                 }

@@ -78,13 +78,22 @@ struct WsRecord {
     // slot; bits 16-20: 8 * (m_i & 3); bit 21: (m_i & 4) != 0
     uint32_t chdesc[kSpG];
     uint32_t esh[kSpG][2];          // byte k of the pair: 8 * e_{k,i}
-    uint32_t poff[kSpDB];           // byte offset, inside the pattern-row buffer, of trial d's word (tau 0, tau 1)
+    uint32_t pofs;                  // byte offset of this stage's pattern rows inside the shared-memory ring
+    int32_t dep;                    // the rows may be written once the consumers are done with stage dep (-1: at once)
+    uint32_t pad2[2];
+    uint32_t poff[kSpDB];           // byte offset, inside the ring, of trial d's word (tau 0, tau 1)
 };
 static_assert(sizeof(WsRecord) % 16 == 0, "records are fetched with 16-byte bulk copies");
-bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t tb, std::vector<WsRecord> &out,
-                     int32_t &rows, int32_t &pbytes);
+constexpr int kWsTeam = 2;          // producer warps that build one stage together
+constexpr int kWsSlots = 16;        // stages are ordered through barrier slots s % kWsSlots ...
+constexpr int kWsWindow = 8;        // ... so a stage never starts before stage s - kWsWindow has been consumed
+// smem_budget: dynamic shared memory the kernel may use; on success rows = bytes per staged channel row and
+// ring_bytes = size of the pattern-row ring (DedispArgs::sp_rows / sp_pbytes)
+bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t tb, size_t smem_budget,
+                     std::vector<WsRecord> &out, int32_t &rows, int32_t &ring_bytes);
 cudaError_t launch_dedisp_ws(const DedispArgs &a, int tb, cudaStream_t st);
-size_t dedisp_ws_smem_bytes(int rows, int pbytes);
+size_t dedisp_ws_fixed_smem_bytes(int rows);            // everything but the ring
+size_t dedisp_ws_smem_bytes(int rows, int ring_bytes);
 cudaError_t dedisp_ws_configure();
 size_t dedisp_sp_smem_bytes(int rows, int pbytes);
 cudaError_t dedisp_sp_configure();

@@ -6,18 +6,21 @@
 // ws_tables.cu); the CTA sums the 4 channels once per pattern into a row of 16-bit sums and each
 // trial then adds ONE row sample per group.  Same integers, same sums, a quarter of the adds.
 //
-// CTA = 16 consumer warps + NPW producer warps, tile = 64 trials x TB samples, one stage per group:
-//   TMA       one producer lane issues cp.async.bulk (1-D, mbarrier complete_tx) for the 4 channel
-//             windows of stage s+2 and the plan-time record of stage s+4.
-//   producers a lane owns 8 consecutive row samples of EVERY pattern: per channel it loads one
+// CTA = 16 consumer warps + 8 producer warps, tile = 64 trials x TB samples, one stage per group:
+//   producers work in teams of TEAM warps; a team owns every NTEAM-th stage.  Its leader requests
+//             the stage's 4 channel windows one turn ahead with cp.async.bulk (TMA 1-D, mbarrier
+//             complete_tx); every warp prefetches its own copy of the plan-time record (cp.async).
+//             A lane owns 8 consecutive row samples of EVERY pattern: per channel it loads one
 //             20-byte window, aligns it to the smallest shift with funnel shifts, and per pattern
 //             adds it with IDP.2A (dp2a: two byte adds into two 15-bit lanes, FMA pipe).  Rows are
 //             stored twice, as (s[2j], s[2j+1]) and (s[2j+1], s[2j+2]) pairs, so that any integer
 //             offset is one aligned 32-bit load (the 9th sample comes from the next lane by SHFL).
+//             Pattern rows live in a shared-memory ring whose offsets are fixed at plan time, so a
+//             stage takes exactly the room it needs and about six stages are in flight.
 //   consumers a warp owns 4 trials, a lane TB/64 words of 2 samples: acc16 += row word (SWAR).
 //             Every sp_flush groups the 16-bit lanes are added into the uint32 output tile (L2).
-//   full[] / empty[] mbarriers hand the three pattern-row buffers back and forth; nothing in the
-//   loop is CTA-wide.
+//   full[] / empty[] mbarrier rings (one slot per stage, modulo 16) order the two sides; nothing in
+//   the loop is CTA-wide.
 // No tensor cores: a gather-add, not a dense contraction.
 #include "aa_internal.h"
 
@@ -30,10 +33,11 @@ constexpr int DB = kSpDB;
 constexpr int NCW = 16;                // consumer warps
 constexpr int NPW = 8;                 // producer warps
 constexpr int DPW = DB / NCW;          // trials per consumer warp
-constexpr int NBUF = 3;                // pattern-row buffers
-constexpr int NRAW = 6;                // staged channel-window slots
-constexpr int DIST = 4;                // windows are requested DIST stages ahead
-constexpr int NREC = 16;               // record ring
+constexpr int TEAM = kWsTeam;          // producer warps per stage
+constexpr int NTEAM = NPW / TEAM;      // stages being built at the same time
+constexpr int NRAW = 2 * NTEAM;        // staged channel-window slots: two per team
+constexpr int NSLOT = kWsSlots;        // full[] / empty[] barrier slots (stage modulo NSLOT)
+constexpr int NRECBUF = 3;             // private record copies per producer warp (this turn, next two)
 constexpr int REC = (int)sizeof(WsRecord);
 constexpr int NT = 32 * (NCW + NPW);
 // Registers: the CTA is launched with 80 per thread (768 * 80 = 61440); the consumer warpgroups
@@ -47,6 +51,7 @@ __device__ __forceinline__ uint32_t smem_u32(const void *p)
 {
     return (uint32_t)__cvta_generic_to_shared(p);
 }
+constexpr uint32_t kSuspendNs = 20000;   // try_wait may park the thread this long; arrival wakes it earlier
 // mbarriers are addressed by their 32-bit shared-window address
 __device__ __forceinline__ void mbar_init(uint32_t bar, uint32_t count)
 {
@@ -65,10 +70,10 @@ __device__ __forceinline__ bool mbar_try(uint32_t bar, uint32_t parity)
     uint32_t ok;
     asm volatile(
         "{\n\t.reg .pred p;\n\t"
-        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2;\n\t"
+        "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], %2, %3;\n\t"
         "selp.u32 %0, 1, 0, p;\n\t}"
         : "=r"(ok)
-        : "r"(bar), "r"(parity)
+        : "r"(bar), "r"(parity), "r"(kSuspendNs)
         : "memory");
     return ok != 0;
 }
@@ -167,6 +172,27 @@ __device__ __forceinline__ void build_batch(const WsRecord *R, const uint8_t *q,
     }
 }
 
+__device__ __forceinline__ void cp_async16(uint32_t dst, const void *src)
+{
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
+}
+
+template <int NPAT_LO, int NPAT_HI>
+__device__ __forceinline__ void build_stage(const WsRecord *R, const uint8_t *rawslot, uint32_t P, uint32_t nchunk,
+                                            uint32_t nbatch, int member, int lane)
+{
+    const uint32_t rowbytes = 16u * nchunk;
+    for (uint32_t b = (uint32_t)member; b < nbatch; b += TEAM) {
+        const uint32_t chunk = b * 31u + (uint32_t)lane;
+        // chunk nchunk is read for its first sample only; nothing beyond it is read
+        const uint8_t *q = rawslot + 8u * (chunk < nchunk ? chunk : nchunk);
+        const uint32_t dst = P + 16u * chunk;
+        const uint32_t st = lane < 31 && chunk < nchunk;
+        build_batch<NPAT_LO, 0>(R, q, dst, st, rowbytes);
+        if (NPAT_HI > 0) build_batch<(NPAT_HI > 0 ? NPAT_HI : 1), NPAT_LO>(R, q, dst, st, rowbytes);
+    }
+}
+
 template <int TB>
 __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
 {
@@ -175,15 +201,14 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
     extern __shared__ __align__(128) uint8_t smem[];
     const uint32_t ROWS = (uint32_t)a.sp_rows;
     const uint32_t raw_bytes = G * ROWS;
-    const uint32_t pbytes = (uint32_t)a.sp_pbytes;
-    uint8_t *P0 = smem;                                     // [NBUF] pattern rows: [pattern][E|O][rowwords] uint32
-    uint8_t *raw0 = P0 + NBUF * pbytes;                     // [NRAW][G][ROWS] staged channel windows
-    uint8_t *rec0 = raw0 + NRAW * raw_bytes;                // [NREC][REC]
+    const uint32_t ring_bytes = (uint32_t)a.sp_pbytes;
+    uint8_t *P0 = smem;                                     // pattern-row ring: per stage [pattern][E|O][4 * nchunk] uint32
+    uint8_t *raw0 = P0 + ring_bytes;                        // [NRAW][G][ROWS] staged channel windows
+    uint8_t *rec0 = raw0 + NRAW * raw_bytes;                // [NPW][NRECBUF][REC] private record copies
     const uint32_t sm_P = smem_u32(P0), sm_raw = smem_u32(raw0), sm_rec = smem_u32(rec0);
-    const uint32_t rawfull = sm_rec + NREC * REC;           // [NRAW] windows of a stage landed
-    const uint32_t recfull = rawfull + 8 * NRAW;            // [NREC] record landed
-    const uint32_t full = recfull + 8 * NREC;               // [NBUF] every producer warp has built its part
-    const uint32_t empty = full + 8 * NBUF;                 // [NBUF] every consumer warp has used the rows
+    const uint32_t rawfull = sm_rec + NPW * NRECBUF * REC;  // [NRAW] windows of a stage landed
+    const uint32_t full = rawfull + 8 * NRAW;               // [NSLOT] the team has built the rows of stage s
+    const uint32_t empty = full + 8 * NSLOT;                // [NSLOT] every consumer warp has used them
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int d0 = blockIdx.x * DB;
@@ -195,10 +220,8 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
 #pragma unroll
         for (int j = 0; j < NRAW; ++j) mbar_init(rawfull + 8 * j, 1);
 #pragma unroll
-        for (int j = 0; j < NREC; ++j) mbar_init(recfull + 8 * j, 1);
-#pragma unroll
-        for (int j = 0; j < NBUF; ++j) {
-            mbar_init(full + 8 * j, NPW);
+        for (int j = 0; j < NSLOT; ++j) {
+            mbar_init(full + 8 * j, TEAM);
             mbar_init(empty + 8 * j, NCW);
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
@@ -208,88 +231,76 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
     if (warp >= NCW) {
         // ================================ producers ================================================
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REG_PROD));
-        const int pw = warp - NCW;
+        const int pw = warp - NCW, team = pw / TEAM, member = pw % TEAM;
         const uint8_t *in = static_cast<const uint8_t *>(a.in) + a.col0 + t0;
+        const uint32_t myrec = sm_rec + pw * (NRECBUF * REC);
+        const uint8_t *myrecp = rec0 + pw * (NRECBUF * REC);
 
-        auto fetch_record = [&](int q) {        // one lane
-            const uint32_t bar = recfull + 8 * (q % NREC);
-            mbar_expect_tx(bar, REC);
-            bulk_g2s(sm_rec + (q % NREC) * REC, recs + (size_t)q * REC, REC, bar);
+        // this warp's private copy of record q into copy slot j (asynchronous; one commit group)
+        auto prefetch_record = [&](int q, int j) {
+            if (q < nstages && lane < REC / 16) cp_async16(myrec + j * REC + lane * 16, recs + (size_t)q * REC + lane * 16);
+            asm volatile("cp.async.commit_group;" ::: "memory");
         };
-        // one lane: the four channel windows of stage q (its record has landed) and the record of stage q+DIST
-        auto issue = [&](int q) {
-            mbar_wait_lane(recfull + 8 * (q % NREC), (uint32_t)((q / NREC) & 1));
-            const WsRecord *R = reinterpret_cast<const WsRecord *>(rec0 + (q % NREC) * REC);
+        // leader lane: the four channel windows of stage q, described by record copy R, into window slot w
+        auto issue = [&](int q, const WsRecord *R, int w) {
             uint32_t bytes = 0;
 #pragma unroll
             for (int i = 0; i < G; ++i) bytes += R->rbytes[i];
-            const uint32_t bar = rawfull + 8 * (q % NRAW);
+            const uint32_t bar = rawfull + 8 * w;
             mbar_expect_tx(bar, bytes);
-            const uint32_t dst = sm_raw + (q % NRAW) * raw_bytes;
+            const uint32_t dst = sm_raw + w * raw_bytes;
 #pragma unroll
             for (int i = 0; i < G; ++i)
                 bulk_g2s(dst + i * ROWS, in + (size_t)(q * G + i) * a.pitch_in + R->rbase[i], R->rbytes[i], bar);
-            if (q + DIST < nstages) fetch_record(q + DIST);
         };
 
-        if (pw == 0 && lane == 0) {
-            for (int q = 0; q < DIST && q < nstages; ++q) fetch_record(q);
-            for (int q = 0; q < DIST && q < nstages; ++q) issue(q);
-        }
+        // turn it of this team is stage s = team + it * NTEAM; record copy slot it % 3, window slot 2 * team + (it & 1)
+        prefetch_record(team, 0);
+        prefetch_record(team + NTEAM, 1);
+        asm volatile("cp.async.wait_group 1;" ::: "memory");
+        __syncwarp();
+        if (member == 0 && lane == 0 && team < nstages) issue(team, reinterpret_cast<const WsRecord *>(myrecp), 2 * team);
         __syncwarp();
 
-        uint32_t rot = 0;                       // batch b of a stage goes to producer (b + rot) % NPW
-        int buf = 0, rs = 0, ws = 0, iss = 0;   // s % NBUF, s % NREC, s % NRAW, s % NPW
-        uint32_t bph = 0, rph = 0, wph = 0;     // parities of the current use of those slots
-        for (int s = 0; s < nstages; ++s) {
-            // the producers take turns requesting the windows of stage s + DIST.  Its slot was last read
-            // by stage s + DIST - NRAW: every producer must be done with that one.
-            if (iss == pw && lane == 0 && s + DIST < nstages) {
-                const int f = s + DIST - NRAW;
-                if (f >= 0) mbar_wait_lane(full + 8 * (f % NBUF), (uint32_t)((f / NBUF) & 1));
-                issue(s + DIST);
+        int rj = 0;                              // it % NRECBUF
+        for (int s = team, it = 0; s < nstages; s += NTEAM, ++it) {
+            const int rj1 = rj + 1 == NRECBUF ? 0 : rj + 1, rj2 = rj1 + 1 == NRECBUF ? 0 : rj1 + 1;
+            // record of the turn after next (its copy slot was last read two turns ago); then the records of
+            // this turn and the next one have landed
+            prefetch_record(s + 2 * NTEAM, rj2);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+            __syncwarp();
+            const WsRecord *R = reinterpret_cast<const WsRecord *>(myrecp + rj * REC);
+            if (member == 0 && lane == 0 && s + NTEAM < nstages) {
+                // next turn's windows go to the slot read one turn ago: the whole team must be done with it
+                const int f = s - NTEAM;
+                if (f >= 0) mbar_wait_lane(full + 8 * (f % NSLOT), (uint32_t)((f / NSLOT) & 1));
+                issue(s + NTEAM, reinterpret_cast<const WsRecord *>(myrecp + rj1 * REC), 2 * team + ((it + 1) & 1));
             }
             __syncwarp();
-            mbar_wait(recfull + 8 * rs, rph);
-            mbar_wait(rawfull + 8 * ws, wph);
-            if (s >= NBUF) mbar_wait(empty + 8 * buf, bph ^ 1);
-
-            const WsRecord *R = reinterpret_cast<const WsRecord *>(rec0 + rs * REC);
             const uint32_t nchunk = R->nchunk, nbatch = R->nbatch, npat = R->npat;
-            const uint32_t rowbytes = 16u * nchunk;
-            const uint8_t *rawslot = raw0 + ws * raw_bytes;
-            const uint32_t P = sm_P + buf * pbytes;
-            for (uint32_t b = ((uint32_t)pw + NPW - rot) % NPW; b < nbatch; b += NPW) {
-                const uint32_t chunk = b * 31u + (uint32_t)lane;
-                // chunk nchunk is read for its first sample only; nothing beyond it is read
-                const uint8_t *q = rawslot + 8u * (chunk < nchunk ? chunk : nchunk);
-                const uint32_t dst = P + 16u * chunk;
-                const uint32_t st = lane < 31 && chunk < nchunk;
-                switch (npat) {
-                    case 1: build_batch<1, 0>(R, q, dst, st, rowbytes); break;
-                    case 2: build_batch<2, 0>(R, q, dst, st, rowbytes); break;
-                    case 3: build_batch<3, 0>(R, q, dst, st, rowbytes); break;
-                    case 4: build_batch<4, 0>(R, q, dst, st, rowbytes); break;
-                    case 5: build_batch<5, 0>(R, q, dst, st, rowbytes); break;
-                    case 6: build_batch<6, 0>(R, q, dst, st, rowbytes); break;
-                    case 7:
-                        build_batch<4, 0>(R, q, dst, st, rowbytes);
-                        build_batch<3, 4>(R, q, dst, st, rowbytes);
-                        break;
-                    default:
-                        build_batch<4, 0>(R, q, dst, st, rowbytes);
-                        build_batch<4, 4>(R, q, dst, st, rowbytes);
-                        break;
-                }
+            const int dep = R->dep;              // last stage whose rows overlap this stage's room in the ring
+            if (dep >= 0) mbar_wait(empty + 8 * (dep % NSLOT), (uint32_t)((dep / NSLOT) & 1));
+            const int w = 2 * team + (it & 1);
+            mbar_wait(rawfull + 8 * w, (uint32_t)((it >> 1) & 1));
+
+            const uint8_t *rawslot = raw0 + w * raw_bytes;
+            const uint32_t P = sm_P + R->pofs;
+            switch (npat) {
+                case 1: build_stage<1, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 2: build_stage<2, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 3: build_stage<3, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 4: build_stage<4, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 5: build_stage<5, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 6: build_stage<6, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 7: build_stage<4, 3>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                default: build_stage<4, 4>(R, rawslot, P, nchunk, nbatch, member, lane); break;
             }
-            rot = (rot + nbatch) % NPW;
             __syncwarp();
-            if (lane == 0) mbar_arrive(full + 8 * buf);
-            if (++buf == NBUF) { buf = 0; bph ^= 1; }
-            if (++rs == NREC) { rs = 0; rph ^= 1; }
-            if (++ws == NRAW) { ws = 0; wph ^= 1; }
-            if (++iss == NPW) iss = 0;
+            if (lane == 0) mbar_arrive(full + 8 * (s % NSLOT));
+            rj = rj1;
         }
+        asm volatile("cp.async.wait_all;" ::: "memory");
         return;
     }
 
@@ -361,28 +372,27 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
     const int FL = a.sp_flush;
     int since = 0;
     bool first = true;
-    int buf = 0, rs = 0;
-    uint32_t bph = 0, rph = 0;
     const uint8_t *Pl = P0 + lane * 4;
-    const uint8_t *poffs = rec0 + offsetof(WsRecord, poff) + warp * (DPW * 4);
+    // this warp's four trial offsets (absolute inside the ring) come straight from the plan-time table in
+    // global memory (L2), one stage ahead
+    const uint8_t *poffs = recs + offsetof(WsRecord, poff) + warp * (DPW * 4);
+    uint4 po = __ldg(reinterpret_cast<const uint4 *>(poffs));
     for (int s = 0; s < nstages; ++s) {
-        mbar_wait(recfull + 8 * rs, rph);
-        mbar_wait(full + 8 * buf, bph);
+        const uint4 pn = __ldg(reinterpret_cast<const uint4 *>(poffs + (size_t)(s + 1 < nstages ? s + 1 : s) * REC));
+        const uint32_t slot = 8u * (uint32_t)(s % NSLOT);
+        mbar_wait(full + slot, (uint32_t)((s / NSLOT) & 1));
 
         // one row word per (trial, group, sample pair)
-        const uint8_t *P = Pl + buf * pbytes;
-        const uint4 po = *reinterpret_cast<const uint4 *>(poffs + rs * REC);
         const uint32_t pof[4] = {po.x, po.y, po.z, po.w};
 #pragma unroll
         for (int k = 0; k < DPW; ++k) {
-            const uint32_t *p = reinterpret_cast<const uint32_t *>(P + pof[k]);
+            const uint32_t *p = reinterpret_cast<const uint32_t *>(Pl + pof[k]);
 #pragma unroll
             for (int i = 0; i < NP; ++i) acc16[k][i] += p[i * 32];
         }
         __syncwarp();
-        if (lane == 0) mbar_arrive(empty + 8 * buf);
-        if (++buf == NBUF) { buf = 0; bph ^= 1; }
-        if (++rs == NREC) { rs = 0; rph ^= 1; }
+        if (lane == 0) mbar_arrive(empty + slot);
+        po = pn;
 
         if (++since == FL) {
             flush(first);
@@ -403,9 +413,14 @@ cudaError_t launch_t(const DedispArgs &a, cudaStream_t st)
 
 }  // namespace
 
-size_t dedisp_ws_smem_bytes(int rows, int pbytes)
+size_t dedisp_ws_fixed_smem_bytes(int rows)
 {
-    return (size_t)NBUF * pbytes + (size_t)NRAW * G * rows + (size_t)NREC * REC + (NRAW + NREC + 2 * NBUF) * 8;
+    return (size_t)NRAW * G * rows + (size_t)NPW * NRECBUF * REC + (NRAW + 2 * NSLOT) * 8;
+}
+
+size_t dedisp_ws_smem_bytes(int rows, int ring_bytes)
+{
+    return (size_t)ring_bytes + dedisp_ws_fixed_smem_bytes(rows);
 }
 
 cudaError_t dedisp_ws_configure()

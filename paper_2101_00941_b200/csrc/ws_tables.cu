@@ -18,13 +18,13 @@
 
 namespace aa {
 
-bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t tb, std::vector<WsRecord> &out,
-                     int32_t &rows, int32_t &pbytes)
+bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t tb, size_t smem_budget,
+                     std::vector<WsRecord> &out, int32_t &rows, int32_t &ring_bytes)
 {
     constexpr int G = kSpG, DB = kSpDB;
     const int nblk = (ndms + DB - 1) / DB, ngrp = (nchans + G - 1) / G;
     out.assign((size_t)nblk * ngrp, WsRecord{});
-    int64_t max_rows = 16, max_pbytes = 16;
+    int64_t max_rows = 16, max_pbytes = 16;      // largest staged channel row / largest stage of pattern rows
     std::vector<std::array<int, G>> mins((size_t)nblk * ngrp);
 
     for (int b = 0; b < nblk; ++b) {
@@ -90,7 +90,7 @@ bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_
             R.nchunk = (uint16_t)nchunk;
             R.nbatch = (uint16_t)((nchunk + 30) / 31);
             const int rowwords = nchunk * 4;
-            for (int dl = 0; dl < DB; ++dl)
+            for (int dl = 0; dl < DB; ++dl)       // relative to the stage's rows; the ring offset is added below
                 R.poff[dl] = (uint32_t)(((kd[dl] * 2 + (off[dl] & 1)) * rowwords + (off[dl] >> 1)) * 4);
 
             max_rows = std::max<int64_t>(max_rows, maxrb);
@@ -104,7 +104,39 @@ bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_
             const uint32_t m = (uint32_t)mins[r][i];
             out[r].chdesc[i] = ((uint32_t)i * (uint32_t)rows + (m & ~7u)) | (8u * (m & 3u)) << 16 | ((m >> 2) & 1u) << 21;
         }
-    pbytes = (int32_t)((max_pbytes + 127) / 128 * 128);
+    // The pattern rows of successive stages go round a ring in shared memory.  Offsets are fixed here, per DM
+    // block; dep = the latest earlier stage whose rows overlap the new ones (the producers wait until the
+    // consumers are done with it), never older than s - kWsWindow (barrier slots are reused modulo kWsSlots).
+    const size_t fixed = dedisp_ws_fixed_smem_bytes(rows);
+    if (smem_budget < fixed + (size_t)max_pbytes + 128) return false;
+    const int64_t C = (int64_t)((smem_budget - fixed) / 128 * 128);
+    if (C > 0x7FFFFFFF) return false;
+    for (int b = 0; b < nblk; ++b) {
+        struct Live { int s; int64_t lo, hi; };
+        std::vector<Live> live;
+        size_t oldest = 0;
+        int64_t head = 0;
+        int dep_run = -1;     // stages dropped from `live` are covered by an earlier wait only if dep never decreases
+        for (int g = 0; g < ngrp; ++g) {
+            WsRecord &R = out[(size_t)b * ngrp + g];
+            const int64_t size = ((int64_t)R.npat * 2 * R.nchunk * 16 + 127) / 128 * 128;
+            if (head + size > C) head = 0;
+            const int64_t lo = head, hi = head + size;
+            head = hi;
+            int dep = -1;
+            // stages are consumed in order: everything up to the newest overlapping one must be gone
+            for (size_t j = oldest; j < live.size(); ++j)
+                if (live[j].lo < hi && lo < live[j].hi) dep = live[j].s;
+            dep = std::max(dep, std::max(dep_run, g - kWsWindow));
+            dep_run = dep;
+            while (oldest < live.size() && live[oldest].s <= dep) ++oldest;
+            live.push_back({g, lo, hi});
+            R.pofs = (uint32_t)lo;
+            R.dep = dep;
+            for (int dl = 0; dl < DB; ++dl) R.poff[dl] += (uint32_t)lo;
+        }
+    }
+    ring_bytes = (int32_t)C;
     return true;
 }
 
