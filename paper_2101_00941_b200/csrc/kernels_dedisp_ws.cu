@@ -206,7 +206,9 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
     uint8_t *raw0 = P0 + ring_bytes;                        // [NRAW][G][ROWS] staged channel windows
     uint8_t *rec0 = raw0 + NRAW * raw_bytes;                // [NPW][NRECBUF][REC] private record copies
     const uint32_t sm_P = smem_u32(P0), sm_raw = smem_u32(raw0), sm_rec = smem_u32(rec0);
-    const uint32_t rawfull = sm_rec + NPW * NRECBUF * REC;  // [NRAW] windows of a stage landed
+    uint8_t *pof0 = rec0 + NPW * NRECBUF * REC;             // [NSLOT][DB] trial offsets of the stages in flight
+    const uint32_t sm_pof = smem_u32(pof0);
+    const uint32_t rawfull = sm_pof + NSLOT * DB * 4;       // [NRAW] windows of a stage landed
     const uint32_t full = rawfull + 8 * NRAW;               // [NSLOT] the team has built the rows of stage s
     const uint32_t empty = full + 8 * NSLOT;                // [NSLOT] every consumer warp has used them
 
@@ -281,6 +283,10 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
             const uint32_t nchunk = R->nchunk, nbatch = R->nbatch, npat = R->npat;
             const int dep = R->dep;              // last stage whose rows overlap this stage's room in the ring
             if (dep >= 0) mbar_wait(empty + 8 * (dep % NSLOT), (uint32_t)((dep / NSLOT) & 1));
+            // the stage's trial offsets go to its barrier slot (last used by stage s - NSLOT, consumed long ago)
+            if (member == 0 && lane < DB / 4)
+                *reinterpret_cast<uint4 *>(pof0 + (s % NSLOT) * (DB * 4) + lane * 16) =
+                    *reinterpret_cast<const uint4 *>(reinterpret_cast<const uint8_t *>(R->poff) + lane * 16);
             const int w = 2 * team + (it & 1);
             mbar_wait(rawfull + 8 * w, (uint32_t)((it >> 1) & 1));
 
@@ -373,26 +379,29 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
     int since = 0;
     bool first = true;
     const uint8_t *Pl = P0 + lane * 4;
-    // this warp's four trial offsets (absolute inside the ring) come straight from the plan-time table in
-    // global memory (L2), one stage ahead
-    const uint8_t *poffs = recs + offsetof(WsRecord, poff) + warp * (DPW * 4);
-    uint4 po = __ldg(reinterpret_cast<const uint4 *>(poffs));
+    // this warp's four trial offsets (absolute inside the ring) are published by the producers with the rows
+    const uint8_t *mypof = pof0 + warp * (DPW * 4);
     for (int s = 0; s < nstages; ++s) {
-        const uint4 pn = __ldg(reinterpret_cast<const uint4 *>(poffs + (size_t)(s + 1 < nstages ? s + 1 : s) * REC));
-        const uint32_t slot = 8u * (uint32_t)(s % NSLOT);
+        const uint32_t sl = (uint32_t)(s % NSLOT), slot = 8u * sl;
         mbar_wait(full + slot, (uint32_t)((s / NSLOT) & 1));
+        const uint4 po = *reinterpret_cast<const uint4 *>(mypof + sl * (DB * 4));
 
-        // one row word per (trial, group, sample pair)
+        // one row word per (trial, group, sample pair); eight loads in flight per batch
         const uint32_t pof[4] = {po.x, po.y, po.z, po.w};
 #pragma unroll
         for (int k = 0; k < DPW; ++k) {
             const uint32_t *p = reinterpret_cast<const uint32_t *>(Pl + pof[k]);
 #pragma unroll
-            for (int i = 0; i < NP; ++i) acc16[k][i] += p[i * 32];
+            for (int h = 0; h < NP; h += 8) {
+                uint32_t v[8];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) v[i] = p[(h + i) * 32];
+#pragma unroll
+                for (int i = 0; i < 8; ++i) acc16[k][h + i] += v[i];
+            }
         }
         __syncwarp();
         if (lane == 0) mbar_arrive(empty + slot);
-        po = pn;
 
         if (++since == FL) {
             flush(first);
@@ -415,7 +424,7 @@ cudaError_t launch_t(const DedispArgs &a, cudaStream_t st)
 
 size_t dedisp_ws_fixed_smem_bytes(int rows)
 {
-    return (size_t)NRAW * G * rows + (size_t)NPW * NRECBUF * REC + (NRAW + 2 * NSLOT) * 8;
+    return (size_t)NRAW * G * rows + (size_t)NPW * NRECBUF * REC + (size_t)NSLOT * DB * 4 + (NRAW + 2 * NSLOT) * 8;
 }
 
 size_t dedisp_ws_smem_bytes(int rows, int ring_bytes)
