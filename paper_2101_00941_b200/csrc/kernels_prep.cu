@@ -39,13 +39,84 @@ __global__ void __launch_bounds__(256) corner_turn_kernel(const uint8_t *__restr
     }
 }
 
+// Vector variant (nchans % 4 == 0; every time offset involved is a multiple of 16, see launch).
+// CTA tile = 128 times x 128 channels.  Warp w takes times [16w, 16w+16): every lane loads the 4
+// channels 4*lane..4*lane+3 of each of them (one 128-byte request per time row), transposes the 16 x 4
+// byte block in registers (PRMT) and stores four 16-byte pieces "16 times of one channel" into the
+// shared tile T[c][piece], pieces XOR-swizzled so that both the stores and the loads below are
+// conflict-free.  Then every thread moves four pieces to the ring with 16-byte stores (8 lanes
+// write 128 contiguous bytes of one channel row).
+constexpr int kCtT = 128, kCtC = 128;
+
+__device__ __forceinline__ void transpose4x4(uint32_t a, uint32_t b, uint32_t c, uint32_t d, uint32_t &o0,
+                                             uint32_t &o1, uint32_t &o2, uint32_t &o3)
+{
+    const uint32_t ab01 = __byte_perm(a, b, 0x5140), cd01 = __byte_perm(c, d, 0x5140);   // a0 b0 a1 b1
+    const uint32_t ab23 = __byte_perm(a, b, 0x7362), cd23 = __byte_perm(c, d, 0x7362);   // a2 b2 a3 b3
+    o0 = __byte_perm(ab01, cd01, 0x5410);
+    o1 = __byte_perm(ab01, cd01, 0x7632);
+    o2 = __byte_perm(ab23, cd23, 0x5410);
+    o3 = __byte_perm(ab23, cd23, 0x7632);
+}
+
+__global__ void __launch_bounds__(256) corner_turn_vec_kernel(const uint8_t *__restrict__ src, int64_t nt,
+                                                              int32_t nchans, int64_t t_abs0,
+                                                              uint8_t *__restrict__ ring, int64_t ring_pitch,
+                                                              int64_t ring_len, int64_t mirror)
+{
+    __shared__ uint4 T[kCtC][kCtT / 16];
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int64_t tb = (int64_t)blockIdx.x * kCtT;
+    const int32_t cb = blockIdx.y * kCtC;
+
+    {
+        const int32_t c = cb + 4 * lane;
+        const int64_t t = tb + 16 * warp;
+        uint32_t x[16];
+#pragma unroll
+        for (int i = 0; i < 16; ++i)
+            x[i] = (c < nchans && t + i < nt) ? __ldcs(reinterpret_cast<const uint32_t *>(src + (t + i) * nchans + c)) : 0u;
+        uint32_t o[4][4];            // [quarter of the 16 times][channel]
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            transpose4x4(x[4 * q], x[4 * q + 1], x[4 * q + 2], x[4 * q + 3], o[q][0], o[q][1], o[q][2], o[q][3]);
+#pragma unroll
+        for (int j = 0; j < 4; ++j)
+            T[4 * lane + j][warp ^ (lane & 7)] = make_uint4(o[0][j], o[1][j], o[2][j], o[3][j]);
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 4; ++k) {
+        const int item = threadIdx.x + 256 * k;          // 128 channels x 8 pieces
+        const int cl = item >> 3, piece = item & 7;
+        const int32_t c = cb + cl;
+        const int64_t t = tb + 16 * piece;
+        if (c < nchans && t < nt) {                      // nt is a multiple of 16
+            const uint4 v = T[cl][piece ^ ((cl >> 2) & 7)];
+            const int64_t col = (t_abs0 + t) % ring_len;
+            uint8_t *dst = ring + c * ring_pitch + col;
+            *reinterpret_cast<uint4 *>(dst) = v;
+            if (col < mirror) *reinterpret_cast<uint4 *>(dst + ring_len) = v;
+        }
+    }
+}
+
 cudaError_t launch_corner_turn(const uint8_t *src, int64_t nt, int32_t nchans, int64_t t_abs0,
                                uint8_t *ring, int64_t ring_pitch, int64_t ring_len, int64_t mirror,
                                cudaStream_t st)
 {
     if (nt <= 0) return cudaSuccess;
-    dim3 grid((unsigned)((nt + 63) / 64), (unsigned)((nchans + 63) / 64));
-    corner_turn_kernel<<<grid, 256, 0, st>>>(src, nt, nchans, t_abs0, ring, ring_pitch, ring_len, mirror);
+    // 16-sample pieces must not straddle the end of the ring, the mirror boundary or the end of the data
+    const bool vec = nchans % 4 == 0 && nt % 16 == 0 && t_abs0 % 16 == 0 && ring_len % 16 == 0 && mirror % 16 == 0 &&
+                     ring_pitch % 16 == 0 && (reinterpret_cast<uintptr_t>(src) & 3) == 0 &&
+                     (reinterpret_cast<uintptr_t>(ring) & 15) == 0;
+    if (vec) {
+        dim3 grid((unsigned)((nt + kCtT - 1) / kCtT), (unsigned)((nchans + kCtC - 1) / kCtC));
+        corner_turn_vec_kernel<<<grid, 256, 0, st>>>(src, nt, nchans, t_abs0, ring, ring_pitch, ring_len, mirror);
+    } else {
+        dim3 grid((unsigned)((nt + 63) / 64), (unsigned)((nchans + 63) / 64));
+        corner_turn_kernel<<<grid, 256, 0, st>>>(src, nt, nchans, t_abs0, ring, ring_pitch, ring_len, mirror);
+    }
     return cudaGetLastError();
 }
 

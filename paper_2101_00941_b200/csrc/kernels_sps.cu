@@ -51,7 +51,7 @@ struct Shared {
 };
 
 template <typename ACC>
-__global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const WidthTable wt)
+__global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const __grid_constant__ WidthTable wt)
 {
     extern __shared__ __align__(16) uint8_t dyn[];
     ACC *P = reinterpret_cast<ACC *>(dyn);          // exclusive prefix sums of the current tile
@@ -199,6 +199,347 @@ __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const WidthTab
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Cluster variant (32-bit boxcar sums, block_len % (4 C) == 0): the normalisation block of one DM row
+// is split over a thread-block cluster of C CTAs, each keeping its segment (<= kSegMax samples plus the
+// boxcar tail) in shared memory, so the dedispersed series is read from HBM exactly once:
+//   load     one cp.async.bulk (TMA 1-D) of the segment + tail onto an mbarrier;
+//   stats    the four passes run on shared memory; the 3-sigma selection |x - mu| <= 3 sigma (double, as
+//            in the oracle) is turned into the exact integer interval [lo, hi] it selects, the partial
+//            sums (m, sum x, sum x^2: exact integers) of every CTA are written into every CTA's shared
+//            memory (DSMEM) and added in rank order after a cluster barrier, so all CTAs form the same
+//            mu and sigma, bit for bit the single-CTA values;
+//   boxcars  in-place exclusive prefix sum of segment + tail (mod 2^32; differences are exact), then four
+//            taus per thread: B_w = P[tau+w] - P[tau] against the integer pre-filter; survivors take the
+//            same double-precision path as the generic kernel.
+constexpr int NT2 = 256;
+constexpr int kSegMax = 16384;
+constexpr int kMaxCluster = 8;
+
+struct SharedC {
+    uint64_t red[3][NT2 / 32];
+    uint64_t part[4][kMaxCluster][3];   // [pass][rank] partial sums, written by the CTA of that rank
+    uint64_t bar;                       // mbarrier of the bulk load
+    double mu, sigma;
+    uint64_t m;
+    uint32_t lo, hi;
+    int empty;
+    uint32_t thr_u[kMaxWidths];
+    double den[kMaxWidths];
+    int w[kMaxWidths];
+    uint32_t warp_tot[NT2 / 32];
+};
+
+__device__ __forceinline__ bool clip_pred(double x, double mu, double lim)
+{
+    return fabs(__dsub_rn(x, mu)) <= lim;
+}
+
+// The integers x in [0, 2^32) with |x - mu| <= lim (evaluated as the oracle does, in double) form an
+// interval, because the rounded difference is monotone in x.  Returns false if it is empty.
+__device__ bool clip_interval(double mu, double lim, uint32_t &lo, uint32_t &hi)
+{
+    const double top = 4294967295.0;
+    double l = ceil(mu - lim), h = floor(mu + lim);
+    if (l < 0.0) l = 0.0;
+    if (h > top) h = top;
+    if (!(l <= top) || !(h >= 0.0)) return false;
+    for (int it = 0; it < 4 && l > 0.0 && clip_pred(l - 1.0, mu, lim); ++it) l -= 1.0;
+    for (int it = 0; it < 8 && l < top && !clip_pred(l, mu, lim); ++it) l += 1.0;
+    for (int it = 0; it < 4 && h < top && clip_pred(h + 1.0, mu, lim); ++it) h += 1.0;
+    for (int it = 0; it < 8 && h > 0.0 && !clip_pred(h, mu, lim); ++it) h -= 1.0;
+    if (!clip_pred(l, mu, lim) || !clip_pred(h, mu, lim) || l > h) return false;
+    lo = (uint32_t)l;
+    hi = (uint32_t)h;
+    return true;
+}
+
+__device__ __forceinline__ uint32_t cluster_rank()
+{
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ void cluster_sync_all()
+{
+    asm volatile("barrier.cluster.arrive.release.aligned;\n\tbarrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void st_cluster_u64(const void *local, uint32_t rank, uint64_t v)
+{
+    uint32_t a = (uint32_t)__cvta_generic_to_shared(local), r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
+    asm volatile("st.shared::cluster.u64 [%0], %1;" ::"r"(r), "l"(v) : "memory");
+}
+
+__global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const __grid_constant__ WidthTable wt, const int C, const int seg)
+{
+    extern __shared__ __align__(16) uint8_t dyn[];
+    uint32_t *X = reinterpret_cast<uint32_t *>(dyn);     // segment + tail; later its exclusive prefix sums
+    __shared__ SharedC sh;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int d = blockIdx.y;
+    const uint32_t rank = C > 1 ? cluster_rank() : 0u;
+    const int64_t blk = blockIdx.x / C;
+    if (tid < kMaxWidths) sh.w[tid] = wt.w[tid];
+    const int64_t b0 = blk * a.block_len;
+    int64_t b1 = b0 + a.block_len;
+    if (b1 > a.nout_left) b1 = a.nout_left;
+    if (b0 >= b1 || b0 >= a.nemit) return;               // uniform over the cluster
+    const int64_t n_k = b1 - b0;
+    const uint32_t *row = a.D + (size_t)d * a.pitch;
+    const int64_t s0 = b0 + (int64_t)rank * seg;         // first column of this CTA's segment
+    const int64_t navail = a.ncols < a.nout_left ? (int64_t)a.ncols : a.nout_left;
+    const int halo = a.wmax - 1;
+    int64_t n_in = navail - s0;                          // columns this CTA holds: segment + boxcar tail
+    if (n_in > seg + halo) n_in = seg + halo;
+    if (n_in < 0) n_in = 0;
+    int64_t n_own = b1 - s0;                             // columns of the block inside the segment
+    if (n_own > seg) n_own = seg;
+    if (n_own < 0) n_own = 0;
+
+    // ---- load -------------------------------------------------------------------------------
+    const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&sh.bar);
+    if (tid == 0) {
+        asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"(bar));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+    }
+    __syncthreads();
+    if (C > 1) cluster_sync_all();                       // every CTA of the cluster runs before DSMEM is written
+    if (n_in > 0) {
+        if (tid == 0) {
+            // whole 16-byte pieces; the row pitch leaves room past the last column
+            const uint32_t bytes = (uint32_t)((n_in + 3) / 4 * 16);
+            asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+            asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                             (uint32_t)__cvta_generic_to_shared(X)),
+                         "l"(row + s0), "r"(bytes), "r"(bar)
+                         : "memory");
+        }
+        uint32_t ok = 0;
+        while (!ok)
+            asm volatile(
+                "{\n\t.reg .pred p;\n\t"
+                "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\t"
+                "selp.u32 %0, 1, 0, p;\n\t}"
+                : "=r"(ok)
+                : "r"(bar)
+                : "memory");
+    }
+
+    // ---- 1. statistics --------------------------------------------------------------------------
+    double mu = 0.0, sigma = 0.0;
+    const int n4 = (int)(n_own / 4);
+    for (int pass = 0; pass < 4; ++pass) {
+        uint32_t lo = 0u, span = 0xFFFFFFFFu;
+        bool run = true;
+        if (pass > 0) {
+            if (tid == 0) {
+                uint32_t l = 0, h = 0;
+                sh.empty = clip_interval(mu, __dmul_rn(3.0, sigma), l, h) ? 0 : 1;
+                sh.lo = l;
+                sh.hi = h;
+            }
+            __syncthreads();
+            run = !sh.empty;
+            lo = sh.lo;
+            span = sh.hi - lo;
+        }
+        uint64_t m = 0, S1 = 0, S2 = 0;
+        if (run) {
+            uint32_t mc = 0;
+            for (int i = tid; i < n4; i += NT2) {
+                const uint4 v = reinterpret_cast<const uint4 *>(X)[i];
+                const uint32_t xs[4] = {v.x, v.y, v.z, v.w};
+#pragma unroll
+                for (int k = 0; k < 4; ++k) {
+                    const bool sel = (xs[k] - lo) <= span;
+                    const uint32_t x = sel ? xs[k] : 0u;
+                    mc += sel ? 1u : 0u;
+                    S1 += x;
+                    S2 += (uint64_t)x * x;
+                }
+            }
+            for (int i = 4 * n4 + tid; i < n_own; i += NT2) {
+                const uint32_t x = X[i];
+                if ((x - lo) <= span) {
+                    mc += 1;
+                    S1 += x;
+                    S2 += (uint64_t)x * x;
+                }
+            }
+            m = mc;
+        }
+        m = warp_sum(m); S1 = warp_sum(S1); S2 = warp_sum(S2);
+        if (lane == 0) { sh.red[0][warp] = m; sh.red[1][warp] = S1; sh.red[2][warp] = S2; }
+        __syncthreads();
+        if (tid == 0) {
+            m = S1 = S2 = 0;
+            for (int w = 0; w < NT2 / 32; ++w) { m += sh.red[0][w]; S1 += sh.red[1][w]; S2 += sh.red[2][w]; }
+            if (C > 1) {
+                for (int r = 0; r < C; ++r) {
+                    st_cluster_u64(&sh.part[pass][rank][0], (uint32_t)r, m);
+                    st_cluster_u64(&sh.part[pass][rank][1], (uint32_t)r, S1);
+                    st_cluster_u64(&sh.part[pass][rank][2], (uint32_t)r, S2);
+                }
+            } else {
+                sh.part[pass][0][0] = m; sh.part[pass][0][1] = S1; sh.part[pass][0][2] = S2;
+            }
+        }
+        if (C > 1) cluster_sync_all(); else __syncthreads();
+        if (tid == 0) {
+            m = S1 = S2 = 0;
+            for (int r = 0; r < C; ++r) { m += sh.part[pass][r][0]; S1 += sh.part[pass][r][1]; S2 += sh.part[pass][r][2]; }
+            sh.m = m;
+            if (m) {
+                const unsigned __int128 N = (unsigned __int128)m * S2 - (unsigned __int128)S1 * S1;
+                const double dm = __ull2double_rn(m);
+                sh.mu = __ddiv_rn(__ull2double_rn(S1), dm);
+                sh.sigma = __dsqrt_rn(__ddiv_rn(u128_to_double(N), __dmul_rn(dm, dm)));
+            }
+        }
+        __syncthreads();
+        const uint64_t msel = sh.m;
+        if (msel) { mu = sh.mu; sigma = sh.sigma; }
+        __syncthreads();
+        if (!msel) break;
+    }
+    if (!(sigma > 0.0) || n_k < 32) return;
+
+    // ---- 2. per-width constants ---------------------------------------------------------------
+    if (tid < a.nwidths) {
+        const double w = (double)sh.w[tid];
+        const double den = __dmul_rn(sigma, __dsqrt_rn(w));
+        sh.den[tid] = den;
+        // B >= floor(w mu + thr sigma sqrt w) - 1 is necessary for S >= thr; clamped to the 32-bit sums
+        const long long bt = __double2ll_rd(w * mu + a.thr * den) - 1;
+        sh.thr_u[tid] = bt <= 0 ? 0u : (bt >= 0xFFFFFFFFll ? 0xFFFFFFFFu : (uint32_t)bt);
+    }
+
+    int64_t e = b1 < a.nemit ? b1 : (int64_t)a.nemit;     // taus [b0, e) of the block may emit
+    int64_t n_emit = e - s0;                              // ... [0, n_emit) of this segment
+    if (n_emit > seg) n_emit = seg;
+    if (n_emit <= 0) return;                              // nothing after this point is cluster-wide
+
+    // ---- 3. exclusive prefix sums in place: X[i] <- sum_{j<i} X[j], i <= n_in; constant beyond ------
+    {
+        const int total = seg + halo + 8;                 // slots the boxcar loop may read
+        int chunk = (int)((n_in + 1 + NT2 - 1) / NT2);    // slots 0 .. n_in
+        chunk |= 1;                                       // odd stride: conflict-free
+        const int64_t i0 = (int64_t)tid * chunk;
+        uint32_t run = 0;
+        for (int k = 0; k < chunk; ++k)
+            if (i0 + k < n_in) run += X[i0 + k];
+        uint32_t incl = run;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) {
+            const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+            if (lane >= o) incl += v;
+        }
+        if (lane == 31) sh.warp_tot[warp] = incl;
+        __syncthreads();
+        uint32_t pre = incl - run;
+        for (int w = 0; w < warp; ++w) pre += sh.warp_tot[w];
+        for (int k = 0; k < chunk; ++k) {
+            const int64_t i = i0 + k;
+            if (i < n_in) {
+                const uint32_t x = X[i];
+                X[i] = pre;
+                pre += x;
+            } else if (i == n_in) {
+                X[i] = pre;
+            }
+        }
+        __syncthreads();
+        const uint32_t last = X[n_in];
+        for (int64_t i = n_in + 1 + tid; i < total; i += NT2) X[i] = last;
+        __syncthreads();
+    }
+
+    // ---- 4. boxcars, four taus per thread ---------------------------------------------------------
+    const int ngroups = (int)((n_emit + 3) / 4);
+    const int nw = a.nwidths;
+    for (int g0 = 0; g0 < ngroups; g0 += NT2) {
+        const int g = g0 + tid;
+        uint32_t any = 0;
+        uint32_t p[4] = {0, 0, 0, 0};
+        if (g < ngroups) {
+            const uint4 pv = reinterpret_cast<const uint4 *>(X)[g];
+            p[0] = pv.x; p[1] = pv.y; p[2] = pv.z; p[3] = pv.w;
+            for (int j = 0; j < nw; ++j) {
+                const int w = sh.w[j];
+                const uint32_t th = sh.thr_u[j];
+                uint32_t q[4];
+                if ((w & 3) == 0) {
+                    const uint4 qv = *reinterpret_cast<const uint4 *>(X + 4 * g + w);
+                    q[0] = qv.x; q[1] = qv.y; q[2] = qv.z; q[3] = qv.w;
+                } else {
+#pragma unroll
+                    for (int k = 0; k < 4; ++k) q[k] = X[4 * g + k + w];
+                }
+#pragma unroll
+                for (int k = 0; k < 4; ++k) any |= ((q[k] - p[k]) >= th ? 1u : 0u) << k;
+            }
+        }
+        if (!__any_sync(0xffffffffu, any != 0)) continue;
+#pragma unroll
+        for (int k = 0; k < 4; ++k) {
+            const int tl = 4 * g + k;
+            const int64_t tau = s0 + tl;                  // column inside the sub-chunk
+            bool has = false;
+            int best_w = 0;
+            double best = 0.0;
+            if (((any >> k) & 1u) && tl < n_emit) {
+                for (int j = 0; j < nw; ++j) {
+                    const int w = sh.w[j];
+                    if (tau + w > a.nout_left) continue;
+                    const long long B = (long long)(uint32_t)(X[tl + w] - p[k]);
+                    const double num = __dsub_rn((double)B, __dmul_rn((double)w, mu));
+                    const double S = __ddiv_rn(num, sh.den[j]);
+                    if (best_w == 0 || S > best) { best = S; best_w = w; }
+                }
+                has = (best_w != 0) && (best >= a.thr);
+            }
+            const unsigned mask = __ballot_sync(0xffffffffu, has);
+            if (mask) {
+                uint32_t base = 0;
+                const int leader = __ffs(mask) - 1;
+                if (lane == leader) base = atomicAdd(a.count, (uint32_t)__popc(mask));
+                base = __shfl_sync(0xffffffffu, base, leader);
+                if (has) {
+                    const uint32_t slot = base + __popc(mask & ((1u << lane) - 1));
+                    if (slot < a.cap) {
+                        aa_candidate c;
+                        c.dm_index = a.dm_base + (uint32_t)d;
+                        c.t_start = (a.tau0 + (uint32_t)tau) * a.bin;
+                        c.width = (uint32_t)best_w * a.bin;
+                        c.snr = (float)best;
+                        a.cands[slot] = c;
+                    }
+                }
+            }
+        }
+    }
+}
+
+// cluster size and segment length of the cluster variant; false: use the generic kernel
+bool sps_cluster_shape(const SpsArgs &a, bool wide, int &C, int &seg)
+{
+    if (wide || a.block_len % 4 != 0 || a.pitch % 4 != 0 || (reinterpret_cast<uintptr_t>(a.D) & 15) != 0) return false;
+    if (a.wmax > 4096) return false;
+    for (C = 1; C <= kMaxCluster; C *= 2) {
+        if (a.block_len % (4 * C)) return false;
+        seg = a.block_len / C;
+        if (seg <= kSegMax) return true;
+    }
+    return false;
+}
+
+size_t sps_cluster_smem(const SpsArgs &a, int seg)
+{
+    return (size_t)(seg + a.wmax - 1 + 8) * 4;
+}
+
 size_t sps_smem(const SpsArgs &a, bool wide)
 {
     return (size_t)(TT + a.wmax + 8) * (wide ? 8 : 4);
@@ -211,13 +552,31 @@ cudaError_t sps_configure()
     cudaError_t e = cudaFuncSetAttribute(sps_kernel<uint32_t>, cudaFuncAttributeMaxDynamicSharedMemorySize,
                                          160 * 1024);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(sps_kernel<uint64_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    e = cudaFuncSetAttribute(sps_kernel<uint64_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(sps_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
 }
 
 cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, cudaStream_t st)
 {
     if (a.nemit <= 0 || a.ndms <= 0) return cudaSuccess;
     const unsigned nblk = (unsigned)((a.nemit + a.block_len - 1) / a.block_len);
+    int C = 1, seg = 0;
+    if (sps_cluster_shape(a, wide, C, seg)) {
+        cudaLaunchConfig_t cfg{};
+        cfg.gridDim = dim3(nblk * (unsigned)C, (unsigned)a.ndms);
+        cfg.blockDim = dim3(NT2);
+        cfg.dynamicSmemBytes = sps_cluster_smem(a, seg);
+        cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = (unsigned)C;
+        at[0].val.clusterDim.y = 1;
+        at[0].val.clusterDim.z = 1;
+        cfg.attrs = at;
+        cfg.numAttrs = 1;
+        return cudaLaunchKernelEx(&cfg, sps_cluster_kernel, a, wt, C, seg);
+    }
     dim3 grid(nblk, (unsigned)a.ndms);
     if (wide)
         sps_kernel<uint64_t><<<grid, NT, sps_smem(a, true), st>>>(a, wt);
