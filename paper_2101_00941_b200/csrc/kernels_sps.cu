@@ -228,6 +228,8 @@ struct SharedC {
     double den[kMaxWidths];
     int w[kMaxWidths];
     uint32_t warp_tot[NT2 / 32];
+    uint2 wl[kMaxWidths];               // (width, pre-filter threshold): multiples of 4 first, then the others
+    int na, nu;
 };
 
 __device__ __forceinline__ bool clip_pred(double x, double mu, double lim)
@@ -415,6 +417,16 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
         const long long bt = __double2ll_rd(w * mu + a.thr * den) - 1;
         sh.thr_u[tid] = bt <= 0 ? 0u : (bt >= 0xFFFFFFFFll ? 0xFFFFFFFFu : (uint32_t)bt);
     }
+    __syncthreads();
+    if (tid == 0) {
+        int n = 0;
+        for (int j = 0; j < a.nwidths; ++j)
+            if ((sh.w[j] & 3) == 0) sh.wl[n++] = make_uint2((uint32_t)sh.w[j], sh.thr_u[j]);
+        sh.na = n;
+        for (int j = 0; j < a.nwidths; ++j)
+            if ((sh.w[j] & 3) != 0) sh.wl[n++] = make_uint2((uint32_t)sh.w[j], sh.thr_u[j]);
+        sh.nu = n - sh.na;
+    }
 
     int64_t e = b1 < a.nemit ? b1 : (int64_t)a.nemit;     // taus [b0, e) of the block may emit
     int64_t n_emit = e - s0;                              // ... [0, n_emit) of this segment
@@ -427,9 +439,15 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
         int chunk = (int)((n_in + 1 + NT2 - 1) / NT2);    // slots 0 .. n_in
         chunk |= 1;                                       // odd stride: conflict-free
         const int64_t i0 = (int64_t)tid * chunk;
+        const bool inside = i0 + chunk <= n_in;           // the whole chunk holds data: no per-element tests
         uint32_t run = 0;
-        for (int k = 0; k < chunk; ++k)
-            if (i0 + k < n_in) run += X[i0 + k];
+        if (inside) {
+#pragma unroll 5
+            for (int k = 0; k < chunk; ++k) run += X[i0 + k];
+        } else {
+            for (int k = 0; k < chunk; ++k)
+                if (i0 + k < n_in) run += X[i0 + k];
+        }
         uint32_t incl = run;
 #pragma unroll
         for (int o = 1; o < 32; o <<= 1) {
@@ -440,14 +458,25 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
         __syncthreads();
         uint32_t pre = incl - run;
         for (int w = 0; w < warp; ++w) pre += sh.warp_tot[w];
-        for (int k = 0; k < chunk; ++k) {
-            const int64_t i = i0 + k;
-            if (i < n_in) {
-                const uint32_t x = X[i];
-                X[i] = pre;
+        if (inside) {
+            uint32_t *xp = X + i0;
+#pragma unroll 5
+            for (int k = 0; k < chunk; ++k) {
+                const uint32_t x = xp[k];
+                xp[k] = pre;
                 pre += x;
-            } else if (i == n_in) {
-                X[i] = pre;
+            }
+            if (i0 + chunk == n_in) xp[chunk] = pre;
+        } else {
+            for (int k = 0; k < chunk; ++k) {
+                const int64_t i = i0 + k;
+                if (i < n_in) {
+                    const uint32_t x = X[i];
+                    X[i] = pre;
+                    pre += x;
+                } else if (i == n_in) {
+                    X[i] = pre;
+                }
             }
         }
         __syncthreads();
@@ -456,44 +485,64 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
         __syncthreads();
     }
 
-    // ---- 4. boxcars, four taus per thread ---------------------------------------------------------
+    // ---- 4. boxcars, eight taus per thread -----------------------------------------------------------
+    // (two groups of four, NT2 groups apart, so that every 16-byte access of a warp is contiguous)
     const int ngroups = (int)((n_emit + 3) / 4);
-    const int nw = a.nwidths;
-    for (int g0 = 0; g0 < ngroups; g0 += NT2) {
+    const int nw = a.nwidths, na = sh.na, nu = sh.nu;
+    constexpr int GB = 4 * NT2;                          // distance of the second group in samples
+    for (int g0 = 0; g0 < ngroups; g0 += 2 * NT2) {
         const int g = g0 + tid;
         uint32_t any = 0;
-        uint32_t p[4] = {0, 0, 0, 0};
         if (g < ngroups) {
-            const uint4 pv = reinterpret_cast<const uint4 *>(X)[g];
-            p[0] = pv.x; p[1] = pv.y; p[2] = pv.z; p[3] = pv.w;
-            for (int j = 0; j < nw; ++j) {
-                const int w = sh.w[j];
-                const uint32_t th = sh.thr_u[j];
-                uint32_t q[4];
-                if ((w & 3) == 0) {
-                    const uint4 qv = *reinterpret_cast<const uint4 *>(X + 4 * g + w);
-                    q[0] = qv.x; q[1] = qv.y; q[2] = qv.z; q[3] = qv.w;
-                } else {
-#pragma unroll
-                    for (int k = 0; k < 4; ++k) q[k] = X[4 * g + k + w];
-                }
-#pragma unroll
-                for (int k = 0; k < 4; ++k) any |= ((q[k] - p[k]) >= th ? 1u : 0u) << k;
+            const bool two = g + NT2 < ngroups;          // else the second group repeats the first
+            const uint32_t *xg = X + 4 * g;
+            const int gb = two ? GB : 0;
+            const uint4 pa = *reinterpret_cast<const uint4 *>(xg), pb = *reinterpret_cast<const uint4 *>(xg + gb);
+            // widths that are multiples of 4: aligned 16-byte loads
+#pragma unroll 2
+            for (int j = 0; j < na; ++j) {
+                const uint2 wt2 = sh.wl[j];
+                const uint32_t th = wt2.y;
+                const uint4 qa = *reinterpret_cast<const uint4 *>(xg + wt2.x);
+                const uint4 qb = *reinterpret_cast<const uint4 *>(xg + wt2.x + gb);
+                any |= ((qa.x - pa.x) >= th ? 1u : 0u) | ((qa.y - pa.y) >= th ? 2u : 0u) | ((qa.z - pa.z) >= th ? 4u : 0u) |
+                       ((qa.w - pa.w) >= th ? 8u : 0u) | ((qb.x - pb.x) >= th ? 16u : 0u) | ((qb.y - pb.y) >= th ? 32u : 0u) |
+                       ((qb.z - pb.z) >= th ? 64u : 0u) | ((qb.w - pb.w) >= th ? 128u : 0u);
+            }
+            // the others: the aligned pieces around tau + w, shifted by w mod 4 (uniform)
+#pragma unroll 1
+            for (int j = na; j < na + nu; ++j) {
+                const uint2 wt2 = sh.wl[j];
+                const uint32_t th = wt2.y;
+                const int r = (int)(wt2.x & 3u);
+                const uint32_t *xq = xg + (wt2.x - (uint32_t)r);
+                const uint4 q0 = *reinterpret_cast<const uint4 *>(xq), q1 = *reinterpret_cast<const uint4 *>(xq + 4),
+                            q2 = *reinterpret_cast<const uint4 *>(xq + gb), q3 = *reinterpret_cast<const uint4 *>(xq + gb + 4);
+                uint32_t v0, v1, v2, v3, v4, v5, v6, v7;
+                if (r == 1) { v0 = q0.y; v1 = q0.z; v2 = q0.w; v3 = q1.x; v4 = q2.y; v5 = q2.z; v6 = q2.w; v7 = q3.x; }
+                else if (r == 2) { v0 = q0.z; v1 = q0.w; v2 = q1.x; v3 = q1.y; v4 = q2.z; v5 = q2.w; v6 = q3.x; v7 = q3.y; }
+                else { v0 = q0.w; v1 = q1.x; v2 = q1.y; v3 = q1.z; v4 = q2.w; v5 = q3.x; v6 = q3.y; v7 = q3.z; }
+                any |= ((v0 - pa.x) >= th ? 1u : 0u) | ((v1 - pa.y) >= th ? 2u : 0u) | ((v2 - pa.z) >= th ? 4u : 0u) |
+                       ((v3 - pa.w) >= th ? 8u : 0u) | ((v4 - pb.x) >= th ? 16u : 0u) | ((v5 - pb.y) >= th ? 32u : 0u) |
+                       ((v6 - pb.z) >= th ? 64u : 0u) | ((v7 - pb.w) >= th ? 128u : 0u);
             }
         }
+        if (g < ngroups && g + NT2 >= ngroups) any &= 15u;   // the repeated group is not evaluated twice
         if (!__any_sync(0xffffffffu, any != 0)) continue;
-#pragma unroll
-        for (int k = 0; k < 4; ++k) {
-            const int tl = 4 * g + k;
+#pragma unroll 1
+        for (int k = 0; k < 8; ++k) {
+            if (!__any_sync(0xffffffffu, (any >> k) & 1u)) continue;
+            const int tl = 4 * (g + (k >> 2) * NT2) + (k & 3);
             const int64_t tau = s0 + tl;                  // column inside the sub-chunk
             bool has = false;
             int best_w = 0;
             double best = 0.0;
             if (((any >> k) & 1u) && tl < n_emit) {
+                const uint32_t p0 = X[tl];
                 for (int j = 0; j < nw; ++j) {
                     const int w = sh.w[j];
                     if (tau + w > a.nout_left) continue;
-                    const long long B = (long long)(uint32_t)(X[tl + w] - p[k]);
+                    const long long B = (long long)(uint32_t)(X[tl + w] - p0);
                     const double num = __dsub_rn((double)B, __dmul_rn((double)w, mu));
                     const double S = __ddiv_rn(num, sh.den[j]);
                     if (best_w == 0 || S > best) { best = S; best_w = w; }
