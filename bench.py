@@ -47,6 +47,22 @@ def peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
 
 
+def ncu_traffic(kernel_name):
+    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
+    `ncu --set full` summary of this round (profiles/r1_dedisp_ws_ncu.txt); None if there is none for it."""
+    path = os.path.join(ROOT, "profiles", "r1_dedisp_ws_ncu.txt")
+    if not kernel_name.startswith("dedisp_ws_kernel<1024>") or not os.path.exists(path):
+        return None
+    tot = 0.0
+    scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}
+    with open(path) as f:
+        for line in f:
+            c = [x.strip() for x in line.split("|")]
+            if len(c) == 3 and c[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum") and c[1] in scale:
+                tot += float(c[2]) * scale[c[1]]
+    return tot or None
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
 
@@ -118,25 +134,30 @@ def pick_workload(k: int, world: int):
     return w, note
 
 
-def cpu_baseline(w, x, budget_rows=48):
-    """The oracle on a bounded sample: `budget_rows` DM trials x one normalisation block."""
+def cpu_baseline(w, x, budget_rows=48, budget_blocks=8):
+    """The oracle, as it stands, on a bounded sample: `budget_rows` DM trials of range 0 over the first
+    `budget_blocks` normalisation blocks (about 10-30 s of CPU work on the 4096-channel workloads)."""
     import oracle
     geo = oracle.geometry(w)
     r = 0
     rg = w.ranges[r]
     rows = sorted(set(np.linspace(0, rg.ndms - 1, budget_rows).astype(int).tolist()))
     L = w.norm_block // rg.bin
-    ntau = min(L + max(w.widths) - 1, geo["nout"][r])
+    # as many whole blocks as the rows of x that were generated allow
+    have = (x.shape[0] - geo["maxshift"]) // rg.bin - (max(w.widths) - 1)
+    nblocks = int(max(1, min(budget_blocks, have // L, geo["nout"][r] // L)))
+    nemit = min(nblocks * L, geo["nout"][r])
+    ntau = min(nemit + max(w.widths) - 1, geo["nout"][r])
     t0 = time.perf_counter()
     D = oracle.dedisperse(x, w, r, rows=rows, tau_first=0, ntau=ntau, geo=geo)
     ncand = 0
     for k in range(len(rows)):
-        tau, _, _ = oracle.sps_row(D[k], w, r, d_first=0, tau_a=0, tau_b=min(L, geo["nout"][r]), nout=geo["nout"][r])
+        tau, _, _ = oracle.sps_row(D[k], w, r, d_first=0, tau_a=0, tau_b=nemit, nout=geo["nout"][r])
         ncand += len(tau)
     dt = time.perf_counter() - t0
-    units = len(rows) * min(L, geo["nout"][r])
+    units = len(rows) * nemit
     return {"value": units / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
-            "sample": f"{len(rows)} DM trials x {min(L, geo['nout'][r])} output samples (one normalisation block) "
+            "sample": f"{len(rows)} DM trials x {nemit} output samples ({nblocks} normalisation blocks) "
                       f"of {w.name}, dedispersion + SPS, {dt:.1f} s", "seconds": dt}
 
 
@@ -148,12 +169,12 @@ def run_reference(args):
     # the oracle needs only the rows its sample touches: a short prefix of the observation
     import oracle
     geo_full = oracle.geometry(w)
-    need = w.norm_block + max(w.widths) * max(r.bin for r in w.ranges) + geo_full["maxshift"] + 64
+    need = args.ref_blocks * w.norm_block + max(w.widths) * max(r.bin for r in w.ranges) + geo_full["maxshift"] + 64
     ws = I.scaled(w, nsamp=min(w.nsamp, int(need)), pulses=w.pulses)
     x = I.fill(ws)
     times, val = [], None
     for i in range(args.warmup + args.steps):
-        cb = cpu_baseline(ws, x, budget_rows=args.ref_rows)
+        cb = cpu_baseline(ws, x, budget_rows=args.ref_rows, budget_blocks=args.ref_blocks)
         if i >= args.warmup:
             times.append(cb["seconds"]); val = cb
     units = val["value"] * val["seconds"]
@@ -176,7 +197,8 @@ def main():
     ap.add_argument("--workload", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--streams", type=int, default=0, help="n_streams of the e2e leg (0: the workload's)")
-    ap.add_argument("--ref-rows", type=int, default=48)
+    ap.add_argument("--ref-rows", type=int, default=48, help="DM trials of the oracle sample")
+    ap.add_argument("--ref-blocks", type=int, default=8, help="normalisation blocks of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--nsamp", type=int, default=0,
                     help="shorten the observation (profiling runs under ncu only; not a bench line)")
@@ -262,6 +284,9 @@ def main():
     t_copy = time.perf_counter() - tc0                 # the transfers alone
     plan = B.Plan(w, n_streams=1, chunk_len=L)
     plan_stats = plan.stats
+    variant = plan.dedisp_variant(0)
+    kernel_name = {0: "dedisp_kernel", 1: "dedisp_sp_kernel<512>", 2: "dedisp_sp_kernel<1024>",
+                   3: "dedisp_ws_kernel<512>", 4: "dedisp_ws_kernel<1024>"}.get(variant, "dedisp")
 
     def step_res():
         c, _ = plan.run_resident(dev_in, max_cands=max_cands, want_taps=False)
@@ -283,8 +308,8 @@ def main():
     achieved = adds_per_launch / avg_launch_s / 1e12              # T adds/s
     sm_mhz = pk.get("sm_max_mhz", 1965.0)
     peak = 148 * 128 * sm_mhz * 1e6 / 1e12                        # T lane-ops/s
-    roofline = {"kernel": "dedisp_kernel", "bound": "alu", "achieved": achieved, "peak": peak,
-                "unit": "T integer adds/s", "frac": achieved / peak, "traffic": None,
+    roofline = {"kernel": kernel_name, "bound": "alu", "achieved": achieved, "peak": peak,
+                "unit": "T integer adds/s", "frac": achieved / peak, "traffic": ncu_traffic(kernel_name),
                 "peak_source": f"148 SMs x 128 lanes x {sm_mhz:.0f} MHz ({pk_src}); one add per lane-op",
                 "avg_launch_ms": avg_launch_s * 1e3, "launches": d_n,
                 "share_of_step": {"dedisp": d_ms / wall_ms, "sps": s_ms / wall_ms, "prep": p_ms / wall_ms}}
@@ -313,7 +338,7 @@ def main():
             "setup": {"pin_s": t_pin, "generate_s": t_gen},
         }
         if not args.no_cpu_baseline:
-            cb = cpu_baseline(w, x, budget_rows=args.ref_rows)
+            cb = cpu_baseline(w, x, budget_rows=args.ref_rows, budget_blocks=args.ref_blocks)
             cb.pop("seconds", None)
             line["cpu_baseline"] = cb
         print(json.dumps(line))

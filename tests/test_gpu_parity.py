@@ -84,6 +84,25 @@ def test_small_cases_bit_exact(B, case):
     assert len(ref) > 0
 
 
+@pytest.mark.parametrize("case", [
+    dict(norm_block=32768, chunk_len=32768, nsamp=150000, ndms=6),            # SPS cluster of 2 CTAs per block
+    dict(norm_block=65536, chunk_len=65536, nsamp=200001, ndms=5),            # cluster of 4, ragged last block
+    dict(norm_block=131072, chunk_len=131072, nsamp=300000, ndms=4),          # cluster of 8
+    dict(norm_block=131072, chunk_len=131072, nsamp=140000, ndms=4),          # ... most CTAs of the cluster hold no data
+    dict(norm_block=262144, chunk_len=262144, nsamp=300000, ndms=3),          # too long for a cluster: generic kernel
+    dict(bins=(8,), norm_block=1040, chunk_len=8 * 1040, nsamp=50000, ndms=12),   # block of 130 samples: generic kernel
+    dict(widths=(2, 6, 7, 12, 20, 33), thr=4.5, norm_block=4096, chunk_len=8192),  # every width alignment
+    dict(nchans=30, nsamp=20011, ndms=33),                                    # byte-wise corner turn (nchans % 4 != 0)
+    dict(nchans=20, bins=(4,), widths=(1, 2, 4, 4096), nsamp=120000, chunk_len=32768, norm_block=32768, ndms=6, thr=4.0),  # long boxcar tail
+])
+def test_sps_and_corner_turn_variants(B, case):
+    """Shapes that select each SPS kernel (cluster sizes 1-8, generic fallback) and each corner-turn kernel."""
+    w = _tiny(**case)
+    cands, ref, res = _check_against_oracle(B, w)
+    assert res["only_gpu"] == 0 and res["only_oracle"] == 0 and res["width_ties"] == 0
+    assert len(ref) > 0
+
+
 @pytest.mark.parametrize("variant,code", [("ws1024", 4), ("ws512", 3), ("sp1024", 2), ("sp512", 1), ("plain", 0)])
 @pytest.mark.parametrize("case", [
     dict(nchans=302, ndms=100, nsamp=21000, chunk_len=8192),                 # padded channel group, partial DM block, ragged tile
