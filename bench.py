@@ -29,6 +29,10 @@ import time
 
 import numpy as np
 
+# one hardware work queue per stream: with the default of 8 connections the streams of a 8- or 16-stream plan
+# share queues and a stream's small D2H copy waits behind another stream's kernels (false dependency)
+os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")
+
 ROOT = os.path.dirname(os.path.abspath(__file__))
 sys.path.insert(0, ROOT)
 

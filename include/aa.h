@@ -85,6 +85,9 @@ typedef struct {
     const uint32_t *tap_dm_indices;
     /* capacity of each stream's device candidate list per sub-chunk; 0 -> 1<<21 */
     uint64_t max_cands_per_subchunk;
+    /* 1: every stream also gets a small pinned input staging buffer ((subchunk_len + halo) * nchans
+     * bytes) so that aa_run_staged can take an observation held in pageable memory */
+    int32_t  stage_input;
 } aa_plan_desc;
 
 typedef struct {
@@ -114,7 +117,23 @@ typedef struct {
     uint64_t n_stored;          /* records written to `out` (< n_candidates only on overflow) */
     int32_t  overflow;          /* 1 if any list was truncated */
     int32_t  n_streams;
+    uint64_t h2h_bytes;         /* aa_run_staged: bytes copied host -> pinned staging by the stream threads */
+    double   h2h_ms;            /* ... and the time those copies took, summed over threads */
 } aa_stats;
+
+/* Device timeline of one sub-chunk of the last run, in milliseconds after the start of the run (CUDA events
+ * on the sub-chunk's stream): the replacement for the paper's visual inspection of the profiler timeline
+ * (Fig. 3-4). */
+typedef struct {
+    uint32_t index;             /* sub-chunk j: raw samples [j*subchunk_len, (j+1)*subchunk_len) */
+    uint32_t stream;            /* stream / host thread that ran it (j mod n_streams) */
+    double   h2d_begin, h2d_end;        /* host-to-device copy of its new rows (equal if resident) */
+    double   prep_end;          /* corner turn done */
+    double   compute_begin;     /* halo of sub-chunk j-1 available: binning / dedispersion may start */
+    double   compute_end;       /* last range's SPS kernel done */
+    double   d2h_end;           /* candidate list in pinned staging */
+    double   dedisp_ms, sps_ms; /* kernel durations summed over ranges */
+} aa_subchunk_times;
 
 typedef struct aa_plan aa_plan;
 
@@ -160,6 +179,15 @@ int aa_plan_dedisp_variant(const aa_plan *p, int32_t r);
 int aa_run(aa_plan *p, const uint8_t *host_input, aa_candidate *out, uint64_t max_cands,
            uint64_t *n_cands, uint32_t *tap_out);
 
+/* The paper's own input arrangement: the observation sits in ordinary PAGEABLE host
+ * memory, too big to pin; every stream's host thread copies the rows of its next sub-chunk into its small
+ * pinned staging buffer (host -> host), from where they go to the device with cudaMemcpyAsync.  The
+ * host copy of sub-chunk j + n_streams runs while the stream still computes sub-chunk j.  Needs a plan
+ * created with stage_input = 1 (AA_ERR_INVALID otherwise); host_input may be pageable or pinned.
+ * Everything else, results included, is identical to aa_run. */
+int aa_run_staged(aa_plan *p, const uint8_t *host_input, aa_candidate *out, uint64_t max_cands,
+                  uint64_t *n_cands, uint32_t *tap_out);
+
 /* Same path with the observation already in device memory (uint8 [nsamp][nchans], device):
  * the H2D step is skipped, everything else is identical.  Used for kernel-only timing. */
 int aa_run_resident(aa_plan *p, const uint8_t *device_input, aa_candidate *out, uint64_t max_cands,
@@ -167,6 +195,10 @@ int aa_run_resident(aa_plan *p, const uint8_t *device_input, aa_candidate *out, 
 
 /* Timings and counters of the last aa_run / aa_run_resident on this plan. */
 int aa_get_stats(const aa_plan *p, aa_stats *out);
+
+/* Per-sub-chunk device timeline of the last run: writes min(max, n_subchunks) entries in sub-chunk order and
+ * the number of sub-chunks to *n. */
+int aa_get_timeline(const aa_plan *p, aa_subchunk_times *out, uint64_t max, uint64_t *n);
 
 /* NULL-safe.  Frees everything the plan allocated (not a caller-owned arena or streams). */
 void aa_destroy(aa_plan *p);

@@ -22,7 +22,7 @@ CAND_DTYPE = np.dtype([("dm_index", np.uint32), ("t_start", np.uint32),
 
 EXPORTS = ["aa_plan_arena_bytes", "aa_plan_create", "aa_plan_query", "aa_plan_nout", "aa_plan_delays",
            "aa_plan_dedisp_variant",
-           "aa_run", "aa_run_resident", "aa_get_stats", "aa_destroy", "aa_host_alloc", "aa_host_free",
+           "aa_run", "aa_run_staged", "aa_run_resident", "aa_get_stats", "aa_get_timeline", "aa_destroy", "aa_host_alloc", "aa_host_free",
            "aa_strerror", "aa_last_cuda_error"]
 
 
@@ -41,7 +41,7 @@ class PlanDescC(ctypes.Structure):
                 ("device_arena", ctypes.c_void_p), ("device_arena_bytes", ctypes.c_uint64),
                 ("streams", ctypes.POINTER(ctypes.c_void_p)),
                 ("ntap", ctypes.c_int32), ("tap_dm_indices", ctypes.POINTER(ctypes.c_uint32)),
-                ("max_cands_per_subchunk", ctypes.c_uint64)]
+                ("max_cands_per_subchunk", ctypes.c_uint64), ("stage_input", ctypes.c_int32)]
 
 
 class PlanInfoC(ctypes.Structure):
@@ -57,7 +57,13 @@ class StatsC(ctypes.Structure):
                 ("dedisp_ms", ctypes.c_double), ("sps_ms", ctypes.c_double),
                 ("dedisp_launches", ctypes.c_uint64), ("sps_launches", ctypes.c_uint64),
                 ("prep_launches", ctypes.c_uint64), ("n_candidates", ctypes.c_uint64), ("n_stored", ctypes.c_uint64),
-                ("overflow", ctypes.c_int32), ("n_streams", ctypes.c_int32)]
+                ("overflow", ctypes.c_int32), ("n_streams", ctypes.c_int32),
+                ("h2h_bytes", ctypes.c_uint64), ("h2h_ms", ctypes.c_double)]
+
+
+class SubchunkTimesC(ctypes.Structure):
+    _fields_ = [("index", ctypes.c_uint32), ("stream", ctypes.c_uint32)] + [(n, ctypes.c_double) for n in
+                ("h2d_begin", "h2d_end", "prep_end", "compute_begin", "compute_end", "d2h_end", "dedisp_ms", "sps_ms")]
 
 
 class AAError(RuntimeError):
@@ -91,13 +97,15 @@ def load_library() -> ctypes.CDLL:
     lib.aa_plan_delays.argtypes = [vp, i32, vp]
     lib.aa_plan_dedisp_variant.restype = ctypes.c_int
     lib.aa_plan_dedisp_variant.argtypes = [vp, i32]
-    for f in (lib.aa_run, lib.aa_run_resident):
+    for f in (lib.aa_run, lib.aa_run_staged, lib.aa_run_resident):
         f.restype = ctypes.c_int
         f.argtypes = [vp, vp, vp, u64, ctypes.POINTER(u64), vp]
     lib.aa_get_stats.restype = ctypes.c_int
     lib.aa_get_stats.argtypes = [vp, ctypes.POINTER(StatsC)]
     lib.aa_destroy.restype = None
     lib.aa_destroy.argtypes = [vp]
+    lib.aa_get_timeline.restype = ctypes.c_int
+    lib.aa_get_timeline.argtypes = [vp, ctypes.POINTER(SubchunkTimesC), u64, ctypes.POINTER(u64)]
     lib.aa_host_alloc.restype = ctypes.c_int
     lib.aa_host_alloc.argtypes = [ctypes.POINTER(vp), u64]
     lib.aa_host_free.restype = None
@@ -130,7 +138,7 @@ class Plan:
 
     def __init__(self, w, *, n_streams: Optional[int] = None, chunk_len: Optional[int] = None,
                  taps: Optional[Sequence[int]] = None, max_cands_per_subchunk: int = 0,
-                 torch_resources: bool = True):
+                 torch_resources: bool = True, stage_input: bool = False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the path has no CPU fallback")
@@ -152,6 +160,7 @@ class Plan:
         d.ntap = len(taps)
         d.tap_dm_indices = self._taps if taps else None
         d.max_cands_per_subchunk = int(max_cands_per_subchunk)
+        d.stage_input = 1 if stage_input else 0
         self._arena = None
         self._streams = None
         if torch_resources:
@@ -205,6 +214,11 @@ class Plan:
         ptr = host_input.data_ptr() if hasattr(host_input, "data_ptr") else host_input.ctypes.data
         return self._run(self.lib.aa_run, ptr, max_cands, want_taps)
 
+    def run_staged(self, host_input, max_cands: int = 1 << 22, want_taps: bool = True):
+        """aa_run_staged on an ordinary (pageable) numpy uint8 array; needs Plan(stage_input=True)."""
+        ptr = host_input.data_ptr() if hasattr(host_input, "data_ptr") else host_input.ctypes.data
+        return self._run(self.lib.aa_run_staged, ptr, max_cands, want_taps)
+
     def run_resident(self, device_input, max_cands: int = 1 << 22, want_taps: bool = True):
         """aa_run_resident on a torch CUDA uint8 tensor holding the whole observation."""
         return self._run(self.lib.aa_run_resident, device_input.data_ptr(), max_cands, want_taps)
@@ -213,6 +227,14 @@ class Plan:
         s = StatsC()
         _check(self.lib, self.lib.aa_get_stats(self.handle, ctypes.byref(s)))
         return {n: getattr(s, n) for n, _ in StatsC._fields_}
+
+    def timeline(self) -> list:
+        """Per-sub-chunk device timeline of the last run (ms after its start), as dicts."""
+        n = ctypes.c_uint64(0)
+        cap = int(self.info["n_subchunks"])
+        arr = (SubchunkTimesC * max(cap, 1))()
+        _check(self.lib, self.lib.aa_get_timeline(self.handle, arr, cap, ctypes.byref(n)))
+        return [{f: getattr(arr[i], f) for f, _ in SubchunkTimesC._fields_} for i in range(min(cap, int(n.value)))]
 
     def close(self):
         if getattr(self, "handle", None) is not None and self.handle:

@@ -69,10 +69,11 @@ struct Stream {
     uint32_t *h_count = nullptr;      // pinned
     aa_candidate *h_cands = nullptr;  // pinned
     uint32_t *h_tap = nullptr;        // pinned
+    uint8_t *h_stage = nullptr;       // pinned input staging (aa_run_staged), (L + halo) * nchans bytes
     std::vector<cudaEvent_t> ev;      // timing events
     // per-run accumulators
-    double h2d_ms = 0, d2h_ms = 0, prep_ms = 0, dedisp_ms = 0, sps_ms = 0;
-    uint64_t h2d_bytes = 0, d2h_bytes = 0, dedisp_launches = 0, sps_launches = 0, prep_launches = 0;
+    double h2d_ms = 0, d2h_ms = 0, prep_ms = 0, dedisp_ms = 0, sps_ms = 0, h2h_ms = 0;
+    uint64_t h2d_bytes = 0, d2h_bytes = 0, dedisp_launches = 0, sps_launches = 0, prep_launches = 0, h2h_bytes = 0;
 };
 
 }  // namespace
@@ -96,12 +97,14 @@ struct aa_plan {
     bool own_arena = false;
     uint8_t *d_ring = nullptr;
     std::vector<Stream> streams;
-    std::vector<cudaEvent_t> ev_loaded;
-    std::unique_ptr<std::atomic<int>[]> loaded, done;
+    std::vector<cudaEvent_t> ev_loaded, ev_dedisp, ev_copied;
+    std::unique_ptr<std::atomic<int>[]> loaded, done, dedisp_issued, copied;
     std::atomic<int> error{0};
     std::atomic<uint64_t> out_pos{0}, total{0};
     std::atomic<int> overflow{0};
     aa_stats stats{};
+    cudaEvent_t ev_start = nullptr;           // recorded on stream 0 when a run begins: origin of the timeline
+    std::vector<aa_subchunk_times> timeline;  // one entry per sub-chunk, written by its stream's thread
 };
 
 namespace {
@@ -337,7 +340,8 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         take(256);
     }
     p.arena_bytes = round_up(off, 256);
-    p.pinned_bytes = (uint64_t)p.n_streams * (256 + p.cap * sizeof(aa_candidate) + p.tap_stage_elems * 4);
+    p.pinned_bytes = (uint64_t)p.n_streams * (256 + p.cap * sizeof(aa_candidate) + p.tap_stage_elems * 4 +
+                                              (d->stage_input ? (p.L + p.halo) * (uint64_t)d->nchans : 0));
     return AA_OK;
 }
 
@@ -373,9 +377,13 @@ void destroy_plan(aa_plan *p)
         if (S.h_count) cudaFreeHost(S.h_count);
         if (S.h_cands) cudaFreeHost(S.h_cands);
         if (S.h_tap) cudaFreeHost(S.h_tap);
+        if (S.h_stage) cudaFreeHost(S.h_stage);
         if (S.own && S.st) cudaStreamDestroy(S.st);
     }
     for (auto e : p->ev_loaded) if (e) cudaEventDestroy(e);
+    for (auto e : p->ev_dedisp) if (e) cudaEventDestroy(e);
+    for (auto e : p->ev_copied) if (e) cudaEventDestroy(e);
+    if (p->ev_start) cudaEventDestroy(p->ev_start);
     if (p->own_arena && p->arena) cudaFree(p->arena);
     delete p;
 }
@@ -402,24 +410,51 @@ inline bool wait_flag(aa_plan *p, std::atomic<int> &f)
     } while (0)
 
 // One stream's host thread: issues every sub-chunk j = s, s+n_streams, ... and copies its results out.
-void worker(aa_plan *p, int s, const uint8_t *input, bool resident, aa_candidate *out, uint64_t max_cands,
+enum class Input { pinned, resident, staged };
+
+void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *out, uint64_t max_cands,
             uint32_t *tap_out)
 {
+    const bool resident = mode == Input::resident, staged = mode == Input::staged;
     Stream &S = p->streams[s];
     cudaStream_t st = S.st;
     const uint64_t L = p->L, halo = p->halo, R = p->ring_len, nsamp = p->desc.nsamp;
     const int nchans = p->desc.nchans;
     const int nr = (int)p->ranges.size();
 
+    // input rows [t_first, t_last) that sub-chunk j brings in (its own span shifted by the halo; j = 0 also the halo)
+    auto new_rows = [&](uint64_t j, uint64_t &t_first, uint64_t &nt) {
+        t_first = j == 0 ? 0 : j * L + halo;
+        const uint64_t t_last = std::min<uint64_t>((j + 1) * L + halo, nsamp);
+        nt = t_last > t_first ? t_last - t_first : 0;
+    };
+    // host -> pinned staging copy of sub-chunk j's rows by this stream's thread
+    auto stage = [&](uint64_t j) {
+        uint64_t t_first, nt;
+        new_rows(j, t_first, nt);
+        if (!nt) return;
+        const auto c0 = std::chrono::steady_clock::now();
+        std::memcpy(S.h_stage, input + t_first * (uint64_t)nchans, nt * (uint64_t)nchans);
+        S.h2h_ms += std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - c0).count();
+        S.h2h_bytes += nt * (uint64_t)nchans;
+    };
+    if (staged && (uint64_t)s < p->n_sub) stage((uint64_t)s);
+
     for (uint64_t j = (uint64_t)s; j < p->n_sub; j += (uint64_t)p->n_streams) {
         // the new rows overwrite ring columns last read by sub-chunks j-n_streams-1 and j-n_streams
         if (j >= (uint64_t)p->n_streams + 1 && !wait_flag(p, p->done[j - p->n_streams - 1])) return;
 
-        const uint64_t t_first = j == 0 ? 0 : j * L + halo;
-        const uint64_t t_last = std::min<uint64_t>((j + 1) * L + halo, nsamp);
-        const uint64_t nt = t_last > t_first ? t_last - t_first : 0;
-        const uint8_t *src = input + t_first * (uint64_t)nchans;
+        uint64_t t_first, nt;
+        new_rows(j, t_first, nt);
+        const uint8_t *src = staged ? S.h_stage : input + t_first * (uint64_t)nchans;
 
+        // First round only (every stream is idle and would start its copy at once): the copies take the link one
+        // after the other in sub-chunk order, so that sub-chunk 0 is complete after 1/n_streams of the time.
+        const bool first_round = !resident && j < (uint64_t)p->n_streams;
+        if (first_round && j > 0) {
+            if (!wait_flag(p, p->copied[j - 1])) return;
+            AA_W(cudaStreamWaitEvent(st, p->ev_copied[j - 1], 0));
+        }
         AA_W(cudaEventRecord(S.ev[0], st));
         if (!resident && nt) {
             AA_W(cudaMemcpyAsync(S.d_raw, src, nt * (uint64_t)nchans, cudaMemcpyHostToDevice, st));
@@ -427,6 +462,10 @@ void worker(aa_plan *p, int s, const uint8_t *input, bool resident, aa_candidate
             src = S.d_raw;
         }
         AA_W(cudaEventRecord(S.ev[1], st));
+        if (first_round) {
+            AA_W(cudaEventRecord(p->ev_copied[j], st));
+            p->copied[j].store(1, std::memory_order_release);
+        }
         AA_W(launch_corner_turn(src, (int64_t)nt, nchans, (int64_t)t_first, p->d_ring, (int64_t)p->ring_pitch,
                                 (int64_t)R, (int64_t)halo, st));
         S.prep_launches += nt ? 1 : 0;
@@ -438,6 +477,13 @@ void worker(aa_plan *p, int s, const uint8_t *input, bool resident, aa_candidate
         if (j > 0) {
             if (!wait_flag(p, p->loaded[j - 1])) return;
             AA_W(cudaStreamWaitEvent(st, p->ev_loaded[j - 1], 0));
+        }
+        // Dedispersion kernels fill the GPU: run them in sub-chunk order, each after the previous sub-chunk's
+        // last one.  Left to themselves the streams' kernels share the SMs, finish together and then all
+        // streams start their next copy at the same moment (a convoy: link and SMs idle in turn).
+        if (j > 0) {
+            if (!wait_flag(p, p->dedisp_issued[j - 1])) return;
+            AA_W(cudaStreamWaitEvent(st, p->ev_dedisp[j - 1], 0));
         }
         const uint64_t col0 = (j * L) % R;
         const uint64_t in_len = std::min<uint64_t>(L + halo, nsamp - j * L);
@@ -486,6 +532,10 @@ void worker(aa_plan *p, int s, const uint8_t *input, bool resident, aa_candidate
                 else AA_W(launch_dedisp(da, Rg.in16, Rg.dpw, st));
                 S.dedisp_launches++;
                 AA_W(cudaEventRecord(e1, st));
+                if (ri == nr - 1) {
+                    AA_W(cudaEventRecord(p->ev_dedisp[j], st));
+                    p->dedisp_issued[j].store(1, std::memory_order_release);
+                }
                 SpsArgs sa{};
                 sa.D = S.d_D;
                 sa.pitch = (int64_t)p->pitchD;
@@ -516,9 +566,19 @@ void worker(aa_plan *p, int s, const uint8_t *input, bool resident, aa_candidate
             } else {
                 AA_W(cudaEventRecord(e1, st));
                 AA_W(cudaEventRecord(e2, st));
+                if (ri == nr - 1) {
+                    AA_W(cudaEventRecord(p->ev_dedisp[j], st));
+                    p->dedisp_issued[j].store(1, std::memory_order_release);
+                }
             }
         }
         AA_W(cudaMemcpyAsync(S.h_count, S.d_count, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+        if (staged && j + (uint64_t)p->n_streams < p->n_sub) {
+            // the staging buffer is free once this sub-chunk's H2D is done: fill it for the next one while
+            // the stream computes
+            AA_W(cudaEventSynchronize(S.ev[1]));
+            stage(j + (uint64_t)p->n_streams);
+        }
         AA_W(cudaStreamSynchronize(st));           // stream-scoped wait, never device-wide
         p->done[j].store(1, std::memory_order_release);
 
@@ -551,12 +611,25 @@ void worker(aa_plan *p, int s, const uint8_t *input, bool resident, aa_candidate
             cudaEventElapsedTime(&ms, S.ev[kEvFixed + 3 * ri + 1], S.ev[kEvFixed + 3 * ri + 2]); S.sps_ms += ms;
         }
         cudaEventElapsedTime(&ms, S.ev[5], S.ev[6]); S.d2h_ms += ms;
+
+        aa_subchunk_times &T = p->timeline[j];
+        T = aa_subchunk_times{};
+        T.index = (uint32_t)j;
+        T.stream = (uint32_t)s;
+        auto at = [&](cudaEvent_t e) { float v = 0; cudaEventElapsedTime(&v, p->ev_start, e); return (double)v; };
+        T.h2d_begin = at(S.ev[0]); T.h2d_end = at(S.ev[1]); T.prep_end = at(S.ev[2]); T.compute_begin = at(S.ev[3]);
+        T.compute_end = at(S.ev[kEvFixed + 3 * (nr - 1) + 2]); T.d2h_end = at(S.ev[6]);
+        for (int ri = 0; ri < nr; ++ri) {
+            cudaEventElapsedTime(&ms, S.ev[kEvFixed + 3 * ri], S.ev[kEvFixed + 3 * ri + 1]); T.dedisp_ms += ms;
+            cudaEventElapsedTime(&ms, S.ev[kEvFixed + 3 * ri + 1], S.ev[kEvFixed + 3 * ri + 2]); T.sps_ms += ms;
+        }
     }
 }
 
-int run_impl(aa_plan *p, const uint8_t *input, bool resident, aa_candidate *out, uint64_t max_cands,
+int run_impl(aa_plan *p, const uint8_t *input, Input mode, aa_candidate *out, uint64_t max_cands,
              uint64_t *n_cands, uint32_t *tap_out)
 {
+    const bool resident = mode == Input::resident;
     if (!p || !input || !n_cands || (!out && max_cands)) return AA_ERR_INVALID;
     if (tap_out && p->taps_in.empty()) return AA_ERR_INVALID;
     g_last_cuda_error = 0;
@@ -565,21 +638,25 @@ int run_impl(aa_plan *p, const uint8_t *input, bool resident, aa_candidate *out,
     if (pe != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
     if (resident) {
         if (at.type != cudaMemoryTypeDevice && at.type != cudaMemoryTypeManaged) return AA_ERR_INVALID;
+    } else if (mode == Input::staged) {
+        if (!p->desc.stage_input || at.type == cudaMemoryTypeDevice) return AA_ERR_INVALID;
     } else if (at.type != cudaMemoryTypeHost) {
         return AA_ERR_NOT_PINNED;                   // never staged through pageable memory silently
     }
 
     const auto t0 = std::chrono::steady_clock::now();
-    for (uint64_t j = 0; j < p->n_sub; ++j) { p->loaded[j].store(0); p->done[j].store(0); }
+    for (uint64_t j = 0; j < p->n_sub; ++j) { p->loaded[j].store(0); p->done[j].store(0); p->dedisp_issued[j].store(0); }
+    for (int j = 0; j < p->n_streams; ++j) p->copied[j].store(0);
     p->error.store(0); p->out_pos.store(0); p->total.store(0); p->overflow.store(0);
     for (auto &S : p->streams) {
-        S.h2d_ms = S.d2h_ms = S.prep_ms = S.dedisp_ms = S.sps_ms = 0;
-        S.h2d_bytes = S.d2h_bytes = S.dedisp_launches = S.sps_launches = S.prep_launches = 0;
+        S.h2d_ms = S.d2h_ms = S.prep_ms = S.dedisp_ms = S.sps_ms = S.h2h_ms = 0;
+        S.h2d_bytes = S.d2h_bytes = S.dedisp_launches = S.sps_launches = S.prep_launches = S.h2h_bytes = 0;
     }
+    if (cudaEventRecord(p->ev_start, p->streams[0].st) != cudaSuccess) { g_last_cuda_error = (int)cudaGetLastError(); return AA_ERR_CUDA; }
     const int nthreads = (int)std::min<uint64_t>((uint64_t)p->n_streams, p->n_sub);
     std::vector<std::thread> th;
-    for (int s = 1; s < nthreads; ++s) th.emplace_back(worker, p, s, input, resident, out, max_cands, tap_out);
-    worker(p, 0, input, resident, out, max_cands, tap_out);
+    for (int s = 1; s < nthreads; ++s) th.emplace_back(worker, p, s, input, mode, out, max_cands, tap_out);
+    worker(p, 0, input, mode, out, max_cands, tap_out);
     for (auto &t : th) t.join();
     if (p->error.load()) {
         for (auto &S : p->streams) cudaStreamSynchronize(S.st);
@@ -606,6 +683,7 @@ int run_impl(aa_plan *p, const uint8_t *input, bool resident, aa_candidate *out,
         st.dedisp_ms += S.dedisp_ms; st.sps_ms += S.sps_ms;
         st.dedisp_launches += S.dedisp_launches; st.sps_launches += S.sps_launches;
         st.prep_launches += S.prep_launches;
+        st.h2h_bytes += S.h2h_bytes; st.h2h_ms += S.h2h_ms;
     }
     st.n_candidates = total;
     st.n_stored = stored;
@@ -664,6 +742,8 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
         if ((e = cudaHostAlloc((void **)&S.h_cands, p->cap * sizeof(aa_candidate), cudaHostAllocDefault)) != cudaSuccess) { cudaGetLastError(); return fail(AA_ERR_OOM, e); }
         if (p->tap_stage_elems)
             if ((e = cudaHostAlloc((void **)&S.h_tap, p->tap_stage_elems * 4, cudaHostAllocDefault)) != cudaSuccess) { cudaGetLastError(); return fail(AA_ERR_OOM, e); }
+        if (d->stage_input)
+            if ((e = cudaHostAlloc((void **)&S.h_stage, (p->L + p->halo) * (uint64_t)d->nchans, cudaHostAllocDefault)) != cudaSuccess) { cudaGetLastError(); return fail(AA_ERR_OOM, e); }
     }
     carve(*p);
     {
@@ -674,8 +754,18 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
     p->ev_loaded.assign(p->n_sub, nullptr);
     for (auto &ev : p->ev_loaded)
         if ((e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess) return fail(AA_ERR_CUDA, e);
+    if ((e = cudaEventCreate(&p->ev_start)) != cudaSuccess) return fail(AA_ERR_CUDA, e);
+    p->timeline.assign(p->n_sub, aa_subchunk_times{});
+    p->ev_dedisp.assign(p->n_sub, nullptr);
+    for (auto &ev : p->ev_dedisp)
+        if ((e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess) return fail(AA_ERR_CUDA, e);
+    p->ev_copied.assign(p->n_streams, nullptr);
+    for (auto &ev : p->ev_copied)
+        if ((e = cudaEventCreateWithFlags(&ev, cudaEventDisableTiming)) != cudaSuccess) return fail(AA_ERR_CUDA, e);
     p->loaded.reset(new std::atomic<int>[p->n_sub]);
     p->done.reset(new std::atomic<int>[p->n_sub]);
+    p->dedisp_issued.reset(new std::atomic<int>[p->n_sub]);
+    p->copied.reset(new std::atomic<int>[p->n_streams]);
     for (auto &R : p->ranges) {
         if ((e = cudaMemcpy(R.d_delays, R.h_delays.data(), R.h_delays.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess)
             return fail(AA_ERR_CUDA, e);
@@ -724,19 +814,34 @@ int aa_plan_dedisp_variant(const aa_plan *p, int32_t r)
 int aa_run(aa_plan *p, const uint8_t *host_input, aa_candidate *out, uint64_t max_cands, uint64_t *n_cands,
            uint32_t *tap_out)
 {
-    return run_impl(p, host_input, false, out, max_cands, n_cands, tap_out);
+    return run_impl(p, host_input, Input::pinned, out, max_cands, n_cands, tap_out);
+}
+
+int aa_run_staged(aa_plan *p, const uint8_t *host_input, aa_candidate *out, uint64_t max_cands, uint64_t *n_cands,
+                  uint32_t *tap_out)
+{
+    return run_impl(p, host_input, Input::staged, out, max_cands, n_cands, tap_out);
 }
 
 int aa_run_resident(aa_plan *p, const uint8_t *device_input, aa_candidate *out, uint64_t max_cands,
                     uint64_t *n_cands, uint32_t *tap_out)
 {
-    return run_impl(p, device_input, true, out, max_cands, n_cands, tap_out);
+    return run_impl(p, device_input, Input::resident, out, max_cands, n_cands, tap_out);
 }
 
 int aa_get_stats(const aa_plan *p, aa_stats *out)
 {
     if (!p || !out) return AA_ERR_INVALID;
     *out = p->stats;
+    return AA_OK;
+}
+
+int aa_get_timeline(const aa_plan *p, aa_subchunk_times *out, uint64_t max, uint64_t *n)
+{
+    if (!p || !n || (!out && max)) return AA_ERR_INVALID;
+    *n = p->timeline.size();
+    const uint64_t m = std::min<uint64_t>(max, p->timeline.size());
+    for (uint64_t i = 0; i < m; ++i) out[i] = p->timeline[i];
     return AA_OK;
 }
 

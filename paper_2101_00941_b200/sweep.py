@@ -18,9 +18,13 @@ There is no CPU fallback: it needs libaa.so and a CUDA device.
 from __future__ import annotations
 
 import argparse
+import os
 import hashlib
 import sys
 import time
+
+
+os.environ.setdefault("CUDA_DEVICE_MAX_CONNECTIONS", "32")   # one hardware queue per stream (scheduler)
 
 
 def main(argv=None) -> int:

@@ -155,6 +155,28 @@ def test_stream_and_chunk_invariance(B):
     assert all(o == outs[0] for o in outs[1:])
 
 
+def test_pageable_input_through_pinned_staging(B):
+    """aa_run_staged (pageable observation, small pinned staging, one copy thread per stream)
+    returns exactly what aa_run returns on the pinned copy; aa_run itself keeps refusing pageable memory."""
+    w = _tiny(nchans=64, nsamp=70000, n_streams=3, chunk_len=3 * 4096, ndms=48)
+    buf, x = _pinned_fill(B, w)
+    taps = list(range(w.ndms_total))
+    with B.Plan(w, taps=taps) as plan:
+        want, want_tap = plan.run(buf)
+        with pytest.raises(B.AAError):
+            plan.run_staged(np.array(x))                   # plan has no staging buffers
+    pageable = np.array(x)                                 # ordinary numpy memory
+    with B.Plan(w, taps=taps, stage_input=True) as plan:
+        got, got_tap = plan.run_staged(pageable)
+        st = plan.stats()
+        assert st["h2h_bytes"] == w.nbytes == st["h2d_bytes"]
+        with pytest.raises(B.AAError):
+            plan.run(pageable)
+        again, _ = plan.run(buf)                           # the same plan still takes pinned input directly
+    assert got.tobytes() == want.tobytes() == again.tobytes() and len(want) > 0
+    assert np.array_equal(got_tap, want_tap)
+
+
 def test_saturated_input_and_constant_input(B):
     w = _tiny(nchans=300, nsamp=9000, foff=-0.3, dm_step=4.0, chunk_len=4096, norm_block=2048)
     buf = B.pinned_empty(w.nbytes)
