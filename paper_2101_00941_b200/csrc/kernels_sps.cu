@@ -492,7 +492,7 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
     constexpr int GB = 4 * NT2;                          // distance of the second group in samples
     for (int g0 = 0; g0 < ngroups; g0 += 2 * NT2) {
         const int g = g0 + tid;
-        bool hit = false;                                // some (tau, width) of this thread passes the pre-filter
+        uint32_t any = 0;
         if (g < ngroups) {
             const bool two = g + NT2 < ngroups;          // else the second group repeats the first
             const uint32_t *xg = X + 4 * g;
@@ -505,8 +505,9 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
                 const uint32_t th = wt2.y;
                 const uint4 qa = *reinterpret_cast<const uint4 *>(xg + wt2.x);
                 const uint4 qb = *reinterpret_cast<const uint4 *>(xg + wt2.x + gb);
-                hit = hit || (qa.x - pa.x) >= th || (qa.y - pa.y) >= th || (qa.z - pa.z) >= th || (qa.w - pa.w) >= th ||
-                      (qb.x - pb.x) >= th || (qb.y - pb.y) >= th || (qb.z - pb.z) >= th || (qb.w - pb.w) >= th;
+                any |= ((qa.x - pa.x) >= th ? 1u : 0u) | ((qa.y - pa.y) >= th ? 2u : 0u) | ((qa.z - pa.z) >= th ? 4u : 0u) |
+                       ((qa.w - pa.w) >= th ? 8u : 0u) | ((qb.x - pb.x) >= th ? 16u : 0u) | ((qb.y - pb.y) >= th ? 32u : 0u) |
+                       ((qb.z - pb.z) >= th ? 64u : 0u) | ((qb.w - pb.w) >= th ? 128u : 0u);
             }
             // the others: the aligned pieces around tau + w, shifted by w mod 4 (uniform)
 #pragma unroll 1
@@ -521,21 +522,22 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
                 if (r == 1) { v0 = q0.y; v1 = q0.z; v2 = q0.w; v3 = q1.x; v4 = q2.y; v5 = q2.z; v6 = q2.w; v7 = q3.x; }
                 else if (r == 2) { v0 = q0.z; v1 = q0.w; v2 = q1.x; v3 = q1.y; v4 = q2.z; v5 = q2.w; v6 = q3.x; v7 = q3.y; }
                 else { v0 = q0.w; v1 = q1.x; v2 = q1.y; v3 = q1.z; v4 = q2.w; v5 = q3.x; v6 = q3.y; v7 = q3.z; }
-                hit = hit || (v0 - pa.x) >= th || (v1 - pa.y) >= th || (v2 - pa.z) >= th || (v3 - pa.w) >= th ||
-                      (v4 - pb.x) >= th || (v5 - pb.y) >= th || (v6 - pb.z) >= th || (v7 - pb.w) >= th;
+                any |= ((v0 - pa.x) >= th ? 1u : 0u) | ((v1 - pa.y) >= th ? 2u : 0u) | ((v2 - pa.z) >= th ? 4u : 0u) |
+                       ((v3 - pa.w) >= th ? 8u : 0u) | ((v4 - pb.x) >= th ? 16u : 0u) | ((v5 - pb.y) >= th ? 32u : 0u) |
+                       ((v6 - pb.z) >= th ? 64u : 0u) | ((v7 - pb.w) >= th ? 128u : 0u);
             }
         }
-        if (!__any_sync(0xffffffffu, hit)) continue;
-        // rare: every tau of a flagged thread takes the exact path (the pre-filter is only a necessary condition)
-        const int kn = (g < ngroups && g + NT2 < ngroups) ? 8 : 4;    // the repeated group is not evaluated twice
+        if (g < ngroups && g + NT2 >= ngroups) any &= 15u;   // the repeated group is not evaluated twice
+        if (!__any_sync(0xffffffffu, any != 0)) continue;
 #pragma unroll 1
         for (int k = 0; k < 8; ++k) {
+            if (!__any_sync(0xffffffffu, (any >> k) & 1u)) continue;
             const int tl = 4 * (g + (k >> 2) * NT2) + (k & 3);
             const int64_t tau = s0 + tl;                  // column inside the sub-chunk
             bool has = false;
             int best_w = 0;
             double best = 0.0;
-            if (hit && k < kn && tl < n_emit) {
+            if (((any >> k) & 1u) && tl < n_emit) {
                 const uint32_t p0 = X[tl];
                 for (int j = 0; j < nw; ++j) {
                     const int w = sh.w[j];

@@ -34,9 +34,12 @@ def main(argv=None) -> int:
     ap.add_argument("--runs", type=int, default=2, help="timed runs per leg (after one warm-up); best is kept")
     ap.add_argument("--nsamp", type=int, default=0, help="shorten the observation (smoke runs)")
     ap.add_argument("--no-resident", action="store_true", help="skip the kernels-alone leg")
+    ap.add_argument("--staged", action="store_true",
+                    help="observation in PAGEABLE memory, aa_run_staged through per-stream pinned staging (PAPER.md:57, :63)")
     ap.add_argument("--out", default="")
     args = ap.parse_args(argv)
 
+    import numpy as np
     import torch
     from . import binding as B
     from . import inputs as I
@@ -54,6 +57,7 @@ def main(argv=None) -> int:
     I.fill(w, x)
     t_gen = time.perf_counter() - t0 - t_pin
 
+    pageable = np.array(x) if args.staged else None      # ordinary, unpinned memory
     dev_in = None if args.no_resident else torch.empty(w.nbytes, dtype=torch.uint8, device="cuda")
     max_cands = 1 << 24
     rows, hashes = [], []
@@ -87,9 +91,12 @@ def main(argv=None) -> int:
             st.synchronize()
         t_xfer, _ = best_of(xfer)
 
-        with B.Plan(w, n_streams=n, chunk_len=w.chunk_len) as plan:
+        with B.Plan(w, n_streams=n, chunk_len=w.chunk_len, stage_input=args.staged) as plan:
             def e2e():
-                c, _ = plan.run(host, max_cands=max_cands, want_taps=False)
+                if args.staged:
+                    c, _ = plan.run_staged(pageable, max_cands=max_cands, want_taps=False)
+                else:
+                    c, _ = plan.run(host, max_cands=max_cands, want_taps=False)
                 return c, plan.stats()
             t_wall, (cands, st) = best_of(e2e)
             units = plan.info["dm_trial_samples"]
@@ -108,7 +115,8 @@ def main(argv=None) -> int:
         longest = t_xfer if not (t_kern == t_kern) else max(t_xfer, t_kern)
         rows.append((n, L, t_wall, t_xfer, t_kern, longest / t_wall, st["h2d_bytes"] / t_xfer / 1e9,
                      st["h2d_bytes"] / t_wall / 1e9, st["d2h_bytes"] / max(st["d2h_ms"], 1e-9) / 1e6,
-                     units / t_wall, w.nsamp * w.tsamp / t_wall, len(cands), h))
+                     units / t_wall, w.nsamp * w.tsamp / t_wall, len(cands), h,
+                     st["h2h_bytes"] / max(st["h2h_ms"], 1e-9) / 1e6 * n if args.staged else 0.0))
 
     lines = [f"# Stream sweep, workload {w.name}: {w.nchans} channels x {w.nsamp} samples, {w.ndms_total} DM trials, "
              f"time chunks of {w.chunk_len} samples",
@@ -120,9 +128,13 @@ def main(argv=None) -> int:
              "| streams | sub-chunk | T_wall s | T_xfer s | T_kern s | overlap eff. | H2D alone GB/s | H2D in run GB/s | D2H GB/s | DM-trial*samples/s | real-time factor | candidates | sha256[:16] |",
              "|---|---|---|---|---|---|---|---|---|---|---|---|---|"]
     for r in rows:
-        lines.append(f"| {r[0]} | {r[1]} | {r[2]:.3f} | {r[3]:.3f} | {r[4]:.3f} | {r[5]:.3f} | {r[6]:.1f} | {r[7]:.1f} | "
+        eff = f"{r[5]:.3f}" if r[4] == r[4] else "n/a"      # needs the kernels-alone leg
+        lines.append(f"| {r[0]} | {r[1]} | {r[2]:.3f} | {r[3]:.3f} | {r[4]:.3f} | {eff} | {r[6]:.1f} | {r[7]:.1f} | "
                      f"{r[8]:.2f} | {r[9]:.3e} | {r[10]:.1f} | {r[11]} | {r[12]} |")
     same = len(set(hashes)) == 1
+    if args.staged:
+        lines += ["", "Input held in pageable memory (aa_run_staged): host-to-pinned-staging copies by one thread per stream, "
+                  "aggregate rate while copying: " + ", ".join(f"{r[0]} streams {r[13]:.1f} GB/s" for r in rows) + "."]
     lines += ["", f"Sorted candidate lists identical across the sweep: **{same}**.",
               "overlap eff. = max(T_xfer, T_kern) / T_wall (1.0 = transfers fully hidden behind the longer leg)."]
     text = "\n".join(lines) + "\n"

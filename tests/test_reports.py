@@ -1,0 +1,38 @@
+"""Host logic of the timeline report (no GPU): interval unions and the copy/compute overlap figure."""
+import pytest
+
+from paper_2101_00941_b200 import timeline as T
+
+
+def _entry(j, h0, h1, p1, c0, c1):
+    return {"index": j, "stream": j % 2, "h2d_begin": h0, "h2d_end": h1, "prep_end": p1, "compute_begin": c0,
+            "compute_end": c1, "d2h_end": c1, "dedisp_ms": c1 - c0, "sps_ms": 0.0}
+
+
+def test_union_and_intersection():
+    u = T._union([(0, 2), (1, 3), (5, 6), (6, 6)])
+    assert u == [[0, 3], [5, 6]] and T._length(u) == 4
+    assert T._intersect(u, T._union([(2, 5.5)])) == pytest.approx(1.5)
+    assert T._intersect(u, []) == 0.0
+
+
+def test_overlap_figures_of_a_hand_made_timeline():
+    # copy 0 alone on the link (nothing to hide behind), copy 1 fully under sub-chunk 0's kernels
+    tl = [_entry(0, 0.0, 10.0, 11.0, 11.0, 41.0), _entry(1, 12.0, 22.0, 23.0, 41.0, 71.0)]
+    s = T.summarise(tl, wall_ms=72.0)
+    assert s["link_busy_ms"] == pytest.approx(20.0)
+    # kernels in flight: [10,11] + [11,41] + [22,23] + [41,71] -> [10,71]
+    assert s["kernels_in_flight_ms"] == pytest.approx(61.0)
+    assert s["overlap_pct"] == pytest.approx(50.0)
+    assert s["kernel_idle_ms"] == pytest.approx(11.0)
+
+
+def test_report_modules_refuse_to_run_without_cuda():
+    import torch
+    from paper_2101_00941_b200 import sweep
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(SystemExit):
+        sweep.main(["--workload", "1", "--streams", "1"])
+    with pytest.raises(SystemExit):
+        T.main(["--workload", "1"])
