@@ -283,19 +283,23 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         // AA_DEDISP=plain forces the plain kernels, =ws1024 / ws512 / sp1024 / sp512 one variant (A/B timing, tests).
         R.sp_tb = 0;
         R.ws = false;
-        if (!R.in16) {
+        {
             const char *env = std::getenv("AA_DEDISP");
             auto allowed = [&](const char *name) { return !env || !*env || std::strcmp(env, name) == 0; };
+            // 16-bit lanes take floor(65535 / (255 bin 4)) groups between flushes: binned input only while that
+            // is at least 8 (bin <= 8); coarser ranges are a few per cent of the work and keep the plain kernel
+            const bool ws_ok = !R.in16 || 65535 / (255 * R.r.bin * kSpG) >= 8;
             for (int tb : {1024, 512}) {
-                if (R.sp_tb || !allowed(tb == 1024 ? "ws1024" : "ws512")) continue;
-                if (ws_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, 226 * 1024, R.h_ws, R.sp_rows, R.sp_pbytes)) {
+                if (!ws_ok || R.sp_tb || !allowed(tb == 1024 ? "ws1024" : "ws512")) continue;
+                if (ws_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, R.in16 ? 2 : 1, 226 * 1024, R.h_ws, R.sp_rows,
+                                    R.sp_pbytes)) {
                     R.sp_tb = tb;
                     R.ws = true;
                 }
             }
             if (!R.ws) { R.h_ws.clear(); R.h_ws.shrink_to_fit(); }
             for (int tb : {1024, 512}) {
-                if (R.sp_tb || !allowed(tb == 1024 ? "sp1024" : "sp512")) continue;
+                if (R.in16 || R.sp_tb || !allowed(tb == 1024 ? "sp1024" : "sp512")) continue;
                 const size_t limit = tb == 1024 ? 227 * 1024 : 113 * 1024;
                 if (sp_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, R.h_sp, R.sp_rows, R.sp_pbytes) &&
                     dedisp_sp_smem_bytes(R.sp_rows, R.sp_pbytes) + 1024 <= limit)
@@ -317,7 +321,8 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
     p.pitch_b.resize(p.bins.size());
     for (size_t k = 0; k < p.bins.size(); ++k) {
         int max_row = 0;
-        for (auto &R : p.ranges) if (R.bin_slot == (int)k) max_row = std::max(max_row, R.row);
+        for (auto &R : p.ranges)
+            if (R.bin_slot == (int)k) max_row = std::max(max_row, std::max(R.row, R.sp_tb ? R.sp_rows + R.sp_tb : 0));
         p.pitch_b[k] = round_up((p.L + p.halo) / p.bins[k] + max_row + kDedispTB + 64, 128);
     }
     p.cap = d->max_cands_per_subchunk ? d->max_cands_per_subchunk : (1ull << 21);
@@ -334,7 +339,7 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
     }
     for (int s = 0; s < p.n_streams; ++s) {
         take((p.L + p.halo) * (uint64_t)d->nchans);
-        for (size_t k = 0; k < p.bins.size(); ++k) take((uint64_t)d->nchans * p.pitch_b[k] * 2);
+        for (size_t k = 0; k < p.bins.size(); ++k) take(round_up((uint64_t)d->nchans, kSpG) * p.pitch_b[k] * 2);
         take(p.d_rows * p.pitchD * 4);
         take(p.cap * sizeof(aa_candidate));
         take(256);
@@ -361,7 +366,7 @@ void carve(aa_plan &p)
         S.d_raw = take((p.L + p.halo) * (uint64_t)nchans);
         S.d_binned.resize(p.bins.size());
         for (size_t k = 0; k < p.bins.size(); ++k)
-            S.d_binned[k] = reinterpret_cast<uint16_t *>(take((uint64_t)nchans * p.pitch_b[k] * 2));
+            S.d_binned[k] = reinterpret_cast<uint16_t *>(take(round_up((uint64_t)nchans, kSpG) * p.pitch_b[k] * 2));
         S.d_D = reinterpret_cast<uint32_t *>(take(p.d_rows * p.pitchD * 4));
         S.d_cands = reinterpret_cast<aa_candidate *>(take(p.cap * sizeof(aa_candidate)));
         S.d_count = reinterpret_cast<uint32_t *>(take(256));
@@ -527,7 +532,7 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
                 da.sp_rows = Rg.sp_rows;
                 da.sp_pbytes = Rg.sp_pbytes;
                 da.sp_flush = Rg.sp_flush;
-                if (Rg.ws) AA_W(launch_dedisp_ws(da, Rg.sp_tb, st));
+                if (Rg.ws) AA_W(launch_dedisp_ws(da, Rg.sp_tb, Rg.in16, st));
                 else if (Rg.sp_tb) AA_W(launch_dedisp_sp(da, Rg.sp_tb, st));
                 else AA_W(launch_dedisp(da, Rg.in16, Rg.dpw, st));
                 S.dedisp_launches++;
@@ -750,6 +755,10 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
         const uint64_t pad_rows = round_up((uint64_t)d->nchans, kSpG) - (uint64_t)d->nchans;
         if (pad_rows && (e = cudaMemset(p->d_ring + (uint64_t)d->nchans * p->ring_pitch, 0, pad_rows * p->ring_pitch)) != cudaSuccess)
             return fail(AA_ERR_CUDA, e);
+        for (auto &S : p->streams)
+            for (size_t k = 0; pad_rows && k < p->bins.size(); ++k)
+                if ((e = cudaMemset(S.d_binned[k] + (uint64_t)d->nchans * p->pitch_b[k], 0, pad_rows * p->pitch_b[k] * 2)) != cudaSuccess)
+                    return fail(AA_ERR_CUDA, e);
     }
     p->ev_loaded.assign(p->n_sub, nullptr);
     for (auto &ev : p->ev_loaded)

@@ -75,9 +75,10 @@ struct WsRecord {
     uint16_t nbatch;                // warp-sized batches of 31 chunks per pattern row
     uint16_t pad;
     // bits 0-15: i * sp_rows + (m_i & ~7), the 8-byte-aligned load offset of chunk 0 inside the staging
-    // slot; bits 16-20: 8 * (m_i & 3); bit 21: (m_i & 4) != 0
+    // slot; bits 16-20: 8 * (m_i & 3); bit 21: (m_i & 4) != 0.  16-bit input: bits 0-15: i * sp_rows +
+    // 2 * (m_i & ~3) (bytes), bits 16-17: m_i & 3
     uint32_t chdesc[kSpG];
-    uint32_t esh[kSpG][2];          // byte k of the pair: 8 * e_{k,i}
+    uint32_t esh[kSpG][2];          // byte k of the pair: 8 * e_{k,i} (16-bit input: e_{k,i} <= 2)
     uint32_t pofs;                  // byte offset of this stage's pattern rows inside the shared-memory ring
     int32_t dep;                    // the rows may be written once the consumers are done with stage dep (-1: at once)
     uint32_t pad2[2];
@@ -89,9 +90,10 @@ constexpr int kWsSlots = 16;        // stages are ordered through barrier slots 
 constexpr int kWsWindow = 8;        // ... so a stage never starts before stage s - kWsWindow has been consumed
 // smem_budget: dynamic shared memory the kernel may use; on success rows = bytes per staged channel row and
 // ring_bytes = size of the pattern-row ring (DedispArgs::sp_rows / sp_pbytes)
-bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t tb, size_t smem_budget,
-                     std::vector<WsRecord> &out, int32_t &rows, int32_t &ring_bytes);
-cudaError_t launch_dedisp_ws(const DedispArgs &a, int tb, cudaStream_t st);
+// elem_bytes: 1 (uint8 input) or 2 (time-binned uint16 input)
+bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t tb, int32_t elem_bytes,
+                     size_t smem_budget, std::vector<WsRecord> &out, int32_t &rows, int32_t &ring_bytes);
+cudaError_t launch_dedisp_ws(const DedispArgs &a, int tb, bool in16, cudaStream_t st);
 size_t dedisp_ws_fixed_smem_bytes(int rows);            // everything but the ring
 size_t dedisp_ws_smem_bytes(int rows, int ring_bytes);
 cudaError_t dedisp_ws_configure();

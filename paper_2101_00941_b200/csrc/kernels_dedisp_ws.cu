@@ -172,12 +172,73 @@ __device__ __forceinline__ void build_batch(const WsRecord *R, const uint8_t *q,
     }
 }
 
+// The same for 16-bit input (time-binned ranges: samples <= 255 * bin, four-channel sums < 2^16, so the two
+// 16-bit lanes of a word are simply added).  q: this lane's first window byte of channel 0 (16 bytes per
+// chunk); a lane reads 12 samples per channel from the 8-byte boundary at or below its first sample, aligns
+// them to the channel's smallest shift (word select + 16-bit funnel shift) and per pattern shifts by the
+// extra e_{k,i} <= 2 samples with one PRMT (selector 0x3210 + e * 0x2222: 0, 2 or 4 bytes into the word pair).
+template <int NPAT, int K0>
+__device__ __forceinline__ void build_batch16(const WsRecord *R, const uint8_t *q, uint32_t dst, uint32_t st, uint32_t rowbytes)
+{
+    uint32_t acc[NPAT][4];
+#pragma unroll
+    for (int k = 0; k < NPAT; ++k)
+#pragma unroll
+        for (int j = 0; j < 4; ++j) acc[k][j] = 0;
+
+#pragma unroll
+    for (int i = 0; i < G; ++i) {
+        const uint32_t cd = R->chdesc[i];
+        const uint8_t *qi = q + (cd & 0xFFFFu);
+        const uint2 v0 = *reinterpret_cast<const uint2 *>(qi);
+        const uint2 v1 = *reinterpret_cast<const uint2 *>(qi + 8);
+        const uint2 v2 = *reinterpret_cast<const uint2 *>(qi + 16);
+        const uint32_t w6 = *reinterpret_cast<const uint32_t *>(qi + 24);
+        const uint32_t sh = (cd >> 16) & 3u;               // smallest shift modulo 4 samples
+        const bool up = sh >= 2u;                          // start one word later
+        const uint32_t a0 = up ? v0.y : v0.x, a1 = up ? v1.x : v0.y, a2 = up ? v1.y : v1.x, a3 = up ? v2.x : v1.y,
+                       a4 = up ? v2.y : v2.x, a5 = up ? w6 : v2.y;
+        const uint32_t f = (sh & 1u) * 16u;
+        const uint32_t t0 = __funnelshift_r(a0, a1, f), t1 = __funnelshift_r(a1, a2, f), t2 = __funnelshift_r(a2, a3, f),
+                       t3 = __funnelshift_r(a3, a4, f), t4 = __funnelshift_r(a4, a5, f);
+        uint2 es = make_uint2(0, 0);
+        if (i > 0) es = *reinterpret_cast<const uint2 *>(R->esh[i]);
+#pragma unroll
+        for (int k = 0; k < NPAT; ++k) {
+            uint32_t x0 = t0, x1 = t1, x2 = t2, x3 = t3;
+            if (i > 0) {                                   // channel 0 is the reference: no extra shift
+                const int kk = K0 + k;
+                const uint32_t e = ((kk < 4 ? es.x : es.y) >> (8 * (kk & 3))) & 0xFFu;   // extra shift of pattern kk
+                const uint32_t sel = 0x3210u + e * 0x2222u;
+                x0 = __byte_perm(t0, t1, sel);
+                x1 = __byte_perm(t1, t2, sel);
+                x2 = __byte_perm(t2, t3, sel);
+                x3 = __byte_perm(t3, t4, sel);
+            }
+            acc[k][0] += x0;
+            acc[k][1] += x1;
+            acc[k][2] += x2;
+            acc[k][3] += x3;
+        }
+    }
+
+#pragma unroll
+    for (int k = 0; k < NPAT; ++k) {
+        const uint32_t *c = acc[k];
+        const uint32_t nx = __shfl_down_sync(0xFFFFFFFFu, c[0], 1);
+        const uint32_t d = dst + (uint32_t)(2 * (K0 + k)) * rowbytes;
+        sts128_if(d, c[0], c[1], c[2], c[3], st);
+        sts128_if(d + rowbytes, __byte_perm(c[0], c[1], 0x5432), __byte_perm(c[1], c[2], 0x5432),
+                  __byte_perm(c[2], c[3], 0x5432), __byte_perm(c[3], nx, 0x5432), st);
+    }
+}
+
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void *src)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
 }
 
-template <int NPAT_LO, int NPAT_HI>
+template <bool IN16, int NPAT_LO, int NPAT_HI>
 __device__ __forceinline__ void build_stage(const WsRecord *R, const uint8_t *rawslot, uint32_t P, uint32_t nchunk,
                                             uint32_t nbatch, int member, int lane)
 {
@@ -185,17 +246,23 @@ __device__ __forceinline__ void build_stage(const WsRecord *R, const uint8_t *ra
     for (uint32_t b = (uint32_t)member; b < nbatch; b += TEAM) {
         const uint32_t chunk = b * 31u + (uint32_t)lane;
         // chunk nchunk is read for its first sample only; nothing beyond it is read
-        const uint8_t *q = rawslot + 8u * (chunk < nchunk ? chunk : nchunk);
+        const uint8_t *q = rawslot + (IN16 ? 16u : 8u) * (chunk < nchunk ? chunk : nchunk);
         const uint32_t dst = P + 16u * chunk;
         const uint32_t st = lane < 31 && chunk < nchunk;
-        build_batch<NPAT_LO, 0>(R, q, dst, st, rowbytes);
-        if (NPAT_HI > 0) build_batch<(NPAT_HI > 0 ? NPAT_HI : 1), NPAT_LO>(R, q, dst, st, rowbytes);
+        if (IN16) {
+            build_batch16<NPAT_LO, 0>(R, q, dst, st, rowbytes);
+            if (NPAT_HI > 0) build_batch16<(NPAT_HI > 0 ? NPAT_HI : 1), NPAT_LO>(R, q, dst, st, rowbytes);
+        } else {
+            build_batch<NPAT_LO, 0>(R, q, dst, st, rowbytes);
+            if (NPAT_HI > 0) build_batch<(NPAT_HI > 0 ? NPAT_HI : 1), NPAT_LO>(R, q, dst, st, rowbytes);
+        }
     }
 }
 
-template <int TB>
+template <int TB, bool IN16>
 __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
 {
+    constexpr int ES = IN16 ? 2 : 1;       // bytes per input sample
     constexpr int NP = TB / 64;            // 2-sample words per consumer lane
 
     extern __shared__ __align__(128) uint8_t smem[];
@@ -234,7 +301,7 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
         // ================================ producers ================================================
         asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REG_PROD));
         const int pw = warp - NCW, team = pw / TEAM, member = pw % TEAM;
-        const uint8_t *in = static_cast<const uint8_t *>(a.in) + a.col0 + t0;
+        const uint8_t *in = static_cast<const uint8_t *>(a.in) + (a.col0 + t0) * ES;
         const uint32_t myrec = sm_rec + pw * (NRECBUF * REC);
         const uint8_t *myrecp = rec0 + pw * (NRECBUF * REC);
 
@@ -253,7 +320,7 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
             const uint32_t dst = sm_raw + w * raw_bytes;
 #pragma unroll
             for (int i = 0; i < G; ++i)
-                bulk_g2s(dst + i * ROWS, in + (size_t)(q * G + i) * a.pitch_in + R->rbase[i], R->rbytes[i], bar);
+                bulk_g2s(dst + i * ROWS, in + ((size_t)(q * G + i) * a.pitch_in + R->rbase[i]) * ES, R->rbytes[i], bar);
         };
 
         // turn it of this team is stage s = team + it * NTEAM; record copy slot it % 3, window slot 2 * team + (it & 1)
@@ -293,14 +360,14 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
             const uint8_t *rawslot = raw0 + w * raw_bytes;
             const uint32_t P = sm_P + R->pofs;
             switch (npat) {
-                case 1: build_stage<1, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
-                case 2: build_stage<2, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
-                case 3: build_stage<3, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
-                case 4: build_stage<4, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
-                case 5: build_stage<5, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
-                case 6: build_stage<6, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
-                case 7: build_stage<4, 3>(R, rawslot, P, nchunk, nbatch, member, lane); break;
-                default: build_stage<4, 4>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 1: build_stage<IN16, 1, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 2: build_stage<IN16, 2, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 3: build_stage<IN16, 3, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 4: build_stage<IN16, 4, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 5: build_stage<IN16, 5, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 6: build_stage<IN16, 6, 0>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                case 7: build_stage<IN16, 4, 3>(R, rawslot, P, nchunk, nbatch, member, lane); break;
+                default: build_stage<IN16, 4, 4>(R, rawslot, P, nchunk, nbatch, member, lane); break;
             }
             __syncwarp();
             if (lane == 0) mbar_arrive(full + 8 * (s % NSLOT));
@@ -412,11 +479,11 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
     if (since || first) flush(first);
 }
 
-template <int TB>
+template <int TB, bool IN16>
 cudaError_t launch_t(const DedispArgs &a, cudaStream_t st)
 {
     dim3 grid((unsigned)((a.ndms + DB - 1) / DB), (unsigned)((a.ncols + TB - 1) / TB));
-    dedisp_ws_kernel<TB><<<grid, NT, dedisp_ws_smem_bytes(a.sp_rows, a.sp_pbytes), st>>>(a);
+    dedisp_ws_kernel<TB, IN16><<<grid, NT, dedisp_ws_smem_bytes(a.sp_rows, a.sp_pbytes), st>>>(a);
     return cudaGetLastError();
 }
 
@@ -434,15 +501,20 @@ size_t dedisp_ws_smem_bytes(int rows, int ring_bytes)
 
 cudaError_t dedisp_ws_configure()
 {
-    cudaError_t e = cudaFuncSetAttribute(dedisp_ws_kernel<1024>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    cudaError_t e = cudaFuncSetAttribute(dedisp_ws_kernel<1024, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(dedisp_ws_kernel<512>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    e = cudaFuncSetAttribute(dedisp_ws_kernel<512, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(dedisp_ws_kernel<1024, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(dedisp_ws_kernel<512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
 }
 
-cudaError_t launch_dedisp_ws(const DedispArgs &a, int tb, cudaStream_t st)
+cudaError_t launch_dedisp_ws(const DedispArgs &a, int tb, bool in16, cudaStream_t st)
 {
     if (a.ncols <= 0 || a.ndms <= 0) return cudaSuccess;
-    return tb == 1024 ? launch_t<1024>(a, st) : launch_t<512>(a, st);
+    if (in16) return tb == 1024 ? launch_t<1024, true>(a, st) : launch_t<512, true>(a, st);
+    return tb == 1024 ? launch_t<1024, false>(a, st) : launch_t<512, false>(a, st);
 }
 
 }  // namespace aa

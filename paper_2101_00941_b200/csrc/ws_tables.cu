@@ -18,9 +18,11 @@
 
 namespace aa {
 
-bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t tb, size_t smem_budget,
-                     std::vector<WsRecord> &out, int32_t &rows, int32_t &ring_bytes)
+bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t tb, int32_t elem_bytes,
+                     size_t smem_budget, std::vector<WsRecord> &out, int32_t &rows, int32_t &ring_bytes)
 {
+    // 8-bit input: extra shifts e <= 3 (bytes inside a word); 16-bit input: e <= 2 (one PRMT over a word pair)
+    const int max_extra = elem_bytes == 1 ? 3 : 2;
     constexpr int G = kSpG, DB = kSpDB;
     const int nblk = (ndms + DB - 1) / DB, ngrp = (nchans + G - 1) / G;
     out.assign((size_t)nblk * ngrp, WsRecord{});
@@ -71,16 +73,18 @@ bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_
                     mn = std::min(mn, pats[k][i]);
                     mx = std::max(mx, pats[k][i]);
                 }
-                if (mx - mn > 3) return false;           // extra shifts are two bits
+                if (mx - mn > max_extra) return false;
                 R.rbase[i] = (ref0 + mn) & ~(kAlign - 1);
                 const int m = ref0 + mn - R.rbase[i];    // smallest shift inside the staged row, 0..15
                 mins[(size_t)b * ngrp + g][i] = m;
                 for (int k = 0; k < npat; ++k) {
-                    const uint32_t e8 = 8u * (uint32_t)(pats[k][i] - mn);
+                    // 8-bit input: funnel-shift bits; 16-bit input: the shift itself
+                    const uint32_t e8 = (elem_bytes == 1 ? 8u : 1u) * (uint32_t)(pats[k][i] - mn);
                     R.esh[i][k >> 2] |= e8 << (8 * (k & 3));
                 }
                 // a producer lane reads 20 bytes from the 8-byte boundary at or below 8*chunk + m, chunk <= nchunk
-                const int need = 8 * nchunk + (m & ~7) + 20;
+                // (16-bit input: 14 samples from the 4-sample boundary at or below it)
+                const int need = elem_bytes == 1 ? 8 * nchunk + (m & ~7) + 20 : 2 * (8 * nchunk + (m & ~3) + 14);
                 const int rb = (need + 15) / 16 * 16;
                 if (rb > 16368) return false;
                 R.rbytes[i] = (uint16_t)rb;
@@ -102,7 +106,9 @@ bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_
     for (size_t r = 0; r < out.size(); ++r)
         for (int i = 0; i < G; ++i) {
             const uint32_t m = (uint32_t)mins[r][i];
-            out[r].chdesc[i] = ((uint32_t)i * (uint32_t)rows + (m & ~7u)) | (8u * (m & 3u)) << 16 | ((m >> 2) & 1u) << 21;
+            out[r].chdesc[i] = elem_bytes == 1
+                                   ? ((uint32_t)i * (uint32_t)rows + (m & ~7u)) | (8u * (m & 3u)) << 16 | ((m >> 2) & 1u) << 21
+                                   : ((uint32_t)i * (uint32_t)rows + 2u * (m & ~3u)) | (m & 3u) << 16;
         }
     // The pattern rows of successive stages go round a ring in shared memory.  Offsets are fixed here, per DM
     // block; dep = the latest earlier stage whose rows overlap the new ones (the producers wait until the

@@ -125,6 +125,45 @@ def test_every_dedispersion_kernel_bit_exact(B, monkeypatch, variant, code, case
     assert res["only_gpu"] == 0 and res["only_oracle"] == 0
 
 
+@pytest.mark.parametrize("variant,code", [("ws1024", 4), ("ws512", 3)])
+@pytest.mark.parametrize("case", [
+    dict(bins=(2,), nchans=302, ndms=100, nsamp=40000, chunk_len=16384),                 # padded channel group, ragged everything
+    dict(bins=(4,), nchans=1024, ndms=64, nsamp=40000, chunk_len=16384, foff=-0.2),      # 16 flushes of the 16-bit lanes
+    dict(bins=(8,), nchans=512, ndms=130, nsamp=80000, chunk_len=32768, foff=-0.4),      # flush every 8 groups
+    dict(bins=(1, 2, 8), nchans=256, ndms=70, nsamp=60000, chunk_len=16384),             # mixed 8-bit and binned ranges
+])
+def test_binned_input_on_the_shared_pattern_kernel(B, monkeypatch, variant, code, case):
+    """Time-binned (uint16) ranges on the warp-specialised shared-pattern kernel, against the oracle."""
+    monkeypatch.setenv("AA_DEDISP", variant)
+    kw = dict(f_top=1500.0, foff=-0.5, dm_step=0.25, norm_block=2048, widths=(1, 2, 4, 8), thr=5.0)
+    kw.update(case)
+    w = _tiny(**kw)
+    buf, x = _pinned_fill(B, w)
+    with B.Plan(w, taps=list(range(w.ndms_total))) as plan:
+        assert all(plan.dedisp_variant(r) == code for r in range(len(w.ranges)))
+        cands, tap = plan.run(buf)
+    ref, dense, geo = oracle.run(x, w, keep_dense=True)
+    base = 0
+    for r, rg in enumerate(w.ranges):
+        assert np.array_equal(tap[base:base + rg.ndms, :geo["nout"][r]], dense[r]), f"range {r}"
+        base += rg.ndms
+    res = compare_candidates(cands, ref, w.snr_threshold)
+    assert res["only_gpu"] == 0 and res["only_oracle"] == 0
+
+
+def test_saturated_binned_input(B, monkeypatch):
+    for variant, b in (("ws1024", 8), ("ws512", 2), ("plain", 4)):
+        monkeypatch.setenv("AA_DEDISP", variant)
+        w = _tiny(bins=(b,), nchans=1024, ndms=70, nsamp=40000, chunk_len=16384, f_top=1500.0, foff=-0.2, dm_step=0.25,
+                  norm_block=2048)
+        buf = B.pinned_empty(w.nbytes)
+        buf.numpy()[:] = 255                         # every 16-bit lane at its limit before every flush
+        with B.Plan(w, taps=list(range(w.ndms_total))) as plan:
+            cands, tap = plan.run(buf)
+            assert len(cands) == 0
+            assert np.all(tap[:, :plan.nout[0]] == 255 * w.nchans * b)
+
+
 def test_saturated_input_every_kernel(B, monkeypatch):
     for variant in ("ws1024", "ws512", "sp1024", "plain"):
         monkeypatch.setenv("AA_DEDISP", variant)
