@@ -494,10 +494,33 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
         const uint64_t in_len = std::min<uint64_t>(L + halo, nsamp - j * L);
 
         AA_W(cudaEventRecord(S.ev[3], st));
-        for (size_t k = 0; k < p->bins.size(); ++k) {
-            AA_W(launch_bin(p->d_ring, (int64_t)p->ring_pitch, (int64_t)col0, nchans, p->bins[k],
-                            (int64_t)(in_len / p->bins[k]), S.d_binned[k], (int64_t)p->pitch_b[k], st));
-            S.prep_launches++;
+        {
+            // power-of-two bins up to 32 share one pass over the ring; anything else is binned on its own
+            BinMultiArgs ba{};
+            bool any = false;
+            for (size_t k = 0; k < p->bins.size(); ++k) {
+                const int b = p->bins[k];
+                int l = -1;
+                for (int q = 0; q < 5; ++q) if (b == (2 << q)) l = q;
+                if (l >= 0 && col0 % 16 == 0 && p->pitch_b[k] % 16 == 0) {
+                    ba.out[l] = S.d_binned[k];
+                    ba.pitch[l] = (int64_t)p->pitch_b[k];
+                    ba.nbinned[l] = (int64_t)(in_len / b);
+                    any = true;
+                } else {
+                    AA_W(launch_bin(p->d_ring, (int64_t)p->ring_pitch, (int64_t)col0, nchans, b, (int64_t)(in_len / b),
+                                    S.d_binned[k], (int64_t)p->pitch_b[k], st));
+                    S.prep_launches++;
+                }
+            }
+            if (any) {
+                ba.ring = p->d_ring;
+                ba.ring_pitch = (int64_t)p->ring_pitch;
+                ba.col0 = (int64_t)col0;
+                ba.ngroups = (int64_t)((in_len + 31) / 32);
+                AA_W(launch_bin_multi(ba, nchans, st));
+                S.prep_launches++;
+            }
         }
         AA_W(cudaEventRecord(S.ev[4], st));
         AA_W(cudaMemsetAsync(S.d_count, 0, sizeof(uint32_t), st));

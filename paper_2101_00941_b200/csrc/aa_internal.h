@@ -128,6 +128,16 @@ cudaError_t launch_corner_turn(const uint8_t *src, int64_t nt, int32_t nchans, i
                                cudaStream_t st);
 cudaError_t launch_bin(const uint8_t *ring, int64_t ring_pitch, int64_t col0, int32_t nchans,
                        int32_t bin, int64_t nbinned, uint16_t *out, int64_t out_pitch, cudaStream_t st);
+// every power-of-two bin 2, 4, .., 32 the plan uses, in one pass (level l = bin 2^(l+1); out[l] == nullptr: not wanted)
+struct BinMultiArgs {
+    const uint8_t *ring;
+    int64_t ring_pitch, col0;   // col0 and every out pitch: multiples of 16 elements
+    int64_t ngroups;            // groups of 32 input samples to read (the last one may be partial)
+    uint16_t *out[5];
+    int64_t pitch[5];           // elements
+    int64_t nbinned[5];         // valid outputs per row
+};
+cudaError_t launch_bin_multi(const BinMultiArgs &a, int32_t nchans, cudaStream_t st);
 // dpw = DMs per warp (4, 2 or 1); in16 = input is uint16
 cudaError_t launch_dedisp(const DedispArgs &a, bool in16, int dpw, cudaStream_t st);
 size_t dedisp_smem_bytes(bool in16, int dpw, int row);

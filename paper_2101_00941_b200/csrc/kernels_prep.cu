@@ -155,4 +155,74 @@ cudaError_t launch_bin(const uint8_t *ring, int64_t ring_pitch, int64_t col0, in
     return cudaGetLastError();
 }
 
+// All power-of-two bins 2..32 of a sub-chunk in one pass over the ring: a thread takes 32 consecutive samples
+// of one channel (two 16-byte loads) and forms the sums of 2, 4, 8, 16 and 32 by successive pairwise addition
+// (16-bit lanes, SWAR), storing the levels the plan asks for.  The ring is read once instead of once per bin.
+__global__ void __launch_bounds__(256) bin_multi_kernel(const BinMultiArgs a)
+{
+    const int32_t c = blockIdx.y;
+    const uint8_t *row = a.ring + c * a.ring_pitch + a.col0;
+    for (int64_t g = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; g < a.ngroups; g += (int64_t)gridDim.x * blockDim.x) {
+        const uint4 x0 = __ldg(reinterpret_cast<const uint4 *>(row + 32 * g));
+        const uint4 x1 = __ldg(reinterpret_cast<const uint4 *>(row + 32 * g + 16));
+        const uint32_t w[8] = {x0.x, x0.y, x0.z, x0.w, x1.x, x1.y, x1.z, x1.w};
+        uint32_t s2[8], s4[4], s8[2], s16, s32;
+#pragma unroll
+        for (int i = 0; i < 8; ++i) s2[i] = (w[i] & 0x00FF00FFu) + ((w[i] >> 8) & 0x00FF00FFu);     // two sums of 2
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {                                                               // two sums of 4
+            const uint32_t lo = (s2[2 * i] & 0xFFFFu) + (s2[2 * i] >> 16), hi = (s2[2 * i + 1] & 0xFFFFu) + (s2[2 * i + 1] >> 16);
+            s4[i] = lo | hi << 16;
+        }
+#pragma unroll
+        for (int i = 0; i < 2; ++i) {
+            const uint32_t lo = (s4[2 * i] & 0xFFFFu) + (s4[2 * i] >> 16), hi = (s4[2 * i + 1] & 0xFFFFu) + (s4[2 * i + 1] >> 16);
+            s8[i] = lo | hi << 16;
+        }
+        {
+            const uint32_t lo = (s8[0] & 0xFFFFu) + (s8[0] >> 16), hi = (s8[1] & 0xFFFFu) + (s8[1] >> 16);
+            s16 = lo | hi << 16;
+            s32 = lo + hi;
+        }
+        // level l holds 32 >> (l + 1) sums of this group, packed two per word
+        auto put = [&](int l, const uint32_t *v, int n) {
+            uint16_t *o = a.out[l];
+            if (!o) return;
+            o += c * a.pitch[l];
+            const int64_t first = g * n;
+            if (first + n <= a.nbinned[l]) {
+                if (n >= 8) {
+#pragma unroll
+                    for (int i = 0; i < n / 8; ++i)
+                        reinterpret_cast<uint4 *>(o + first)[i] = make_uint4(v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
+                } else if (n == 4) {
+                    *reinterpret_cast<uint2 *>(o + first) = make_uint2(v[0], v[1]);
+                } else if (n == 2) {
+                    *reinterpret_cast<uint32_t *>(o + first) = v[0];
+                } else {
+                    o[first] = (uint16_t)v[0];
+                }
+            } else {
+                for (int i = 0; i < n; ++i)
+                    if (first + i < a.nbinned[l]) o[first + i] = (uint16_t)(v[i >> 1] >> (16 * (i & 1)));
+            }
+        };
+        put(0, s2, 16);
+        put(1, s4, 8);
+        put(2, s8, 4);
+        put(3, &s16, 2);
+        put(4, &s32, 1);
+    }
+}
+
+cudaError_t launch_bin_multi(const BinMultiArgs &a, int32_t nchans, cudaStream_t st)
+{
+    if (a.ngroups <= 0) return cudaSuccess;
+    unsigned gx = (unsigned)((a.ngroups + 255) / 256);
+    if (gx > 16) gx = 16;
+    dim3 grid(gx, (unsigned)nchans);
+    bin_multi_kernel<<<grid, 256, 0, st>>>(a);
+    return cudaGetLastError();
+}
+
 }  // namespace aa
