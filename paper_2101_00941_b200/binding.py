@@ -196,11 +196,15 @@ class Plan:
             _check(self.lib, v)
         return v
 
-    def _run(self, fn, ptr: int, max_cands: int, want_taps: bool):
+    def _run(self, fn, ptr: int, max_cands: int, want_taps: bool, tap_out=None):
         out = np.empty(int(max_cands), dtype=CAND_DTYPE)
         n = ctypes.c_uint64(0)
         tap = None
-        if want_taps and self.taps:
+        if tap_out is not None:                      # caller's buffer (e.g. a 68 GB dense plane, touched once)
+            assert tap_out.dtype == np.uint32 and tap_out.flags.c_contiguous
+            assert tap_out.shape == (len(self.taps), self.info["tap_row_len"])
+            tap = tap_out
+        elif want_taps and self.taps:
             tap = np.zeros((len(self.taps), self.info["tap_row_len"]), dtype=np.uint32)
         rc = fn(self.handle, ptr, out.ctypes.data, int(max_cands), ctypes.byref(n),
                 tap.ctypes.data if tap is not None else None)
@@ -209,10 +213,10 @@ class Plan:
         self.n_found = int(n.value)
         return out[:int(self.stats()["n_stored"])], tap
 
-    def run(self, host_input, max_cands: int = 1 << 22, want_taps: bool = True):
+    def run(self, host_input, max_cands: int = 1 << 22, want_taps: bool = True, tap_out=None):
         """aa_run on a pinned host buffer (torch pinned tensor or its numpy view)."""
         ptr = host_input.data_ptr() if hasattr(host_input, "data_ptr") else host_input.ctypes.data
-        return self._run(self.lib.aa_run, ptr, max_cands, want_taps)
+        return self._run(self.lib.aa_run, ptr, max_cands, want_taps, tap_out)
 
     def run_staged(self, host_input, max_cands: int = 1 << 22, want_taps: bool = True):
         """aa_run_staged on an ordinary (pageable) numpy uint8 array; needs Plan(stage_input=True)."""

@@ -584,12 +584,20 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
                 AA_W(launch_sps(sa, p->wt, Rg.wide, st));
                 S.sps_launches++;
                 AA_W(cudaEventRecord(e2, st));
-                for (auto &tp : Rg.taps) {
-                    AA_W(cudaMemcpyAsync(S.h_tap + tap_off, S.d_D + (uint64_t)tp.first * p->pitchD, nemit * 4,
-                                         cudaMemcpyDeviceToHost, st));
-                    tapcopies.push_back({tp.second, tau0, nemit, tap_off});
-                    tap_off += nemit;
-                    S.d2h_bytes += nemit * 4;
+                // tapped rows: runs of consecutive trials leave in one strided copy (all rows tapped = the dense
+                // DM x time plane of the sub-chunk, the paper's device-to-host path)
+                for (size_t a0 = 0; a0 < Rg.taps.size();) {
+                    size_t a1 = a0 + 1;
+                    while (a1 < Rg.taps.size() && Rg.taps[a1].first == Rg.taps[a1 - 1].first + 1) ++a1;
+                    const uint64_t nrows = a1 - a0;
+                    AA_W(cudaMemcpy2DAsync(S.h_tap + tap_off, nemit * 4, S.d_D + (uint64_t)Rg.taps[a0].first * p->pitchD,
+                                           p->pitchD * 4, nemit * 4, nrows, cudaMemcpyDeviceToHost, st));
+                    for (size_t q = a0; q < a1; ++q) {
+                        tapcopies.push_back({Rg.taps[q].second, tau0, nemit, tap_off});
+                        tap_off += nemit;
+                    }
+                    S.d2h_bytes += nrows * nemit * 4;
+                    a0 = a1;
                 }
             } else {
                 AA_W(cudaEventRecord(e1, st));
