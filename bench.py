@@ -51,20 +51,23 @@ def peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
 
 
-def ncu_traffic(kernel_name):
-    """dram__bytes_read.sum + dram__bytes_write.sum of one launch of the dominant kernel, from the committed
-    `ncu --set full` summary of this round (profiles/r1_dedisp_ws_ncu.txt); None if there is none for it."""
+def ncu_counters(kernel_name):
+    """Per-launch counters of the dominant kernel from the committed `ncu --set full` summary of this round
+    (profiles/r1_dedisp_ws_ncu.txt, same launch shape as the bench): (dram bytes read + written, shared-memory
+    wavefronts); (None, None) if there is no summary for this kernel."""
     path = os.path.join(ROOT, "profiles", "r1_dedisp_ws_ncu.txt")
     if not kernel_name.startswith("dedisp_ws_kernel<1024>") or not os.path.exists(path):
-        return None
-    tot = 0.0
+        return None, None
+    tot, wf = 0.0, None
     scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}
     with open(path) as f:
         for line in f:
             c = [x.strip() for x in line.split("|")]
             if len(c) == 3 and c[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum") and c[1] in scale:
                 tot += float(c[2]) * scale[c[1]]
-    return tot or None
+            if len(c) == 3 and c[0] == "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum":
+                wf = float(c[2])
+    return (tot or None), wf
 
 
 class ClockSampler:
@@ -312,11 +315,18 @@ def main():
     achieved = adds_per_launch / avg_launch_s / 1e12              # T adds/s
     sm_mhz = pk.get("sm_max_mhz", 1965.0)
     peak = 148 * 128 * sm_mhz * 1e6 / 1e12                        # T lane-ops/s
+    traffic, smem_wf = ncu_counters(kernel_name)
     roofline = {"kernel": kernel_name, "bound": "alu", "achieved": achieved, "peak": peak,
-                "unit": "T integer adds/s", "frac": achieved / peak, "traffic": ncu_traffic(kernel_name),
+                "unit": "T integer adds/s", "frac": achieved / peak, "traffic": traffic,
                 "peak_source": f"148 SMs x 128 lanes x {sm_mhz:.0f} MHz ({pk_src}); one add per lane-op",
                 "avg_launch_ms": avg_launch_s * 1e3, "launches": d_n,
                 "share_of_step": {"dedisp": d_ms / wall_ms, "sps": s_ms / wall_ms, "prep": p_ms / wall_ms}}
+    if smem_wf:
+        # the resource that binds this kernel: one 128-byte shared-memory wavefront per clock per SM
+        roofline["shared_memory_pipe"] = {"wavefronts_per_launch": smem_wf, "peak_per_s": 148 * sm_mhz * 1e6,
+                                          "frac": smem_wf / avg_launch_s / (148 * sm_mhz * 1e6),
+                                          "source": "ncu l1tex__data_pipe_lsu_wavefronts_mem_shared.sum (profiles/r1_dedisp_ws_ncu.txt) "
+                                                    "over the launch time measured here"}
 
     if rank == 0:
         value = world * units * args.steps / t_res

@@ -80,7 +80,10 @@ typedef struct {
     void    *device_arena;       /* device */
     uint64_t device_arena_bytes; /* must be >= aa_plan_arena_bytes(desc) */
     void *const *streams;        /* cudaStream_t[n_streams] or NULL */
-    /* dense rows to hand back for parity checks: global dm indices, ascending */
+    /* dense dedispersed rows to hand back: global dm indices, ascending.  A few rows serve parity checks; all of
+     * them give the whole DM x time plane (the paper's device-to-host path): runs of consecutive
+     * trials leave the device in one strided copy into the stream's pinned staging and the stream's host thread
+     * moves them into tap_out.  Staging: sum over ranges of ntap_r * subchunk_len / bin_r * 4 bytes per stream. */
     int32_t  ntap;
     const uint32_t *tap_dm_indices;
     /* capacity of each stream's device candidate list per sub-chunk; 0 -> 1<<21 */
