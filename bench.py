@@ -207,6 +207,9 @@ def main():
     ap.add_argument("--ref-rows", type=int, default=48, help="DM trials of the oracle sample")
     ap.add_argument("--ref-blocks", type=int, default=8, help="normalisation blocks of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--shard-observation", action="store_true",
+                    help="strong scaling: ONE observation split by time over the ranks (whole normalisation blocks + halo "
+                         "per rank, candidate lists gathered on rank 0); default: one observation per rank (weak)")
     ap.add_argument("--nsamp", type=int, default=0,
                     help="shorten the observation (profiling runs under ncu only; not a bench line)")
     args = ap.parse_args()
@@ -228,15 +231,27 @@ def main():
     if args.nsamp:
         w = I.scaled(w, nsamp=args.nsamp, name=w.name + f"_nsamp{args.nsamp}")
         note = "shortened observation for profiling; not a bench line"
-    w = dist_util.rank_workload(w, rank)
     n_streams = args.streams or w.n_streams
     L = w.chunk_len // w.n_streams                     # sub-chunk length of both legs
+    shard = None
+    if args.shard_observation:
+        # one observation, rank r takes a contiguous run of whole normalisation blocks (+ DM sweep + boxcar tail)
+        g = B.plan_geometry(w)
+        shard = dist_util.time_shards(w.nsamp, g["maxshift"], w.norm_block, g["halo"] - g["maxshift"], world)[rank]
+        if shard.nsamp == 0:
+            raise SystemExit(f"rank {rank}: nothing to do ({world} ranks for {w.nsamp} samples)")
+        w_full, w = w, dist_util.shard_workload(w, shard)
+    else:
+        w = dist_util.rank_workload(w, rank)
 
     t_gen0 = time.perf_counter()
     host = B.pinned_empty(w.nbytes)
     t_pin = time.perf_counter() - t_gen0
     x = host.numpy().reshape(w.nsamp, w.nchans)
-    I.fill(w, x)
+    if shard is not None:
+        I.fill_span(w_full, shard.t_first, shard.nsamp, x)
+    else:
+        I.fill(w, x)
     t_gen = time.perf_counter() - t_gen0 - t_pin
 
     def barrier():
@@ -269,11 +284,16 @@ def main():
     plan_stats = plan.stats
     info = plan.info
     units = info["dm_trial_samples"]
+    if shard is not None:
+        # work units this rank owns: the output samples of its blocks (the tail belongs to the next rank)
+        units = dist_util.sum_over_ranks(sum(r.ndms * (shard.keep // r.bin) for r in w.ranges)) // world
     last = {}
 
     def step_e2e():
         c, _ = plan.run(host, max_cands=max_cands, want_taps=False)
-        last["n"] = len(c)
+        if shard is not None:
+            c = dist_util.merge_shards(c, shard)       # gather + sort on rank 0: part of the job
+        last["n"] = len(c) if c is not None else 0
 
     sampler.start()
     t_e2e, st_e2e = timed(step_e2e, args.steps, args.warmup)
@@ -335,8 +355,8 @@ def main():
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * t_res / args.steps, "higher_is_better": True,
-            "scaling": "weak", "vs_baseline": None, "dtype": "u8 input, u32 exact sums, f64 S/N",
-            "data": "synthetic",
+            "scaling": "strong" if shard is not None else "weak", "vs_baseline": None,
+            "dtype": "u8 input, u32 exact sums, f64 S/N", "data": "synthetic",
             "config": {"workload": w.name, "nchans": w.nchans, "nsamp": w.nsamp, "ndms": w.ndms_total,
                        "widths": list(w.widths), "n_streams_e2e": n_streams, "subchunk_len": L,
                        "chunk_len_e2e": L * n_streams, "l2": "inputs (34 GB) >> L2; no flush needed",

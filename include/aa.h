@@ -144,6 +144,10 @@ typedef struct aa_plan aa_plan;
  * Returns 0 if the descriptor is invalid. */
 uint64_t aa_plan_arena_bytes(const aa_plan_desc *d);
 
+/* The geometry a plan built from `d` would have (maxshift, halo, sub-chunks, work units, memory), without
+ * creating it: no CUDA call, usable on a host without a GPU (e.g. to split an observation over ranks). */
+int aa_plan_geometry(const aa_plan_desc *d, aa_plan_info *out);
+
 /* Allocation phase (PAPER.md:19 part 2, :41 steps 1-2, :71): validates the descriptor, builds
  * the delay tables in double (north_star formula), creates streams and events, allocates the
  * device ring, per-stream work buffers, candidate lists and pinned staging.  Nothing is

@@ -22,7 +22,7 @@ CAND_DTYPE = np.dtype([("dm_index", np.uint32), ("t_start", np.uint32),
 
 EXPORTS = ["aa_plan_arena_bytes", "aa_plan_create", "aa_plan_query", "aa_plan_nout", "aa_plan_delays",
            "aa_plan_dedisp_variant",
-           "aa_run", "aa_run_staged", "aa_run_resident", "aa_get_stats", "aa_get_timeline", "aa_destroy", "aa_host_alloc", "aa_host_free",
+           "aa_plan_geometry", "aa_run", "aa_run_staged", "aa_run_resident", "aa_get_stats", "aa_get_timeline", "aa_destroy", "aa_host_alloc", "aa_host_free",
            "aa_strerror", "aa_last_cuda_error"]
 
 
@@ -104,6 +104,8 @@ def load_library() -> ctypes.CDLL:
     lib.aa_get_stats.argtypes = [vp, ctypes.POINTER(StatsC)]
     lib.aa_destroy.restype = None
     lib.aa_destroy.argtypes = [vp]
+    lib.aa_plan_geometry.restype = ctypes.c_int
+    lib.aa_plan_geometry.argtypes = [ctypes.POINTER(PlanDescC), ctypes.POINTER(PlanInfoC)]
     lib.aa_get_timeline.restype = ctypes.c_int
     lib.aa_get_timeline.argtypes = [vp, ctypes.POINTER(SubchunkTimesC), u64, ctypes.POINTER(u64)]
     lib.aa_host_alloc.restype = ctypes.c_int
@@ -131,6 +133,24 @@ def pinned_empty(nbytes: int):
     """Pinned host uint8 tensor (torch owns it)."""
     import torch
     return torch.empty(int(nbytes), dtype=torch.uint8, pin_memory=True)
+
+
+def plan_geometry(w, *, n_streams: Optional[int] = None, chunk_len: Optional[int] = None) -> dict:
+    """aa_plan_geometry: maxshift, halo, sub-chunks, work units and memory of the plan for workload `w`, without
+    creating it (no GPU needed)."""
+    lib = load_library()
+    ranges = (DMRangeC * len(w.ranges))(*[DMRangeC(r.dm_low, r.dm_step, r.ndms, r.bin) for r in w.ranges])
+    widths = (ctypes.c_int32 * len(w.widths))(*w.widths)
+    d = PlanDescC()
+    d.nchans, d.nsamp, d.tsamp, d.f_top, d.foff = w.nchans, w.nsamp, w.tsamp, w.f_top, w.foff
+    d.nranges, d.ranges, d.nwidths, d.widths = len(w.ranges), ranges, len(w.widths), widths
+    d.snr_threshold = float(w.snr_threshold)
+    d.n_streams = int(n_streams if n_streams is not None else w.n_streams)
+    d.chunk_len = int(chunk_len if chunk_len is not None else w.chunk_len)
+    d.norm_block = int(getattr(w, "norm_block", 65536))
+    info = PlanInfoC()
+    _check(lib, lib.aa_plan_geometry(ctypes.byref(d), ctypes.byref(info)))
+    return {n: int(getattr(info, n)) for n, _ in PlanInfoC._fields_}
 
 
 class Plan:

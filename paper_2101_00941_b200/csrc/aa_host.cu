@@ -818,15 +818,32 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
     return AA_OK;
 }
 
+static void fill_info(const aa_plan *p, aa_plan_info *o);
+
+int aa_plan_geometry(const aa_plan_desc *d, aa_plan_info *o)
+{
+    if (!o) return AA_ERR_INVALID;
+    aa_plan tmp;
+    const int rc = build_geometry(tmp, d);
+    if (rc != AA_OK) return rc;
+    fill_info(&tmp, o);
+    return AA_OK;
+}
+
 int aa_plan_query(const aa_plan *p, aa_plan_info *o)
 {
     if (!p || !o) return AA_ERR_INVALID;
+    fill_info(p, o);
+    return AA_OK;
+}
+
+static void fill_info(const aa_plan *p, aa_plan_info *o)
+{
     o->maxshift = p->maxshift; o->t_valid = p->t_valid; o->halo = p->halo; o->subchunk_len = p->L;
     o->n_subchunks = p->n_sub;
     o->ndms_total = 0; o->dm_trial_samples = 0;
     for (auto &R : p->ranges) { o->ndms_total += (uint64_t)R.r.ndms; o->dm_trial_samples += (uint64_t)R.r.ndms * R.nout; }
     o->arena_bytes = p->arena_bytes; o->pinned_bytes = p->pinned_bytes; o->tap_row_len = p->tap_row_len;
-    return AA_OK;
 }
 
 uint64_t aa_plan_nout(const aa_plan *p, int32_t r)

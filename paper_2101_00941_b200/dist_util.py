@@ -1,8 +1,13 @@
-"""Multi-GPU plumbing for bench.py: one process per GPU, independent observations per rank.
+"""Multi-GPU plumbing: one process per GPU, no data-path collective.
 
-The path shards by observation / time span with no exchange step: there is no
-data-path collective.  torch.distributed is used only for the barrier around the timed region and
-the max-over-ranks of the measured time.  Backend-agnostic so the host logic is testable with gloo.
+Two ways to use several GPUs, both without an exchange step on the data path:
+  * independent observations, one per rank (bench.py --gpus N: weak scaling);
+  * ONE observation sharded by time (`time_shards`, `shard_workload`, `merge_shards`): rank r searches a
+    contiguous run of whole normalisation blocks plus the DM-sweep / boxcar halo, keeps the candidates that
+    start inside its blocks and rank 0 gathers and sorts the lists.  Because normalisation blocks live on the
+    absolute sample index (A9) the merged list equals the single-GPU list exactly.
+torch.distributed is used for the barrier around the timed region, the max-over-ranks of the measured time
+and the gather of the candidate lists.  Backend-agnostic so the host logic is testable with gloo.
 """
 from __future__ import annotations
 
@@ -66,6 +71,60 @@ def sum_over_ranks(v: int) -> int:
 def rank_workload(w, rank: int):
     """Rank r searches its own observation: same shape and plan, its own noise seed."""
     return dataclasses.replace(w, noise_seed=w.noise_seed + 1000 * rank) if rank else w
+
+
+@dataclasses.dataclass(frozen=True)
+class TimeShard:
+    rank: int
+    t_first: int      # first raw input sample of the shard
+    nsamp: int        # raw input samples the shard reads (its blocks + DM sweep + boxcar tail); 0 = nothing to do
+    keep: int         # candidates with local t_start < keep belong to this shard
+
+
+def time_shards(nsamp: int, maxshift: int, norm_block: int, tail: int, world: int):
+    """Split the valid output span [0, nsamp - maxshift) into `world` contiguous runs of whole normalisation
+    blocks.  `tail` = (wmax - 1) * bin_max rounded up to a multiple of every bin: the samples past a shard's
+    last block that its boxcars may touch (the halo of DESIGN.md section 5 is maxshift + tail)."""
+    t_valid = nsamp - maxshift
+    if t_valid <= 0:
+        raise ValueError("observation shorter than the DM sweep")
+    nblocks = -(-t_valid // norm_block)
+    per = -(-nblocks // world)
+    out = []
+    for r in range(world):
+        b0 = min(r * per, nblocks)
+        b1 = min(b0 + per, nblocks)
+        if b0 == b1:
+            out.append(TimeShard(r, 0, 0, 0))
+            continue
+        t_first = b0 * norm_block
+        keep = min(b1 * norm_block, t_valid) - t_first
+        n_in = nsamp - t_first if b1 == nblocks else min(keep + maxshift + tail, nsamp - t_first)
+        out.append(TimeShard(r, t_first, n_in, keep))
+    return out
+
+
+def shard_workload(w, shard: TimeShard):
+    """The plan of one shard: same band, DM plan and widths on `shard.nsamp` samples (pulses are data, not plan)."""
+    return dataclasses.replace(w, nsamp=shard.nsamp, pulses=(), name=f"{w.name}_shard{shard.rank}")
+
+
+def merge_shards(cands, shard: TimeShard):
+    """Keep this shard's own candidates, move them to absolute time, gather on rank 0 and sort by
+    (dm_index, t_start).  Returns the merged structured array on rank 0 (every rank if not distributed),
+    None elsewhere."""
+    import numpy as np
+    mine = cands[cands["t_start"] < shard.keep].copy()
+    mine["t_start"] += np.uint32(shard.t_first)
+    import torch.distributed as dist
+    if dist.is_available() and dist.is_initialized():
+        rank, world = dist.get_rank(), dist.get_world_size()
+        parts = [None] * world if rank == 0 else None
+        dist.gather_object(mine, parts, dst=0)
+        if rank != 0:
+            return None
+        mine = np.concatenate(parts)
+    return mine[np.lexsort((mine["t_start"], mine["dm_index"]))]
 
 
 def shutdown() -> None:

@@ -262,9 +262,29 @@ def fill(w: Workload, out: Optional[np.ndarray] = None) -> np.ndarray:
     return out
 
 
-def _inject(lib, w: Workload, out: np.ndarray) -> None:
+def fill_span(w: Workload, t_first: int, n: int, out: Optional[np.ndarray] = None) -> np.ndarray:
+    """Rows [t_first, t_first + n) of workload `w`'s filterbank (what `fill(w)[t_first:t_first+n]` holds) without
+    generating the rest: the generator is counter-based, so a rank of a time-sharded run makes only its span."""
+    lib = _load()
+    assert 0 <= t_first and t_first + n <= w.nsamp
+    if out is None:
+        out = np.empty((n, w.nchans), dtype=np.uint8)
+    assert out.dtype == np.uint8 and out.shape == (n, w.nchans) and out.flags.c_contiguous
+    cdf = quantile_table(NOISE_MEAN)
+    lut = _lut16(cdf)
+    lib.aain_fill_noise(out.ctypes.data, t_first * w.nchans, n * w.nchans, w.noise_seed, cdf.ctypes.data, lut.ctypes.data)
+    _inject(lib, w, out, t_first, n)
+    return out
+
+
+def _inject(lib, w: Workload, out: np.ndarray, t_first: int = 0, n: Optional[int] = None) -> None:
+    """Pulse samples of rows [t_first, t_first + n) (default: the whole observation) re-drawn in `out`."""
     if not w.pulses:
         return
+    if n is None:
+        n = w.nsamp
+    # aain_patch indexes rows by absolute time: hand it the address row 0 would have
+    base = out.ctypes.data - t_first * w.nchans
     offs = [pulse_offsets(w, p.dm) for p in w.pulses]
     tables = {}
     for c in range(w.nchans):
@@ -278,8 +298,10 @@ def _inject(lib, w: Workload, out: np.ndarray) -> None:
             tab = tables.get(amp)
             if tab is None:
                 tab = tables[amp] = quantile_table(NOISE_MEAN + NOISE_SIGMA * amp)
-            lib.aain_patch(out.ctypes.data, w.nchans, w.nsamp, c, a, b - a, w.noise_seed,
-                           tab.ctypes.data)
+            a, b = max(a, t_first), min(b, t_first + n)
+            if a >= b:
+                continue
+            lib.aain_patch(base, w.nchans, t_first + n, c, a, b - a, w.noise_seed, tab.ctypes.data)
 
 
 def sample(w: Workload, t: int, c: int) -> int:

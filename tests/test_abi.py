@@ -64,3 +64,17 @@ def test_product_path_fails_loudly_without_cuda():
         pytest.skip("a GPU is present")
     with pytest.raises(RuntimeError):
         B.Plan(I.workload(1))
+
+
+def test_plan_geometry_without_a_gpu_matches_the_oracle():
+    """aa_plan_geometry is pure host code: maxshift / valid span / work units equal the oracle's on every workload."""
+    import oracle
+    from paper_2101_00941_b200 import binding as B
+    from paper_2101_00941_b200 import inputs as I
+    for k in (1, 2, 3, 4, 5):
+        w = I.workload(k)
+        g = B.plan_geometry(w)
+        geo = oracle.geometry(w)
+        assert g["maxshift"] == geo["maxshift"] and g["t_valid"] == geo["t_valid"]
+        assert g["dm_trial_samples"] == sum(r.ndms * n for r, n in zip(w.ranges, geo["nout"]))
+        assert g["subchunk_len"] == w.chunk_len // w.n_streams and g["halo"] >= g["maxshift"]

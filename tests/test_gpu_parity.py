@@ -216,6 +216,32 @@ def test_pageable_input_through_pinned_staging(B):
     assert np.array_equal(got_tap, want_tap)
 
 
+def test_time_sharded_observation_equals_the_whole(B):
+    """one observation split by time over several GPUs (here: the shards one after the other on one
+    GPU, through the same dist_util code the ranks use) gives the single-run candidate list, bit for bit."""
+    from paper_2101_00941_b200 import dist_util
+    w = _tiny(nchans=64, nsamp=90000, ndms=48, norm_block=2048, chunk_len=8192, n_streams=2, bins=(1, 2))
+    buf, x = _pinned_fill(B, w)
+    with B.Plan(w) as plan:
+        whole, _ = plan.run(buf, want_taps=False)
+        info = plan.info
+    tail = info["halo"] - info["maxshift"]
+    for world in (2, 3, 5):
+        parts = []
+        for shard in dist_util.time_shards(w.nsamp, info["maxshift"], w.norm_block, tail, world):
+            if shard.nsamp == 0:
+                continue
+            ws = dist_util.shard_workload(w, shard)
+            sbuf = B.pinned_empty(ws.nbytes)
+            I.fill_span(w, shard.t_first, shard.nsamp, sbuf.numpy().reshape(shard.nsamp, w.nchans))
+            with B.Plan(ws) as plan:
+                c, _ = plan.run(sbuf, want_taps=False)
+            parts.append(dist_util.merge_shards(c, shard))
+        merged = np.concatenate(parts)
+        merged = merged[np.lexsort((merged["t_start"], merged["dm_index"]))]
+        assert merged.tobytes() == whole.tobytes() and len(whole) > 0, world
+
+
 def test_saturated_input_and_constant_input(B):
     w = _tiny(nchans=300, nsamp=9000, foff=-0.3, dm_step=4.0, chunk_len=4096, norm_block=2048)
     buf = B.pinned_empty(w.nbytes)

@@ -51,3 +51,12 @@ def test_workload_table_matches_baseline_configs():
     assert w5.nsamp == 1 << 24 and len(w5.pulses) == 64 and w5.nbytes == 68719476736
     assert I.workload(2).widths == (1, 2, 4, 8, 16, 32, 64, 128)
     assert I.workload(1).widths == (1, 2, 4, 8, 16, 32)
+
+
+def test_fill_span_equals_the_slice_of_the_whole():
+    """A rank of a time-sharded run generates only its own rows (counter-based generator + clipped pulses)."""
+    w = I.scaled(I.workload(1), nsamp=9000,
+                 pulses=(I.Pulse(dm=50.0, t0=2990, width=8, amp=3.0), I.Pulse(dm=120.0, t0=5990, width=32, amp=2.0)))
+    x = I.fill(w)
+    for t_first, n in [(0, 9000), (3000, 3000), (2995, 10), (6000, 3000), (8999, 1)]:
+        assert np.array_equal(I.fill_span(w, t_first, n), x[t_first:t_first + n]), (t_first, n)

@@ -51,3 +51,71 @@ def test_single_process_helpers_are_noops():
     assert dist_util.max_over_ranks(3.5) == 3.5 and dist_util.sum_over_ranks(7) == 7
     w = I.workload(1)
     assert dist_util.rank_workload(w, 0) is w and dist_util.rank_workload(w, 3).noise_seed == w.noise_seed + 3000
+
+
+# ---- one observation sharded by time over the ranks -----------------------------------------
+def _shard_setup():
+    import math
+    from paper_2101_00941_b200 import inputs as I
+    import oracle
+    w = I.scaled(I.workload(1), nsamp=30000, name="shardme",
+                 pulses=(I.Pulse(dm=50.0, t0=7000, width=8, amp=3.0), I.Pulse(dm=90.0, t0=16380, width=16, amp=2.5),
+                         I.Pulse(dm=20.0, t0=24500, width=4, amp=4.0)))
+    w = I.scaled(w, norm_block=2048)
+    x = I.fill(w)
+    geo = oracle.geometry(w)
+    bmax = max(r.bin for r in w.ranges)
+    lcm = math.lcm(*[r.bin for r in w.ranges])
+    tail = -(-(max(w.widths) - 1) * bmax // lcm) * lcm
+    return w, x, geo, tail
+
+
+def test_time_shards_partition_the_valid_span():
+    from paper_2101_00941_b200 import dist_util
+    for nsamp, maxshift, nb, tail, world in [(30000, 159, 2048, 31, 3), (1 << 20, 29664, 65536, 255, 8), (5000, 100, 4096, 31, 4)]:
+        sh = dist_util.time_shards(nsamp, maxshift, nb, tail, world)
+        assert len(sh) == world
+        pos = 0
+        for s in sh:
+            if s.nsamp == 0:
+                assert s.keep == 0
+                continue
+            assert s.t_first == pos and s.t_first % nb == 0 and s.t_first + s.nsamp <= nsamp
+            assert s.nsamp >= s.keep + maxshift                      # every kept output sample has its DM sweep
+            pos += s.keep
+        assert pos == nsamp - maxshift                               # the kept spans tile [0, t_valid)
+
+
+def _shard_worker(rank, world, port, q):
+    os.environ.update(RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank),
+                      MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
+    from paper_2101_00941_b200 import dist_util
+    import oracle
+    assert dist_util.init("gloo")
+    w, x, geo, tail = _shard_setup()
+    shard = dist_util.time_shards(w.nsamp, geo["maxshift"], w.norm_block, tail, world)[rank]
+    ws = dist_util.shard_workload(w, shard)
+    # each rank searches only its own span -- here through the oracle (CPU box); on GPUs through aa_run
+    cands, _ = oracle.run(np.ascontiguousarray(x[shard.t_first:shard.t_first + shard.nsamp]), ws)
+    merged = dist_util.merge_shards(cands, shard)
+    q.put((rank, None if merged is None else merged.tobytes()))
+    dist_util.shutdown()
+
+
+def test_time_sharded_observation_equals_the_whole_gloo():
+    import oracle
+    w, x, geo, tail = _shard_setup()
+    whole, _ = oracle.run(x, w)
+    assert len(whole) > 100
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    ps = [ctx.Process(target=_shard_worker, args=(r, 2, port, q)) for r in range(2)]
+    for p in ps:
+        p.start()
+    out = dict(q.get(timeout=180) for _ in ps)
+    for p in ps:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    assert out[1] is None
+    assert out[0] == whole.tobytes()          # bit-identical candidate list, S/N included
