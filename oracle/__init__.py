@@ -172,6 +172,30 @@ def pack_candidates(dm_index: int, bin_: int, tau, ww, sn) -> np.ndarray:
     return out
 
 
+def find_peaks(cands: np.ndarray) -> np.ndarray:
+    """Peak finding on a candidate list (reading A17; SURVEY 8(f) item 1 -- the paper only cites the
+    step, so this is the build's definition written out, brute force over all pairs).
+
+    Two candidates are NEIGHBOURS if their DM indices differ by at most 1 and their boxcars overlap or touch in
+    raw samples: t' <= t + w and t <= t' + w'.  A candidate is a PEAK iff no neighbour beats it, where c' beats c
+    iff snr' > snr, or snr' == snr and (dm_index', t_start') < (dm_index, t_start).  Returns the peaks in input
+    order.  O(n^2): for tests on small lists only.
+    """
+    n = len(cands)
+    d = cands["dm_index"].astype(np.int64)
+    t = cands["t_start"].astype(np.int64)
+    w = cands["width"].astype(np.int64)
+    s = cands["snr"]
+    keep = np.ones(n, dtype=bool)
+    for i in range(n):
+        nb = (np.abs(d - d[i]) <= 1) & (t <= t[i] + w[i]) & (t[i] <= t + w)
+        nb[i] = False
+        beats = (s > s[i]) | ((s == s[i]) & ((d < d[i]) | ((d == d[i]) & (t < t[i]))))
+        if np.any(nb & beats):
+            keep[i] = False
+    return cands[keep]
+
+
 def run(x: np.ndarray, w, *, keep_dense: bool = False, row_subset: Optional[Dict[int, Sequence[int]]] = None,
         threads: Optional[int] = None):
     """Whole observation at once: candidates sorted by (dm_index, t_start) [+ dense D per range].

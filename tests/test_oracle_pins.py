@@ -325,3 +325,52 @@ def test_binned_range_units_are_raw_samples():
     hit = c[(c["dm_index"] == 3 + 1)]
     top = hit[np.argmax(hit["snr"])]
     assert top["t_start"] == t0 and top["width"] == 8 and top["t_start"] % 4 == 0
+
+
+# ---- peak finding (reading A17) ----------------------------------------------------------------------------
+def _cl(rows):
+    a = np.zeros(len(rows), dtype=oracle.CAND_DTYPE)
+    for i, r in enumerate(rows):
+        a[i] = r
+    return a
+
+
+def test_peaks_hand_made_cases():
+    # an isolated candidate is a peak; a clump keeps its maximum only
+    c = _cl([(5, 100, 4, 7.0), (5, 102, 4, 9.0), (6, 101, 8, 8.0), (5, 300, 1, 6.5)])
+    assert [tuple(x) for x in oracle.find_peaks(c)] == [(5, 102, 4, 9.0), (5, 300, 1, 6.5)]
+    # touching boxcars (t' == t + w) are neighbours, a gap of one sample is not
+    c = _cl([(0, 10, 5, 8.0), (0, 15, 2, 7.0), (0, 18, 2, 6.0)])
+    assert [int(x["t_start"]) for x in oracle.find_peaks(c)] == [10, 18]
+    # DM distance 2 is not a neighbour, distance 1 is
+    c = _cl([(3, 50, 4, 9.0), (5, 50, 4, 8.0), (4, 50, 4, 7.0)])
+    assert [int(x["dm_index"]) for x in oracle.find_peaks(c)] == [3, 5]
+    # equal S/N: the smaller (dm_index, t_start) wins, so exactly one of a tie survives
+    c = _cl([(7, 20, 4, 8.0), (7, 22, 4, 8.0), (6, 23, 4, 8.0)])
+    assert [tuple(x)[:2] for x in oracle.find_peaks(c)] == [(6, 23)]
+    # the rule is a local maximum, not a transitive clustering: a chain 9 > 8 > 7 with the ends apart keeps 9 and 7's
+    # other-side survivor only if nothing beats it
+    c = _cl([(1, 0, 4, 9.0), (1, 4, 4, 8.0), (1, 8, 4, 7.0), (1, 100, 4, 6.1)])
+    assert [int(x["t_start"]) for x in oracle.find_peaks(c)] == [0, 100]
+    assert len(oracle.find_peaks(_cl([]))) == 0
+
+
+def test_peaks_invariants_on_a_real_candidate_list():
+    """peaks are a subset; no two peaks are neighbours; every dropped candidate has a neighbour that beats it;
+    the injected cfg1 pulse gives one peak at exactly (DM 50, t 20000, w 8)."""
+    w = I.scaled(I.workload(1), nsamp=1 << 16, norm_block=1 << 14, pulses=(I.Pulse(dm=50.0, t0=20000, width=8, amp=3.0),))
+    x = I.fill(w)
+    cands, _ = oracle.run(x, w)
+    assert len(cands) > 1000
+    peaks = oracle.find_peaks(cands)
+    assert 0 < len(peaks) < len(cands) // 20
+    key = lambda a: set(zip(a["dm_index"].tolist(), a["t_start"].tolist()))
+    assert key(peaks) <= key(cands)
+    d, t, ww, s = (peaks[k].astype(np.float64) for k in ("dm_index", "t_start", "width", "snr"))
+    for i in range(len(peaks)):
+        nb = (np.abs(d - d[i]) <= 1) & (t <= t[i] + ww[i]) & (t[i] <= t + ww)
+        assert nb.sum() == 1                                   # only itself
+    top = peaks[np.argmax(peaks["snr"])]
+    assert (int(top["dm_index"]), int(top["t_start"]), int(top["width"])) == (50, 20000, 8)
+    near = peaks[(np.abs(peaks["dm_index"].astype(int) - 50) <= 1) & (np.abs(peaks["t_start"].astype(int) - 20000) <= 8)]
+    assert len(near) == 1
