@@ -294,12 +294,20 @@ def main():
         if shard is not None:
             c = dist_util.merge_shards(c, shard)       # gather + sort on rank 0: part of the job
         last["n"] = len(c) if c is not None else 0
+        last["c"] = c
 
     sampler.start()
     t_e2e, st_e2e = timed(step_e2e, args.steps, args.warmup)
     h2d = st_e2e[-1]["h2d_bytes"]; d2h = st_e2e[-1]["d2h_bytes"]
     launches_e2e = sum(s["dedisp_launches"] + s["sps_launches"] + s["prep_launches"] for s in st_e2e)
     n_cands = last["n"]
+    # optional host post-step (outside the timed region): peak finding on the returned list (A17)
+    peaks = None
+    if last.get("c") is not None:
+        tp0 = time.perf_counter()
+        n_peaks = len(B.find_peaks(last["c"]))
+        peaks = {"n": n_peaks, "ms": 1e3 * (time.perf_counter() - tp0), "where": "host threads, after aa_run, not in the timed region"}
+    last.pop("c", None)
     plan.close()
 
     # ---- leg 2: observation resident in HBM, one stream (kernel-only; per-launch event times) --
@@ -368,7 +376,7 @@ def main():
                     "transfer_alone_s": t_copy, "kernels_alone_s": t_res / args.steps,
                     "overlap_efficiency": max(t_copy, t_res / args.steps) / step_s},
             "gpu_launches": int(launches_e2e),
-            "candidates": n_cands, "clocks": clocks, "roofline": roofline,
+            "candidates": n_cands, "peaks": peaks, "clocks": clocks, "roofline": roofline,
             "setup": {"pin_s": t_pin, "generate_s": t_gen},
         }
         if not args.no_cpu_baseline:

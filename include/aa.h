@@ -207,6 +207,18 @@ int aa_get_stats(const aa_plan *p, aa_stats *out);
  * the number of sub-chunks to *n. */
 int aa_get_timeline(const aa_plan *p, aa_subchunk_times *out, uint64_t max, uint64_t *n);
 
+/* Optional post-step on the host (the paper only cites the step): peak finding.
+ * Two candidates are neighbours if their dm_index differ by at most 1 and their boxcars overlap or touch in raw
+ * samples (t' <= t + w and t <= t' + w'); a candidate is a peak iff no neighbour has a larger snr (the stored
+ * float), ties going to the smaller (dm_index, t_start).
+ *   cands    : host, n records sorted by (dm_index, t_start) as aa_run returns them (AA_ERR_INVALID otherwise)
+ *   out      : host, room for max_out records; receives the peaks in the same order (may alias nothing in cands)
+ *   n_out    : host, number of peaks found; AA_ERR_OVERFLOW if it exceeds max_out (the first max_out are stored)
+ *   nthreads : host threads to use (rows of DM trials are spread over them); < 1 -> all hardware threads
+ * Pure host code: needs no plan and no GPU. */
+int aa_find_peaks(const aa_candidate *cands, uint64_t n, aa_candidate *out, uint64_t max_out, uint64_t *n_out,
+                  int32_t nthreads);
+
 /* NULL-safe.  Frees everything the plan allocated (not a caller-owned arena or streams). */
 void aa_destroy(aa_plan *p);
 

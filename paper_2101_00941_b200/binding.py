@@ -22,7 +22,7 @@ CAND_DTYPE = np.dtype([("dm_index", np.uint32), ("t_start", np.uint32),
 
 EXPORTS = ["aa_plan_arena_bytes", "aa_plan_create", "aa_plan_query", "aa_plan_nout", "aa_plan_delays",
            "aa_plan_dedisp_variant",
-           "aa_plan_geometry", "aa_run", "aa_run_staged", "aa_run_resident", "aa_get_stats", "aa_get_timeline", "aa_destroy", "aa_host_alloc", "aa_host_free",
+           "aa_plan_geometry", "aa_run", "aa_run_staged", "aa_run_resident", "aa_get_stats", "aa_get_timeline", "aa_find_peaks", "aa_destroy", "aa_host_alloc", "aa_host_free",
            "aa_strerror", "aa_last_cuda_error"]
 
 
@@ -106,6 +106,8 @@ def load_library() -> ctypes.CDLL:
     lib.aa_destroy.argtypes = [vp]
     lib.aa_plan_geometry.restype = ctypes.c_int
     lib.aa_plan_geometry.argtypes = [ctypes.POINTER(PlanDescC), ctypes.POINTER(PlanInfoC)]
+    lib.aa_find_peaks.restype = ctypes.c_int
+    lib.aa_find_peaks.argtypes = [vp, u64, vp, u64, ctypes.POINTER(u64), ctypes.c_int32]
     lib.aa_get_timeline.restype = ctypes.c_int
     lib.aa_get_timeline.argtypes = [vp, ctypes.POINTER(SubchunkTimesC), u64, ctypes.POINTER(u64)]
     lib.aa_host_alloc.restype = ctypes.c_int
@@ -133,6 +135,16 @@ def pinned_empty(nbytes: int):
     """Pinned host uint8 tensor (torch owns it)."""
     import torch
     return torch.empty(int(nbytes), dtype=torch.uint8, pin_memory=True)
+
+
+def find_peaks(cands: np.ndarray, nthreads: int = 0) -> np.ndarray:
+    """aa_find_peaks on a candidate array sorted by (dm_index, t_start) (what Plan.run returns)."""
+    lib = load_library()
+    cands = np.ascontiguousarray(cands, dtype=CAND_DTYPE)
+    out = np.empty(len(cands), dtype=CAND_DTYPE)
+    n = ctypes.c_uint64(0)
+    _check(lib, lib.aa_find_peaks(cands.ctypes.data, len(cands), out.ctypes.data, len(out), ctypes.byref(n), int(nthreads)))
+    return out[:int(n.value)]
 
 
 def plan_geometry(w, *, n_streams: Optional[int] = None, chunk_len: Optional[int] = None) -> dict:
