@@ -634,9 +634,29 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
             const uint64_t m = std::min<uint64_t>(n, max_cands - pos);
             if (m) std::memcpy(out + pos, S.h_cands, m * sizeof(aa_candidate));
         }
-        if (tap_out)
-            for (auto &tc : tapcopies)
-                std::memcpy(tap_out + (uint64_t)tc.row * p->tap_row_len + tc.tau0, S.h_tap + tc.off, tc.n * 4);
+        if (tap_out && !tapcopies.empty()) {
+            // host-to-host copy of the tapped rows; a dense plane is hundreds of MB per sub-chunk,
+            // so the stream's thread takes helpers when the machine has cores to spare
+            auto copy_rows = [&](size_t a, size_t b) {
+                for (size_t i = a; i < b; ++i) {
+                    const TapCopy &tc = tapcopies[i];
+                    std::memcpy(tap_out + (uint64_t)tc.row * p->tap_row_len + tc.tau0, S.h_tap + tc.off, tc.n * 4);
+                }
+            };
+            const uint64_t bytes = tap_off * 4;
+            const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
+            const size_t K = bytes < (64ull << 20) ? 1 : std::min<size_t>(std::max<size_t>(hw / (unsigned)p->n_streams, 1), 4);
+            if (K == 1) {
+                copy_rows(0, tapcopies.size());
+            } else {
+                std::vector<std::thread> helpers;
+                const size_t per = (tapcopies.size() + K - 1) / K;
+                for (size_t k = 1; k < K; ++k)
+                    helpers.emplace_back(copy_rows, std::min(k * per, tapcopies.size()), std::min((k + 1) * per, tapcopies.size()));
+                copy_rows(0, std::min(per, tapcopies.size()));
+                for (auto &h : helpers) h.join();
+            }
+        }
 
         float ms = 0;
         if (!resident && nt) { cudaEventElapsedTime(&ms, S.ev[0], S.ev[1]); S.h2d_ms += ms; }
