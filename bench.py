@@ -302,11 +302,11 @@ def main():
     launches_e2e = sum(s["dedisp_launches"] + s["sps_launches"] + s["prep_launches"] for s in st_e2e)
     n_cands = last["n"]
     # optional host post-step (outside the timed region): peak finding on the returned list (A17)
-    peaks = None
+    peak_info = None
     if last.get("c") is not None:
         tp0 = time.perf_counter()
         n_peaks = len(B.find_peaks(last["c"]))
-        peaks = {"n": n_peaks, "ms": 1e3 * (time.perf_counter() - tp0), "where": "host threads, after aa_run, not in the timed region"}
+        peak_info = {"n": n_peaks, "ms": 1e3 * (time.perf_counter() - tp0), "where": "host threads, after aa_run, not in the timed region"}
     last.pop("c", None)
     plan.close()
 
@@ -376,7 +376,7 @@ def main():
                     "transfer_alone_s": t_copy, "kernels_alone_s": t_res / args.steps,
                     "overlap_efficiency": max(t_copy, t_res / args.steps) / step_s},
             "gpu_launches": int(launches_e2e),
-            "candidates": n_cands, "peaks": peaks, "clocks": clocks, "roofline": roofline,
+            "candidates": n_cands, "peaks": peak_info, "clocks": clocks, "roofline": roofline,
             "setup": {"pin_s": t_pin, "generate_s": t_gen},
         }
         if not args.no_cpu_baseline:
