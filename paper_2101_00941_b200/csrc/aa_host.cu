@@ -286,10 +286,17 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         {
             const char *env = std::getenv("AA_DEDISP");
             auto allowed = [&](const char *name) { return !env || !*env || std::strcmp(env, name) == 0; };
-            // 16-bit lanes take floor(65535 / (255 bin 4)) groups between flushes: binned input only while that
-            // is at least 8 (bin <= 8); coarser ranges are a few per cent of the work and keep the plain kernel
+            // 16-bit lanes take floor(65535 / (255 bin 4)) groups between flushes: binned input only while that is at
+            // least 8 (bin <= 8).  Measured on cfg4: with flushes every 4 / 2 groups (bins 16 / 32) the L2
+            // read-modify-write of the tile costs more than the plain kernel does (2.58 -> 2.78 s per step).
             const bool ws_ok = !R.in16 || 65535 / (255 * R.r.bin * kSpG) >= 8;
-            for (int tb : {1024, 512}) {
+            // time tile: 1024 samples unless the range is so short per sub-chunk that 512-sample tiles (about 0.65 of
+            // the time per CTA) need fewer waves of CTAs over the 148 SMs
+            const uint64_t cols = p.L / (uint64_t)R.r.bin + (uint64_t)p.wmax - 1, nblk = ((uint64_t)R.r.ndms + kSpDB - 1) / kSpDB;
+            const double cost1024 = (double)(((cols + 1023) / 1024 * nblk + 147) / 148);
+            const double cost512 = 0.65 * (double)(((cols + 511) / 512 * nblk + 147) / 148);
+            const int order[2] = {cost512 < cost1024 ? 512 : 1024, cost512 < cost1024 ? 1024 : 512};
+            for (int tb : order) {
                 if (!ws_ok || R.sp_tb || !allowed(tb == 1024 ? "ws1024" : "ws512")) continue;
                 if (ws_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, R.in16 ? 2 : 1, 226 * 1024, R.h_ws, R.sp_rows,
                                     R.sp_pbytes)) {

@@ -152,7 +152,7 @@ def test_binned_input_on_the_shared_pattern_kernel(B, monkeypatch, variant, code
 
 
 def test_saturated_binned_input(B, monkeypatch):
-    for variant, b in (("ws1024", 8), ("ws512", 2), ("plain", 4)):
+    for variant, b in (("ws1024", 8), ("ws512", 2), ("plain", 4), ("plain", 32)):
         monkeypatch.setenv("AA_DEDISP", variant)
         w = _tiny(bins=(b,), nchans=1024, ndms=70, nsamp=40000, chunk_len=16384, f_top=1500.0, foff=-0.2, dm_step=0.25,
                   norm_block=2048)
