@@ -165,7 +165,8 @@ int aa_plan_delays(const aa_plan *p, int32_t r, int32_t *out);
 
 /* Which dedispersion kernel the plan chose for range r (the choice depends only on the delay table):
  * 0 = plain tiled kernel, 1 / 2 = shared-pattern kernel with 512 / 1024-sample tiles, 3 / 4 =
- * warp-specialised shared-pattern kernel with 512 / 1024-sample tiles; AA_ERR_INVALID if r is out
+ * warp-specialised shared-pattern kernel with 512 / 1024-sample tiles, 5 = the same with 32-bit accumulators
+ * (coarse time bins); AA_ERR_INVALID if r is out
  * of range.  Used by tests to make sure every kernel is covered. */
 int aa_plan_dedisp_variant(const aa_plan *p, int32_t r);
 

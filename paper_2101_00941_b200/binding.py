@@ -222,7 +222,8 @@ class Plan:
         return out
 
     def dedisp_variant(self, r: int) -> int:
-        """0 plain, 1/2 shared-pattern 512/1024, 3/4 warp-specialised shared-pattern 512/1024."""
+        """0 plain, 1/2 shared-pattern 512/1024, 3/4 warp-specialised shared-pattern 512/1024, 5 the latter with
+        32-bit accumulators (coarse time bins)."""
         v = self.lib.aa_plan_dedisp_variant(self.handle, r)
         if v < 0:
             _check(self.lib, v)

@@ -47,6 +47,7 @@ struct Range {
     int bin_slot = -1;          // index into the per-stream binned buffers
     int sp_tb = 0;              // shared-pattern kernel: time tile (1024 or 512); 0 = plain kernel
     bool ws = false;            // warp-specialised variant of the shared-pattern kernel
+    bool ws_wide = false;       // ... with 32-bit accumulators and no intermediate flush (coarse time bins)
     std::vector<SpRecord> h_sp;
     std::vector<WsRecord> h_ws;
     void *d_sp = nullptr;
@@ -286,10 +287,11 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         {
             const char *env = std::getenv("AA_DEDISP");
             auto allowed = [&](const char *name) { return !env || !*env || std::strcmp(env, name) == 0; };
-            // 16-bit lanes take floor(65535 / (255 bin 4)) groups between flushes: binned input only while that is at
-            // least 8 (bin <= 8).  Measured on cfg4: with flushes every 4 / 2 groups (bins 16 / 32) the L2
-            // read-modify-write of the tile costs more than the plain kernel does (2.58 -> 2.78 s per step).
-            const bool ws_ok = !R.in16 || 65535 / (255 * R.r.bin * kSpG) >= 8;
+            // 16-bit lanes take floor(65535 / (255 bin 4)) groups between flushes.  Below 8 (bins 16, 32) the L2
+            // read-modify-write of the tile costs more than the plain kernel does (measured on cfg4: 2.58 -> 2.78 s
+            // per step), so those ranges use the 32-bit-accumulator variant (512-sample tiles, no flush) instead.
+            R.ws_wide = R.in16 && 65535 / (255 * R.r.bin * kSpG) < 8 && 4ull * 255 * R.r.bin <= 65535;
+            const bool ws_ok = true;
             // time tile: 1024 samples unless the range is so short per sub-chunk that 512-sample tiles (about 0.65 of
             // the time per CTA) need fewer waves of CTAs over the 148 SMs
             const uint64_t cols = p.L / (uint64_t)R.r.bin + (uint64_t)p.wmax - 1, nblk = ((uint64_t)R.r.ndms + kSpDB - 1) / kSpDB;
@@ -297,7 +299,9 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
             const double cost512 = 0.65 * (double)(((cols + 511) / 512 * nblk + 147) / 148);
             const int order[2] = {cost512 < cost1024 ? 512 : 1024, cost512 < cost1024 ? 1024 : 512};
             for (int tb : order) {
-                if (!ws_ok || R.sp_tb || !allowed(tb == 1024 ? "ws1024" : "ws512")) continue;
+                if (R.ws_wide ? (tb != 512 || !(allowed("ws1024") || allowed("ws512"))) : !allowed(tb == 1024 ? "ws1024" : "ws512"))
+                    continue;
+                if (!ws_ok || R.sp_tb) continue;
                 if (ws_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, R.in16 ? 2 : 1, 226 * 1024, R.h_ws, R.sp_rows,
                                     R.sp_pbytes)) {
                     R.sp_tb = tb;
@@ -314,6 +318,8 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
             }
             if (!R.sp_tb || R.ws) { R.h_sp.clear(); R.h_sp.shrink_to_fit(); }
             if (R.sp_tb) R.sp_flush = 65535 / (255 * R.r.bin * kSpG);
+            if (!R.ws) R.ws_wide = false;
+            if (R.ws_wide) R.sp_flush = 0;          // launch_dedisp_ws: 0 selects the 32-bit-accumulator kernel
         }
         if (!R.in16) max_row_u8 = std::max(max_row_u8, std::max(R.row, R.sp_tb ? R.sp_rows + R.sp_tb : 0));
         p.d_rows = std::max<uint64_t>(p.d_rows, (uint64_t)R.r.ndms);
@@ -892,6 +898,7 @@ int aa_plan_dedisp_variant(const aa_plan *p, int32_t r)
     if (!p || r < 0 || r >= (int32_t)p->ranges.size()) return AA_ERR_INVALID;
     const Range &R = p->ranges[r];
     if (!R.sp_tb) return 0;
+    if (R.ws_wide) return 5;
     return (R.ws ? 3 : 1) + (R.sp_tb == 1024 ? 1 : 0);
 }
 

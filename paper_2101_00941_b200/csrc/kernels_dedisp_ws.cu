@@ -259,9 +259,12 @@ __device__ __forceinline__ void build_stage(const WsRecord *R, const uint8_t *ra
     }
 }
 
-template <int TB, bool IN16>
+// WIDE: the consumers keep one 32-bit accumulator per sample (TB = 512) and never flush: for coarse time bins,
+// whose four-channel sums would fill 16-bit lanes after two or four groups.
+template <int TB, bool IN16, bool WIDE = false>
 __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
 {
+    static_assert(!WIDE || TB == 512, "32-bit accumulators: 4 trials x 16 samples per lane");
     constexpr int ES = IN16 ? 2 : 1;       // bytes per input sample
     constexpr int NP = TB / 64;            // 2-sample words per consumer lane
 
@@ -379,6 +382,49 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
 
     // ==================================== consumers ================================================
     asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REG_CONS));
+    if constexpr (WIDE) {
+        uint32_t acc[DPW][2 * NP];
+#pragma unroll
+        for (int k = 0; k < DPW; ++k)
+#pragma unroll
+            for (int i = 0; i < 2 * NP; ++i) acc[k][i] = 0;
+        const uint8_t *Pl = P0 + lane * 4;
+        const uint8_t *mypof = pof0 + warp * (DPW * 4);
+        for (int s = 0; s < nstages; ++s) {
+            const uint32_t sl = (uint32_t)(s % NSLOT), slot = 8u * sl;
+            mbar_wait(full + slot, (uint32_t)((s / NSLOT) & 1));
+            const uint4 po = *reinterpret_cast<const uint4 *>(mypof + sl * (DB * 4));
+            const uint32_t pof[4] = {po.x, po.y, po.z, po.w};
+#pragma unroll
+            for (int k = 0; k < DPW; ++k) {
+                const uint32_t *p = reinterpret_cast<const uint32_t *>(Pl + pof[k]);
+                uint32_t v[NP];
+#pragma unroll
+                for (int i = 0; i < NP; ++i) v[i] = p[i * 32];
+#pragma unroll
+                for (int i = 0; i < NP; ++i) {
+                    // low / high 16-bit lane of the row word into its own 32-bit accumulator (IDP.2A)
+                    asm("dp2a.lo.u32.u32 %0, %1, %2, %0;" : "+r"(acc[k][2 * i]) : "r"(v[i]), "r"(0x00000001u));
+                    asm("dp2a.lo.u32.u32 %0, %1, %2, %0;" : "+r"(acc[k][2 * i + 1]) : "r"(v[i]), "r"(0x00000100u));
+                }
+            }
+            __syncwarp();
+            if (lane == 0) mbar_arrive(empty + slot);
+        }
+#pragma unroll
+        for (int k = 0; k < DPW; ++k) {
+            const int d = d0 + warp * DPW + k;
+            if (d >= a.ndms) continue;
+            uint32_t *orow = a.out + (size_t)d * a.pitch_out + t0 + 2 * lane;
+#pragma unroll
+            for (int i = 0; i < NP; ++i) {
+                const int64_t t = t0 + 2 * (lane + 32 * i);
+                if (t + 1 < a.ncols) __stcg(reinterpret_cast<uint2 *>(orow + 64 * i), make_uint2(acc[k][2 * i], acc[k][2 * i + 1]));
+                else if (t < a.ncols) __stcg(orow + 64 * i, acc[k][2 * i]);
+            }
+        }
+        return;
+    }
     uint32_t acc16[DPW][NP];
 #pragma unroll
     for (int k = 0; k < DPW; ++k)
@@ -479,11 +525,11 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
     if (since || first) flush(first);
 }
 
-template <int TB, bool IN16>
+template <int TB, bool IN16, bool WIDE = false>
 cudaError_t launch_t(const DedispArgs &a, cudaStream_t st)
 {
     dim3 grid((unsigned)((a.ndms + DB - 1) / DB), (unsigned)((a.ncols + TB - 1) / TB));
-    dedisp_ws_kernel<TB, IN16><<<grid, NT, dedisp_ws_smem_bytes(a.sp_rows, a.sp_pbytes), st>>>(a);
+    dedisp_ws_kernel<TB, IN16, WIDE><<<grid, NT, dedisp_ws_smem_bytes(a.sp_rows, a.sp_pbytes), st>>>(a);
     return cudaGetLastError();
 }
 
@@ -507,12 +553,15 @@ cudaError_t dedisp_ws_configure()
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(dedisp_ws_kernel<1024, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(dedisp_ws_kernel<512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    e = cudaFuncSetAttribute(dedisp_ws_kernel<512, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(dedisp_ws_kernel<512, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
 }
 
 cudaError_t launch_dedisp_ws(const DedispArgs &a, int tb, bool in16, cudaStream_t st)
 {
     if (a.ncols <= 0 || a.ndms <= 0) return cudaSuccess;
+    if (a.sp_flush == 0) return launch_t<512, true, true>(a, st);      // 32-bit accumulators (coarse bins)
     if (in16) return tb == 1024 ? launch_t<1024, true>(a, st) : launch_t<512, true>(a, st);
     return tb == 1024 ? launch_t<1024, false>(a, st) : launch_t<512, false>(a, st);
 }
