@@ -246,6 +246,23 @@ def test_time_sharded_observation_equals_the_whole(B):
         assert merged.tobytes() == whole.tobytes() and len(whole) > 0, world
 
 
+def test_timeline_of_a_streamed_run(B):
+    """aa_get_timeline: one entry per sub-chunk, on its own stream, events in pipeline order; dedispersion kernels of
+    successive sub-chunks do not overlap (they are ordered across streams)."""
+    w = _tiny(nchans=64, nsamp=70000, n_streams=3, chunk_len=3 * 4096, ndms=48)
+    buf, _ = _pinned_fill(B, w)
+    with B.Plan(w) as plan:
+        plan.run(buf, want_taps=False)
+        tl = plan.timeline()
+        assert len(tl) == plan.info["n_subchunks"] > 6
+    for j, t in enumerate(tl):
+        assert t["index"] == j and t["stream"] == j % 3
+        assert 0 <= t["h2d_begin"] <= t["h2d_end"] <= t["prep_end"] <= t["compute_begin"] <= t["compute_end"] <= t["d2h_end"]
+        assert t["dedisp_ms"] > 0 and t["sps_ms"] > 0
+    for a, b in zip(tl[:-1], tl[1:]):
+        assert b["compute_end"] >= a["compute_end"] - a["sps_ms"] - 1e-3     # sub-chunk order on the device
+
+
 def test_saturated_input_and_constant_input(B):
     w = _tiny(nchans=300, nsamp=9000, foff=-0.3, dm_step=4.0, chunk_len=4096, norm_block=2048)
     buf = B.pinned_empty(w.nbytes)
