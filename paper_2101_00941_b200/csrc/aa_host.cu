@@ -44,6 +44,7 @@ struct Range {
     bool in16 = false;
     int flush_ch = 2;
     bool wide = false;          // 64-bit boxcar sums
+    bool small31 = false;       // boxcar sums below 2^31 (signed pre-filter arithmetic in the SPS kernel)
     int bin_slot = -1;          // index into the per-stream binned buffers
     int sp_tb = 0;              // shared-pattern kernel: time tile (1024 or 512); 0 = plain kernel
     bool ws = false;            // warp-specialised variant of the shared-pattern kernel
@@ -240,6 +241,7 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         R.flush_ch = (int)((65535 / (255 * R.r.bin)) & ~1);
         if (R.flush_ch < 2) return AA_ERR_INVALID;
         R.wide = 255ull * d->nchans * R.r.bin * p.wmax >= (1ull << 32);
+        R.small31 = 255ull * d->nchans * R.r.bin * p.wmax < (1ull << 31);
         if (R.in16) {
             auto it = std::find(p.bins.begin(), p.bins.end(), R.r.bin);
             if (it == p.bins.end()) { p.bins.push_back(R.r.bin); R.bin_slot = (int)p.bins.size() - 1; }
@@ -596,7 +598,7 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
                 sa.cands = S.d_cands;
                 sa.count = S.d_count;
                 sa.cap = (uint32_t)p->cap;
-                AA_W(launch_sps(sa, p->wt, Rg.wide, st));
+                AA_W(launch_sps(sa, p->wt, Rg.wide, Rg.small31, st));
                 S.sps_launches++;
                 AA_W(cudaEventRecord(e2, st));
                 // tapped rows: runs of consecutive trials leave in one strided copy (all rows tapped = the dense

@@ -143,7 +143,8 @@ cudaError_t launch_dedisp(const DedispArgs &a, bool in16, int dpw, cudaStream_t 
 size_t dedisp_smem_bytes(bool in16, int dpw, int row);
 int dedisp_stage_channels(bool in16);
 cudaError_t dedisp_configure();   // opt in to large dynamic shared memory (once per process)
-cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, cudaStream_t st);
+// wide: boxcar sums need 64 bits (255 nchans bin wmax >= 2^32); small31: they stay below 2^31
+cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, bool small31, cudaStream_t st);
 cudaError_t sps_configure();
 
 }  // namespace aa

@@ -273,6 +273,9 @@ __device__ __forceinline__ void st_cluster_u64(const void *local, uint32_t rank,
     asm volatile("st.shared::cluster.u64 [%0], %1;" ::"r"(r), "l"(v) : "memory");
 }
 
+// SMALL: every boxcar sum is below 2^31 (255 nchans bin wmax < 2^31), so the pre-filter B >= th is the sign of
+// (th - 1) - B and costs one 3-input add and one OR per (tau, width).
+template <bool SMALL>
 __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const __grid_constant__ WidthTable wt, const int C, const int seg)
 {
     extern __shared__ __align__(16) uint8_t dyn[];
@@ -348,7 +351,26 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
             span = sh.hi - lo;
         }
         uint64_t m = 0, S1 = 0, S2 = 0;
-        if (run) {
+        if (pass == 0) {                                  // every sample: no selection
+            uint32_t mc = 0;
+            for (int i = tid; i < n4; i += NT2) {
+                const uint4 v = reinterpret_cast<const uint4 *>(X)[i];
+                S1 += (uint64_t)v.x + v.y;
+                S1 += (uint64_t)v.z + v.w;
+                S2 += (uint64_t)v.x * v.x;
+                S2 += (uint64_t)v.y * v.y;
+                S2 += (uint64_t)v.z * v.z;
+                S2 += (uint64_t)v.w * v.w;
+                mc += 4;
+            }
+            for (int i = 4 * n4 + tid; i < n_own; i += NT2) {
+                const uint32_t x = X[i];
+                mc += 1;
+                S1 += x;
+                S2 += (uint64_t)x * x;
+            }
+            m = mc;
+        } else if (run) {
             uint32_t mc = 0;
             for (int i = tid; i < n4; i += NT2) {
                 const uint4 v = reinterpret_cast<const uint4 *>(X)[i];
@@ -419,12 +441,14 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
     }
     __syncthreads();
     if (tid == 0) {
+        // SMALL: th - 1 as a signed number, B >= th  <=>  (th - 1) - B < 0; th above every possible B -> never
+        auto enc = [&](uint32_t th) { return SMALL ? (th == 0u ? 0xFFFFFFFFu : (th > 0x7FFFFFFFu ? 0x7FFFFFFFu : th - 1u)) : th; };
         int n = 0;
         for (int j = 0; j < a.nwidths; ++j)
-            if ((sh.w[j] & 3) == 0) sh.wl[n++] = make_uint2((uint32_t)sh.w[j], sh.thr_u[j]);
+            if ((sh.w[j] & 3) == 0) sh.wl[n++] = make_uint2((uint32_t)sh.w[j], enc(sh.thr_u[j]));
         sh.na = n;
         for (int j = 0; j < a.nwidths; ++j)
-            if ((sh.w[j] & 3) != 0) sh.wl[n++] = make_uint2((uint32_t)sh.w[j], sh.thr_u[j]);
+            if ((sh.w[j] & 3) != 0) sh.wl[n++] = make_uint2((uint32_t)sh.w[j], enc(sh.thr_u[j]));
         sh.nu = n - sh.na;
     }
 
@@ -493,6 +517,7 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
     for (int g0 = 0; g0 < ngroups; g0 += 2 * NT2) {
         const int g = g0 + tid;
         uint32_t any = 0;
+        uint32_t f0 = 0, f1 = 0, f2 = 0, f3 = 0, f4 = 0, f5 = 0, f6 = 0, f7 = 0;   // SMALL: sign bits collect the hits
         if (g < ngroups) {
             const bool two = g + NT2 < ngroups;          // else the second group repeats the first
             const uint32_t *xg = X + 4 * g;
@@ -505,6 +530,11 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
                 const uint32_t th = wt2.y;
                 const uint4 qa = *reinterpret_cast<const uint4 *>(xg + wt2.x);
                 const uint4 qb = *reinterpret_cast<const uint4 *>(xg + wt2.x + gb);
+                if (SMALL) {
+                    f0 |= th + pa.x - qa.x; f1 |= th + pa.y - qa.y; f2 |= th + pa.z - qa.z; f3 |= th + pa.w - qa.w;
+                    f4 |= th + pb.x - qb.x; f5 |= th + pb.y - qb.y; f6 |= th + pb.z - qb.z; f7 |= th + pb.w - qb.w;
+                    continue;
+                }
                 any |= ((qa.x - pa.x) >= th ? 1u : 0u) | ((qa.y - pa.y) >= th ? 2u : 0u) | ((qa.z - pa.z) >= th ? 4u : 0u) |
                        ((qa.w - pa.w) >= th ? 8u : 0u) | ((qb.x - pb.x) >= th ? 16u : 0u) | ((qb.y - pb.y) >= th ? 32u : 0u) |
                        ((qb.z - pb.z) >= th ? 64u : 0u) | ((qb.w - pb.w) >= th ? 128u : 0u);
@@ -522,11 +552,19 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
                 if (r == 1) { v0 = q0.y; v1 = q0.z; v2 = q0.w; v3 = q1.x; v4 = q2.y; v5 = q2.z; v6 = q2.w; v7 = q3.x; }
                 else if (r == 2) { v0 = q0.z; v1 = q0.w; v2 = q1.x; v3 = q1.y; v4 = q2.z; v5 = q2.w; v6 = q3.x; v7 = q3.y; }
                 else { v0 = q0.w; v1 = q1.x; v2 = q1.y; v3 = q1.z; v4 = q2.w; v5 = q3.x; v6 = q3.y; v7 = q3.z; }
+                if (SMALL) {
+                    f0 |= th + pa.x - v0; f1 |= th + pa.y - v1; f2 |= th + pa.z - v2; f3 |= th + pa.w - v3;
+                    f4 |= th + pb.x - v4; f5 |= th + pb.y - v5; f6 |= th + pb.z - v6; f7 |= th + pb.w - v7;
+                    continue;
+                }
                 any |= ((v0 - pa.x) >= th ? 1u : 0u) | ((v1 - pa.y) >= th ? 2u : 0u) | ((v2 - pa.z) >= th ? 4u : 0u) |
                        ((v3 - pa.w) >= th ? 8u : 0u) | ((v4 - pb.x) >= th ? 16u : 0u) | ((v5 - pb.y) >= th ? 32u : 0u) |
                        ((v6 - pb.z) >= th ? 64u : 0u) | ((v7 - pb.w) >= th ? 128u : 0u);
             }
         }
+        if (SMALL)
+            any = (f0 >> 31) | (f1 >> 31) << 1 | (f2 >> 31) << 2 | (f3 >> 31) << 3 | (f4 >> 31) << 4 | (f5 >> 31) << 5 |
+                  (f6 >> 31) << 6 | (f7 >> 31) << 7;
         if (g < ngroups && g + NT2 >= ngroups) any &= 15u;   // the repeated group is not evaluated twice
         if (!__any_sync(0xffffffffu, any != 0)) continue;
 #pragma unroll 1
@@ -603,10 +641,12 @@ cudaError_t sps_configure()
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(sps_kernel<uint64_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
     if (e != cudaSuccess) return e;
-    return cudaFuncSetAttribute(sps_cluster_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+    e = cudaFuncSetAttribute(sps_cluster_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+    if (e != cudaSuccess) return e;
+    return cudaFuncSetAttribute(sps_cluster_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
 }
 
-cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, cudaStream_t st)
+cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, bool small31, cudaStream_t st)
 {
     if (a.nemit <= 0 || a.ndms <= 0) return cudaSuccess;
     const unsigned nblk = (unsigned)((a.nemit + a.block_len - 1) / a.block_len);
@@ -624,7 +664,8 @@ cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, cudaSt
         at[0].val.clusterDim.z = 1;
         cfg.attrs = at;
         cfg.numAttrs = 1;
-        return cudaLaunchKernelEx(&cfg, sps_cluster_kernel, a, wt, C, seg);
+        return small31 ? cudaLaunchKernelEx(&cfg, sps_cluster_kernel<true>, a, wt, C, seg)
+                       : cudaLaunchKernelEx(&cfg, sps_cluster_kernel<false>, a, wt, C, seg);
     }
     dim3 grid(nblk, (unsigned)a.ndms);
     if (wide)
