@@ -233,6 +233,26 @@ __device__ __forceinline__ void build_batch16(const WsRecord *R, const uint8_t *
     }
 }
 
+// ---- tensor memory (TMEM) as the second-level accumulator -------------------------------------------------
+// The 256 KB of TMEM of the SM hold the CTA's uint32 output tile (64 trials x 1024 samples): the 16-bit lanes
+// are flushed into it with tcgen05.ld / add / tcgen05.st (on-chip, ~12 cycles) instead of a read-modify-write
+// of the tile in L2.  A warp reaches the 32 TMEM lanes of its quadrant (warp % 4), one lane per thread
+// (shape 32x32b: register j of thread t <-> TMEM lane base + t, column + j).
+__device__ __forceinline__ void tmem_ld8(uint32_t (&v)[8], uint32_t taddr)
+{
+    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0, %1, %2, %3, %4, %5, %6, %7}, [%8];"
+                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
+                 : "r"(taddr)
+                 : "memory");
+    asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+}
+__device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&v)[8])
+{
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(v[0]), "r"(v[1]),
+                 "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+                 : "memory");
+}
+
 __device__ __forceinline__ void cp_async16(uint32_t dst, const void *src)
 {
     asm volatile("cp.async.ca.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(src) : "memory");
@@ -288,6 +308,13 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
     const int nstages = (a.nchans + G - 1) / G;
     const uint8_t *recs = static_cast<const uint8_t *>(a.sp_tab) + (size_t)blockIdx.x * nstages * REC;
 
+    // TMEM columns of the tile: 2 per packed accumulator word, 4 column groups (warp / 4) x 4 lane quadrants (warp % 4)
+    constexpr uint32_t TCOLS = WIDE ? 32u : (uint32_t)(8 * DPW * NP);
+    const uint32_t tmem_slot = empty + 8 * NSLOT;           // the allocator writes the TMEM base address here
+    if (!WIDE && warp == 0) {
+        asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"(tmem_slot), "n"(TCOLS) : "memory");
+        asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;" ::: "memory");
+    }
     if (tid == 0) {
 #pragma unroll
         for (int j = 0; j < NRAW; ++j) mbar_init(rawfull + 8 * j, 1);
@@ -298,7 +325,11 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
         }
         asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
     }
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
     __syncthreads();
+    asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+    uint32_t tmem_base_s;
+    asm volatile("ld.shared.u32 %0, [%1];" : "=r"(tmem_base_s) : "r"(tmem_slot) : "memory");
 
     if (warp >= NCW) {
         // ================================ producers ================================================
@@ -434,55 +465,59 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
     const bool whole = d0 + DB <= a.ndms && t0 + TB <= (int64_t)a.ncols;   // CTA-uniform: no edge tests
     uint32_t *otile = a.out + (size_t)(d0 + warp * DPW) * a.pitch_out + t0 + 2 * lane;
 
-    // adds the 16-bit lanes into the uint32 output tile (first time: plain store) and clears them
+    // this warp's part of the tile in TMEM: lane quadrant warp % 4, 2 * DPW * NP columns from (warp / 4) * that
+    const uint32_t ttile = tmem_base_s + ((uint32_t)(32 * (warp & 3)) << 16) + (uint32_t)((warp >> 2) * (2 * DPW * NP));
+
+    // adds the 16-bit lanes into the uint32 tile in TMEM (first time: plain store) and clears them
     auto flush = [&](bool first) {
-        if (whole) {
 #pragma unroll
-            for (int k = 0; k < DPW; ++k) {
-                uint2 *orow = reinterpret_cast<uint2 *>(otile + (size_t)k * a.pitch_out);
+        for (int k = 0; k < DPW; ++k) {
+#pragma unroll
+            for (int h = 0; h < NP; h += 4) {
+                const uint32_t col = ttile + (uint32_t)(2 * (k * NP + h));
+                uint32_t v[8];
                 if (first) {
 #pragma unroll
-                    for (int i = 0; i < NP; ++i) {
-                        __stcg(orow + 32 * i, make_uint2(acc16[k][i] & 0xFFFFu, acc16[k][i] >> 16));
-                        acc16[k][i] = 0;
-                    }
+                    for (int i = 0; i < 8; ++i) v[i] = 0;
                 } else {
-#pragma unroll
-                    for (int h = 0; h < NP; h += 8) {
-                        uint2 v[8];
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) v[i] = __ldcg(orow + 32 * (h + i));
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) {
-                            v[i].x += acc16[k][h + i] & 0xFFFFu;
-                            v[i].y += acc16[k][h + i] >> 16;
-                            acc16[k][h + i] = 0;
-                            __stcg(orow + 32 * (h + i), v[i]);
-                        }
-                    }
+                    tmem_ld8(v, col);
                 }
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    v[2 * i] += acc16[k][h + i] & 0xFFFFu;
+                    v[2 * i + 1] += acc16[k][h + i] >> 16;
+                    acc16[k][h + i] = 0;
+                }
+                tmem_st8(col, v);
             }
-            return;
         }
+        asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory");
+    };
+    // the finished tile: TMEM (if anything was flushed) plus what is still in the 16-bit lanes, to global memory
+    auto write_out = [&](bool first) {
 #pragma unroll
         for (int k = 0; k < DPW; ++k) {
             const int d = d0 + warp * DPW + k;
             uint32_t *orow = otile + (size_t)k * a.pitch_out;
 #pragma unroll
-            for (int i = 0; i < NP; ++i) {
-                const int64_t t = t0 + 2 * (lane + 32 * i);
-                const uint32_t lo = acc16[k][i] & 0xFFFFu, hi = acc16[k][i] >> 16;
-                acc16[k][i] = 0;
-                if (d >= a.ndms) continue;
-                if (t + 1 < a.ncols) {
-                    uint2 v = make_uint2(0, 0);
-                    if (!first) v = __ldcg(reinterpret_cast<const uint2 *>(orow + 64 * i));
-                    v.x += lo;
-                    v.y += hi;
-                    __stcg(reinterpret_cast<uint2 *>(orow + 64 * i), v);
-                } else if (t < a.ncols) {
-                    const uint32_t v = first ? 0u : __ldcg(orow + 64 * i);
-                    __stcg(orow + 64 * i, v + lo);
+            for (int h = 0; h < NP; h += 4) {
+                uint32_t v[8];
+                if (first) {
+#pragma unroll
+                    for (int i = 0; i < 8; ++i) v[i] = 0;
+                } else {
+                    tmem_ld8(v, ttile + (uint32_t)(2 * (k * NP + h)));
+                }
+#pragma unroll
+                for (int i = 0; i < 4; ++i) {
+                    const uint32_t lo = v[2 * i] + (acc16[k][h + i] & 0xFFFFu), hi = v[2 * i + 1] + (acc16[k][h + i] >> 16);
+                    if (whole) {
+                        __stcg(reinterpret_cast<uint2 *>(orow + 64 * (h + i)), make_uint2(lo, hi));
+                    } else if (d < a.ndms) {
+                        const int64_t t = t0 + 2 * (lane + 32 * (h + i));
+                        if (t + 1 < a.ncols) __stcg(reinterpret_cast<uint2 *>(orow + 64 * (h + i)), make_uint2(lo, hi));
+                        else if (t < a.ncols) __stcg(orow + 64 * (h + i), lo);
+                    }
                 }
             }
         }
@@ -522,7 +557,14 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
             since = 0;
         }
     }
-    if (since || first) flush(first);
+    write_out(first);
+    // every consumer warp is done with TMEM before warp 0 gives it back
+    asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+    asm volatile("bar.sync 1, %0;" ::"n"(32 * NCW) : "memory");
+    if (warp == 0) {
+        asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+        asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(tmem_base_s), "n"(TCOLS) : "memory");
+    }
 }
 
 template <int TB, bool IN16, bool WIDE = false>
@@ -537,7 +579,7 @@ cudaError_t launch_t(const DedispArgs &a, cudaStream_t st)
 
 size_t dedisp_ws_fixed_smem_bytes(int rows)
 {
-    return (size_t)NRAW * G * rows + (size_t)NPW * NRECBUF * REC + (size_t)NSLOT * DB * 4 + (NRAW + 2 * NSLOT) * 8;
+    return (size_t)NRAW * G * rows + (size_t)NPW * NRECBUF * REC + (size_t)NSLOT * DB * 4 + (NRAW + 2 * NSLOT) * 8 + 8;
 }
 
 size_t dedisp_ws_smem_bytes(int rows, int ring_bytes)
