@@ -289,12 +289,12 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         {
             const char *env = std::getenv("AA_DEDISP");
             auto allowed = [&](const char *name) { return !env || !*env || std::strcmp(env, name) == 0; };
-            // 16-bit lanes take floor(65535 / (255 bin 4)) groups between flushes.  With frequent flushes the L2
-            // read-modify-write of the tile dominates (bins 16, 32 were slower than the plain kernel), so ranges
-            // with fewer than 32 groups between flushes (bin >= 4) use the 32-bit-accumulator variant (512-sample
-            // tiles, no flush).  Measured on cfg4, seconds per step: wide for bin >= 16: 2.36, >= 8: 2.27,
-            // >= 4: 2.24, >= 2: 2.28.
-            R.ws_wide = R.in16 && 65535 / (255 * R.r.bin * kSpG) < 32 && 4ull * 255 * R.r.bin <= 65535;
+            // 16-bit lanes take floor(65535 / (255 bin 4)) groups between flushes into the TMEM tile.  Only with fewer
+            // than 4 (bin 32) the 32-bit-accumulator variant (512-sample tiles, no flush) is the faster one.  Measured
+            // on cfg4, seconds per step: wide for bin >= 4: 2.17, >= 16: 2.08, 32 only: 2.07, never: 2.08 (with the
+            // earlier L2 read-modify-write flushes: wide for bin >= 4 was best, and bins 16 / 32 on 16-bit lanes lost
+            // to the plain kernel).
+            R.ws_wide = R.in16 && 65535 / (255 * R.r.bin * kSpG) < 4 && 4ull * 255 * R.r.bin <= 65535;
             const bool ws_ok = true;
             // time tile: 1024 samples unless the range is so short per sub-chunk that 512-sample tiles (about 0.65 of
             // the time per CTA) need fewer waves of CTAs over the 148 SMs

@@ -132,8 +132,8 @@ def test_every_dedispersion_kernel_bit_exact(B, monkeypatch, variant, code, case
     dict(bins=(4,), nchans=1024, ndms=64, nsamp=40000, chunk_len=16384, foff=-0.2),      # 16 flushes of the 16-bit lanes
     dict(bins=(8,), nchans=512, ndms=130, nsamp=80000, chunk_len=32768, foff=-0.4),      # flush every 8 groups
     dict(bins=(1, 2, 8), nchans=256, ndms=70, nsamp=60000, chunk_len=16384),             # mixed 8-bit and binned ranges
-    dict(bins=(16,), nchans=512, ndms=70, nsamp=160000, chunk_len=65536, foff=-0.4, norm_block=4096),   # 32-bit accumulators
-    dict(bins=(32,), nchans=516, ndms=66, nsamp=300000, chunk_len=131072, foff=-0.4, norm_block=8192),
+    dict(bins=(16,), nchans=512, ndms=70, nsamp=160000, chunk_len=65536, foff=-0.4, norm_block=4096),   # flush every 4 groups
+    dict(bins=(32,), nchans=516, ndms=66, nsamp=300000, chunk_len=131072, foff=-0.4, norm_block=8192),  # 32-bit accumulators
 ])
 def test_binned_input_on_the_shared_pattern_kernel(B, monkeypatch, variant, code, case):
     """Time-binned (uint16) ranges on the warp-specialised shared-pattern kernel, against the oracle."""
@@ -143,7 +143,7 @@ def test_binned_input_on_the_shared_pattern_kernel(B, monkeypatch, variant, code
     w = _tiny(**kw)
     buf, x = _pinned_fill(B, w)
     with B.Plan(w, taps=list(range(w.ndms_total))) as plan:
-        want = [5 if rg.bin >= 4 else code for rg in w.ranges]      # bins >= 4: the 32-bit-accumulator variant
+        want = [5 if rg.bin >= 32 else code for rg in w.ranges]     # bin 32: the 32-bit-accumulator variant
         assert [plan.dedisp_variant(r) for r in range(len(w.ranges))] == want
         cands, tap = plan.run(buf)
     ref, dense, geo = oracle.run(x, w, keep_dense=True)
