@@ -78,3 +78,20 @@ def test_plan_geometry_without_a_gpu_matches_the_oracle():
         assert g["maxshift"] == geo["maxshift"] and g["t_valid"] == geo["t_valid"]
         assert g["dm_trial_samples"] == sum(r.ndms * n for r, n in zip(w.ranges, geo["nout"]))
         assert g["subchunk_len"] == w.chunk_len // w.n_streams and g["halo"] >= g["maxshift"]
+
+
+def test_sass_shows_the_blackwell_paths():
+    """The built library really contains what DESIGN.md claims (B200_PROFILING.md mnemonics): TMA bulk copies (UBLKCP),
+    mbarrier transactions (SYNCS), TMEM loads / stores and allocation for the dedispersion tile (LDTM / STTM / UTCATOMSWS),
+    setmaxnreg warp specialisation, cluster barriers of the SPS kernel, and no tensor-core MMA."""
+    import shutil
+    import subprocess
+    from paper_2101_00941_b200 import binding, build
+    build.build_cuda()
+    exe = shutil.which("cuobjdump") or "/usr/local/cuda/bin/cuobjdump"
+    if not os.path.exists(exe):
+        pytest.skip("cuobjdump not available")
+    sass = subprocess.run([exe, "-sass", binding.LIB_PATH], capture_output=True, text=True, check=True).stdout
+    for mnemonic in ("UBLKCP", "SYNCS.ARRIVE.TRANS64", "LDTM", "STTM", "UTCATOMSWS", "USETMAXREG", "UCGABAR_ARV", "IDP.2A"):
+        assert mnemonic in sass, mnemonic
+    assert "UTCMMA" not in sass and "HMMA" not in sass and "IMMA" not in sass      # a gather-add: no tensor-core contraction
