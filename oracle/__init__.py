@@ -179,7 +179,8 @@ def find_peaks(cands: np.ndarray) -> np.ndarray:
     Two candidates are NEIGHBOURS if their DM indices differ by at most 1 and their boxcars overlap or touch in
     raw samples: t' <= t + w and t <= t' + w'.  A candidate is a PEAK iff no neighbour beats it, where c' beats c
     iff snr' > snr, or snr' == snr and (dm_index', t_start') < (dm_index, t_start).  Returns the peaks in input
-    order.  O(n^2): for tests on small lists only.
+    order.  O(n^2): for tests on small lists only.  Parity unpinned against the paper (it fixes no rule): pinned
+    to this definition by hand-made lists and invariants (tests/test_oracle_pins.py).
     """
     n = len(cands)
     d = cands["dm_index"].astype(np.int64)
