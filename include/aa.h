@@ -39,6 +39,15 @@ typedef enum {
                                 the run is otherwise valid and *n_cands is the true total */
 } aa_status;
 
+typedef enum {
+    AA_DEDISP_AUTO = 0,
+    AA_DEDISP_PLAIN = 1,     /* plain tiled kernel */
+    AA_DEDISP_SP512 = 2,     /* shared-pattern kernel, 512-sample tiles */
+    AA_DEDISP_SP1024 = 3,    /* ... 1024-sample tiles */
+    AA_DEDISP_WS512 = 4,     /* warp-specialised shared-pattern kernel, 512-sample tiles */
+    AA_DEDISP_WS1024 = 5     /* ... 1024-sample tiles */
+} aa_dedisp_choice;
+
 /* One DM range of the plan: DM_i = dm_low + i*dm_step (double), i = 0..ndms-1, searched on
  * the input summed over `bin` consecutive raw samples (time decimation). */
 typedef struct {
@@ -91,6 +100,11 @@ typedef struct {
     /* 1: every stream also gets a small pinned input staging buffer ((subchunk_len + halo) * nchans
      * bytes) so that aa_run_staged can take an observation held in pageable memory */
     int32_t  stage_input;
+    /* Debug / A-B timing knob (an aa_dedisp_choice): AA_DEDISP_AUTO (0) lets the plan pick the dedispersion kernel of
+     * every range from its delay table.  Any other value restricts the choice to that one kernel family; a range the
+     * forced kernel cannot serve (tables do not fit) runs on the plain kernel.  Unknown values: AA_ERR_INVALID.  All
+     * kernels compute the same exact sums; tests force each one against the oracle. */
+    int32_t  dedisp_variant;
 } aa_plan_desc;
 
 typedef struct {

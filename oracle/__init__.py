@@ -51,8 +51,6 @@ def _load():
         lib.aaor_block_stats.argtypes = [vp, u64, vp, vp, vp]
         lib.aaor_sps_row.restype = i64
         lib.aaor_sps_row.argtypes = [vp, u64, u64, u64, u64, vp, i32, dbl, u64, u64, vp, vp, vp, i64]
-        lib.aaor_snr_at.restype = i32
-        lib.aaor_snr_at.argtypes = [vp, u64, u64, u64, dbl, dbl, vp, i32, u64, vp]
         lib.aaor_num_threads.restype = i32
         _lib = lib
     return _lib
@@ -146,20 +144,6 @@ def sps_row(d: np.ndarray, w, r: int, *, d_first: int = 0, tau_a: int = 0,
         if n <= cap:
             return tau[:n].copy(), ww[:n].copy(), sn[:n].copy()
         cap = int(n)
-
-
-def snr_at(d: np.ndarray, w, r: int, tau: int, mu: float, sigma: float, *, d_first: int = 0,
-           nout: Optional[int] = None) -> np.ndarray:
-    """S/N of every width at one tau (-inf where the boxcar does not fit)."""
-    d = np.ascontiguousarray(d, dtype=np.uint32)
-    widths = np.asarray(w.widths, dtype=np.int32)
-    out = np.empty(widths.size, dtype=np.float64)
-    if nout is None:
-        nout = geometry(w)["nout"][r]
-    if _load().aaor_snr_at(d.ctypes.data, d_first, d.size, nout, mu, sigma, widths.ctypes.data,
-                           widths.size, tau, out.ctypes.data) != 0:
-        raise ValueError("row segment does not cover tau")
-    return out
 
 
 def pack_candidates(dm_index: int, bin_: int, tau, ww, sn) -> np.ndarray:

@@ -96,7 +96,11 @@ int aaor_dedisperse(const uint32_t *y, int nchans, uint64_t y_first, uint64_t ny
         for (int c = 0; c < nchans; ++c) {
             int64_t dl = delays[(size_t)i * nchans + c];
             int64_t first = (int64_t)tau_first + dl - (int64_t)y_first;
-            if (first < 0 || (uint64_t)first + ntau > ny) { bad = 1; continue; }
+            if (first < 0 || (uint64_t)first + ntau > ny) {
+                #pragma omp atomic write
+                bad = 1;
+                continue;
+            }
             const uint32_t *src = y + (size_t)c * ny + (size_t)first;
             for (uint64_t k = 0; k < ntau; ++k) row[k] += src[k];
         }
@@ -181,23 +185,6 @@ int64_t aaor_sps_row(const uint32_t *d, uint64_t d_first, uint64_t d_count,
         }
     }
     return found;
-}
-
-/* S/N of every width at one tau (for tolerance-aware comparisons in tests). */
-int aaor_snr_at(const uint32_t *d, uint64_t d_first, uint64_t d_count, uint64_t nout,
-                double mu, double sigma, const int32_t *widths, int nwidths,
-                uint64_t tau, double *snr_out)
-{
-    for (int j = 0; j < nwidths; ++j) {
-        uint64_t w = (uint64_t)widths[j];
-        snr_out[j] = -INFINITY;
-        if (tau + w > nout) continue;
-        if (tau < d_first || tau + w > d_first + d_count) return -1;
-        int64_t B = 0;
-        for (uint64_t i = 0; i < w; ++i) B += d[tau + i - d_first];
-        snr_out[j] = ((double)B - (double)w * mu) / (sigma * sqrt((double)w));
-    }
-    return 0;
 }
 
 int aaor_num_threads(void)

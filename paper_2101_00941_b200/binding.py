@@ -16,6 +16,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libaa.so")
 
 AA_OK, AA_ERR_INVALID, AA_ERR_NOT_PINNED, AA_ERR_OOM, AA_ERR_CUDA, AA_ERR_OVERFLOW = 0, -1, -2, -3, -4, -5
+#: aa_dedisp_choice (aa_plan_desc.dedisp_variant)
+DEDISP_CHOICE = {"auto": 0, "plain": 1, "sp512": 2, "sp1024": 3, "ws512": 4, "ws1024": 5}
 
 CAND_DTYPE = np.dtype([("dm_index", np.uint32), ("t_start", np.uint32),
                        ("width", np.uint32), ("snr", np.float32)])
@@ -41,7 +43,8 @@ class PlanDescC(ctypes.Structure):
                 ("device_arena", ctypes.c_void_p), ("device_arena_bytes", ctypes.c_uint64),
                 ("streams", ctypes.POINTER(ctypes.c_void_p)),
                 ("ntap", ctypes.c_int32), ("tap_dm_indices", ctypes.POINTER(ctypes.c_uint32)),
-                ("max_cands_per_subchunk", ctypes.c_uint64), ("stage_input", ctypes.c_int32)]
+                ("max_cands_per_subchunk", ctypes.c_uint64), ("stage_input", ctypes.c_int32),
+                ("dedisp_variant", ctypes.c_int32)]
 
 
 class PlanInfoC(ctypes.Structure):
@@ -170,7 +173,7 @@ class Plan:
 
     def __init__(self, w, *, n_streams: Optional[int] = None, chunk_len: Optional[int] = None,
                  taps: Optional[Sequence[int]] = None, max_cands_per_subchunk: int = 0,
-                 torch_resources: bool = True, stage_input: bool = False):
+                 torch_resources: bool = True, stage_input: bool = False, dedisp_variant="auto"):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the path has no CPU fallback")
@@ -193,6 +196,7 @@ class Plan:
         d.tap_dm_indices = self._taps if taps else None
         d.max_cands_per_subchunk = int(max_cands_per_subchunk)
         d.stage_input = 1 if stage_input else 0
+        d.dedisp_variant = DEDISP_CHOICE[dedisp_variant] if isinstance(dedisp_variant, str) else int(dedisp_variant)
         self._arena = None
         self._streams = None
         if torch_resources:

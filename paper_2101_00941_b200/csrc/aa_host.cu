@@ -131,6 +131,7 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         return AA_ERR_INVALID;
     if (d->n_streams < 1 || d->n_streams > 64 || d->chunk_len < 1) return AA_ERR_INVALID;
     if (d->ntap < 0 || (d->ntap > 0 && !d->tap_dm_indices)) return AA_ERR_INVALID;
+    if (d->dedisp_variant < AA_DEDISP_AUTO || d->dedisp_variant > AA_DEDISP_WS1024) return AA_ERR_INVALID;
     if (d->nsamp > 0xFFFFFFFFull) return AA_ERR_INVALID;       // candidates carry 32-bit sample indices
 
     p.desc = *d;
@@ -282,20 +283,22 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
                         }
                     }
         }
-        // shared-pattern kernels: uint8 input, tables within limits, rows within shared memory.
-        // AA_DEDISP=plain forces the plain kernels, =ws1024 / ws512 / sp1024 / sp512 one variant (A/B timing, tests).
+        // shared-pattern kernels: tables within limits, rows within shared memory.  desc.dedisp_variant restricts
+        // the choice to one kernel family (A/B timing, tests).
         R.sp_tb = 0;
         R.ws = false;
         {
-            const char *env = std::getenv("AA_DEDISP");
-            auto allowed = [&](const char *name) { return !env || !*env || std::strcmp(env, name) == 0; };
+            const int force = d->dedisp_variant;
+            auto allowed = [&](int v) { return force == AA_DEDISP_AUTO || force == v; };
             // 16-bit lanes take floor(65535 / (255 bin 4)) groups between flushes into the TMEM tile.  Only with fewer
             // than 4 (bin 32) the 32-bit-accumulator variant (512-sample tiles, no flush) is the faster one.  Measured
             // on cfg4, seconds per step: wide for bin >= 4: 2.17, >= 16: 2.08, 32 only: 2.07, never: 2.08 (with the
             // earlier L2 read-modify-write flushes: wide for bin >= 4 was best, and bins 16 / 32 on 16-bit lanes lost
             // to the plain kernel).
-            R.ws_wide = R.in16 && 65535 / (255 * R.r.bin * kSpG) < 4 && 4ull * 255 * R.r.bin <= 65535;
-            const bool ws_ok = true;
+            // The producers add the four channels of a group in 16-bit lanes: binned samples need 4 * 255 * bin < 2^16,
+            // i.e. bin <= 64; coarser bins run on the plain kernel.
+            const bool ws_ok = !R.in16 || 4ull * 255 * R.r.bin <= 65535;
+            R.ws_wide = R.in16 && ws_ok && 65535 / (255 * R.r.bin * kSpG) < 4;
             // time tile: 1024 samples unless the range is so short per sub-chunk that 512-sample tiles (about 0.65 of
             // the time per CTA) need fewer waves of CTAs over the 148 SMs
             const uint64_t cols = p.L / (uint64_t)R.r.bin + (uint64_t)p.wmax - 1, nblk = ((uint64_t)R.r.ndms + kSpDB - 1) / kSpDB;
@@ -303,7 +306,8 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
             const double cost512 = 0.65 * (double)(((cols + 511) / 512 * nblk + 147) / 148);
             const int order[2] = {cost512 < cost1024 ? 512 : 1024, cost512 < cost1024 ? 1024 : 512};
             for (int tb : order) {
-                if (R.ws_wide ? (tb != 512 || !(allowed("ws1024") || allowed("ws512"))) : !allowed(tb == 1024 ? "ws1024" : "ws512"))
+                if (R.ws_wide ? (tb != 512 || !(allowed(AA_DEDISP_WS1024) || allowed(AA_DEDISP_WS512)))
+                              : !allowed(tb == 1024 ? AA_DEDISP_WS1024 : AA_DEDISP_WS512))
                     continue;
                 if (!ws_ok || R.sp_tb) continue;
                 if (ws_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, R.in16 ? 2 : 1, 226 * 1024, R.h_ws, R.sp_rows,
@@ -314,16 +318,15 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
             }
             if (!R.ws) { R.h_ws.clear(); R.h_ws.shrink_to_fit(); }
             for (int tb : {1024, 512}) {
-                if (R.in16 || R.sp_tb || !allowed(tb == 1024 ? "sp1024" : "sp512")) continue;
+                if (R.in16 || R.sp_tb || !allowed(tb == 1024 ? AA_DEDISP_SP1024 : AA_DEDISP_SP512)) continue;
                 const size_t limit = tb == 1024 ? 227 * 1024 : 113 * 1024;
                 if (sp_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, tb, R.h_sp, R.sp_rows, R.sp_pbytes) &&
                     dedisp_sp_smem_bytes(R.sp_rows, R.sp_pbytes) + 1024 <= limit)
                     R.sp_tb = tb;
             }
             if (!R.sp_tb || R.ws) { R.h_sp.clear(); R.h_sp.shrink_to_fit(); }
-            if (R.sp_tb) R.sp_flush = 65535 / (255 * R.r.bin * kSpG);
+            if (R.sp_tb) R.sp_flush = std::max(1, 65535 / (255 * R.r.bin * kSpG));
             if (!R.ws) R.ws_wide = false;
-            if (R.ws_wide) R.sp_flush = 0;          // launch_dedisp_ws: 0 selects the 32-bit-accumulator kernel
         }
         if (!R.in16) max_row_u8 = std::max(max_row_u8, std::max(R.row, R.sp_tb ? R.sp_rows + R.sp_tb : 0));
         p.d_rows = std::max<uint64_t>(p.d_rows, (uint64_t)R.r.ndms);
@@ -572,7 +575,7 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
                 da.sp_rows = Rg.sp_rows;
                 da.sp_pbytes = Rg.sp_pbytes;
                 da.sp_flush = Rg.sp_flush;
-                if (Rg.ws) AA_W(launch_dedisp_ws(da, Rg.sp_tb, Rg.in16, st));
+                if (Rg.ws) AA_W(launch_dedisp_ws(da, Rg.sp_tb, Rg.in16, Rg.ws_wide, st));
                 else if (Rg.sp_tb) AA_W(launch_dedisp_sp(da, Rg.sp_tb, st));
                 else AA_W(launch_dedisp(da, Rg.in16, Rg.dpw, st));
                 S.dedisp_launches++;

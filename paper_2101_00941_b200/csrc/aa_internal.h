@@ -93,7 +93,8 @@ constexpr int kWsWindow = 8;        // ... so a stage never starts before stage 
 // elem_bytes: 1 (uint8 input) or 2 (time-binned uint16 input)
 bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t tb, int32_t elem_bytes,
                      size_t smem_budget, std::vector<WsRecord> &out, int32_t &rows, int32_t &ring_bytes);
-cudaError_t launch_dedisp_ws(const DedispArgs &a, int tb, bool in16, cudaStream_t st);
+// wide: the 32-bit-accumulator variant (512-sample tiles, 16-bit input only)
+cudaError_t launch_dedisp_ws(const DedispArgs &a, int tb, bool in16, bool wide, cudaStream_t st);
 size_t dedisp_ws_fixed_smem_bytes(int rows);            // everything but the ring
 size_t dedisp_ws_smem_bytes(int rows, int ring_bytes);
 cudaError_t dedisp_ws_configure();

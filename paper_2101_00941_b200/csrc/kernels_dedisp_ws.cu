@@ -18,7 +18,8 @@
 //             Pattern rows live in a shared-memory ring whose offsets are fixed at plan time, so a
 //             stage takes exactly the room it needs and about six stages are in flight.
 //   consumers a warp owns 4 trials, a lane TB/64 words of 2 samples: acc16 += row word (SWAR).
-//             Every sp_flush groups the 16-bit lanes are added into the uint32 output tile (L2).
+//             Every sp_flush groups the 16-bit lanes are added into the uint32 output tile, which lives in
+//             tensor memory (TMEM); only the finished tile goes to global memory.
 //   full[] / empty[] mbarrier rings (one slot per stage, modulo 16) order the two sides; nothing in
 //   the loop is CTA-wide.
 // No tensor cores: a gather-add, not a dense contraction.
@@ -600,10 +601,10 @@ cudaError_t dedisp_ws_configure()
     return cudaFuncSetAttribute(dedisp_ws_kernel<512, true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024);
 }
 
-cudaError_t launch_dedisp_ws(const DedispArgs &a, int tb, bool in16, cudaStream_t st)
+cudaError_t launch_dedisp_ws(const DedispArgs &a, int tb, bool in16, bool wide, cudaStream_t st)
 {
     if (a.ncols <= 0 || a.ndms <= 0) return cudaSuccess;
-    if (a.sp_flush == 0) return launch_t<512, true, true>(a, st);      // 32-bit accumulators (coarse bins)
+    if (wide) return launch_t<512, true, true>(a, st);                 // 32-bit accumulators (coarse bins)
     if (in16) return tb == 1024 ? launch_t<1024, true>(a, st) : launch_t<512, true>(a, st);
     return tb == 1024 ? launch_t<1024, false>(a, st) : launch_t<512, false>(a, st);
 }

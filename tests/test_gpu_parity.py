@@ -76,6 +76,13 @@ def test_delay_tables_match_oracle_entry_by_entry(B):
     dict(n_streams=3, chunk_len=3 * 2048, nsamp=30000),         # streams
     dict(widths=(1, 3, 5, 32), thr=4.0),                        # arbitrary widths
     dict(nchans=300, nsamp=12000, foff=-0.3, dm_step=4.0, chunk_len=4096, norm_block=2048),  # flushes of the 16-bit lanes
+    # bins that are not 2..32 powers of two: the generic binning kernel
+    dict(bins=(3,), norm_block=1536, chunk_len=3 * 1536, nsamp=30000),
+    dict(bins=(1, 6), norm_block=1536, chunk_len=4 * 1536, nsamp=40000),
+    dict(bins=(5, 10), norm_block=1280, chunk_len=5 * 1280, nsamp=50000, n_streams=5),
+    dict(bins=(2, 3), norm_block=1536, chunk_len=4 * 1536, nsamp=40000, nchans=30),          # fused and generic binning together
+    dict(bins=(64,), norm_block=4096, chunk_len=32768, nsamp=200000, ndms=12),
+    dict(bins=(128,), norm_block=8192, chunk_len=65536, nsamp=400000, ndms=8, widths=(1, 2, 4)),
 ])
 def test_small_cases_bit_exact(B, case):
     w = _tiny(**case)
@@ -108,14 +115,13 @@ def test_sps_and_corner_turn_variants(B, case):
     dict(nchans=302, ndms=100, nsamp=21000, chunk_len=8192),                 # padded channel group, partial DM block, ragged tile
     dict(nchans=1024, ndms=64, nsamp=9000, chunk_len=4096, foff=-0.2),      # four flushes of the 16-bit lanes
 ])
-def test_every_dedispersion_kernel_bit_exact(B, monkeypatch, variant, code, case):
-    """Fine channels / fine DM steps so that the shared-pattern tables exist; AA_DEDISP picks the kernel."""
-    monkeypatch.setenv("AA_DEDISP", variant)
+def test_every_dedispersion_kernel_bit_exact(B, variant, code, case):
+    """Fine channels / fine DM steps so that the shared-pattern tables exist; aa_plan_desc.dedisp_variant picks the kernel."""
     kw = dict(f_top=1500.0, foff=-0.5, dm_step=0.25, norm_block=1024, widths=(1, 2, 4, 8), thr=5.0)
     kw.update(case)
     w = _tiny(**kw)
     buf, x = _pinned_fill(B, w)
-    with B.Plan(w, taps=list(range(w.ndms_total))) as plan:
+    with B.Plan(w, taps=list(range(w.ndms_total)), dedisp_variant=variant) as plan:
         assert plan.dedisp_variant(0) == code
         cands, tap = plan.run(buf)
         nout = plan.nout
@@ -134,16 +140,21 @@ def test_every_dedispersion_kernel_bit_exact(B, monkeypatch, variant, code, case
     dict(bins=(1, 2, 8), nchans=256, ndms=70, nsamp=60000, chunk_len=16384),             # mixed 8-bit and binned ranges
     dict(bins=(16,), nchans=512, ndms=70, nsamp=160000, chunk_len=65536, foff=-0.4, norm_block=4096),   # flush every 4 groups
     dict(bins=(32,), nchans=516, ndms=66, nsamp=300000, chunk_len=131072, foff=-0.4, norm_block=8192),  # 32-bit accumulators
+    dict(bins=(3,), nchans=302, ndms=100, nsamp=60000, chunk_len=4 * 3072, norm_block=3072),           # generic binning kernel
+    dict(bins=(6, 12), nchans=512, ndms=70, nsamp=120000, chunk_len=8 * 3072, norm_block=3072, foff=-0.4),
+    dict(bins=(48,), nchans=516, ndms=66, nsamp=400000, chunk_len=16 * 6144, foff=-0.4, norm_block=6144),  # 32-bit accumulators
+    dict(bins=(64,), nchans=512, ndms=66, nsamp=500000, chunk_len=131072, foff=-0.4, norm_block=8192),    # 4*255*64 = 65280: the limit of the 16-bit rows
+    dict(bins=(96,), nchans=512, ndms=40, nsamp=700000, chunk_len=16 * 12288, foff=-0.4, norm_block=12288),  # past it: plain kernel
 ])
-def test_binned_input_on_the_shared_pattern_kernel(B, monkeypatch, variant, code, case):
+def test_binned_input_on_the_shared_pattern_kernel(B, variant, code, case):
     """Time-binned (uint16) ranges on the warp-specialised shared-pattern kernel, against the oracle."""
-    monkeypatch.setenv("AA_DEDISP", variant)
     kw = dict(f_top=1500.0, foff=-0.5, dm_step=0.25, norm_block=2048, widths=(1, 2, 4, 8), thr=5.0)
     kw.update(case)
     w = _tiny(**kw)
     buf, x = _pinned_fill(B, w)
-    with B.Plan(w, taps=list(range(w.ndms_total))) as plan:
-        want = [5 if rg.bin >= 32 else code for rg in w.ranges]     # bin 32: the 32-bit-accumulator variant
+    with B.Plan(w, taps=list(range(w.ndms_total)), dedisp_variant=variant) as plan:
+        # bins 32..64: the 32-bit-accumulator variant; coarser: four-channel sums overflow 16 bits -> plain kernel
+        want = [0 if rg.bin > 64 else 5 if rg.bin >= 32 else code for rg in w.ranges]
         assert [plan.dedisp_variant(r) for r in range(len(w.ranges))] == want
         cands, tap = plan.run(buf)
     ref, dense, geo = oracle.run(x, w, keep_dense=True)
@@ -155,26 +166,26 @@ def test_binned_input_on_the_shared_pattern_kernel(B, monkeypatch, variant, code
     assert res["only_gpu"] == 0 and res["only_oracle"] == 0
 
 
-def test_saturated_binned_input(B, monkeypatch):
-    for variant, b in (("ws1024", 8), ("ws512", 2), ("plain", 4), ("plain", 32), ("ws512", 32), ("ws512", 16)):
-        monkeypatch.setenv("AA_DEDISP", variant)
-        w = _tiny(bins=(b,), nchans=1024, ndms=70, nsamp=40000, chunk_len=16384, f_top=1500.0, foff=-0.2, dm_step=0.25,
-                  norm_block=2048)
+def test_saturated_binned_input(B):
+    for variant, b in (("ws1024", 8), ("ws512", 2), ("plain", 4), ("plain", 32), ("ws512", 32), ("ws512", 16),
+                       ("auto", 64), ("plain", 64), ("auto", 128), ("auto", 48), ("auto", 96)):
+        nb = 2048 if 2048 % b == 0 else 32 * b       # a multiple of the bin and of 16
+        w = _tiny(bins=(b,), nchans=1024, ndms=70, nsamp=40000, chunk_len=8 * nb, f_top=1500.0, foff=-0.2, dm_step=0.25,
+                  norm_block=nb)
         buf = B.pinned_empty(w.nbytes)
         buf.numpy()[:] = 255                         # every 16-bit lane at its limit before every flush
-        with B.Plan(w, taps=list(range(w.ndms_total))) as plan:
+        with B.Plan(w, taps=list(range(w.ndms_total)), dedisp_variant=variant) as plan:
             cands, tap = plan.run(buf)
             assert len(cands) == 0
             assert np.all(tap[:, :plan.nout[0]] == 255 * w.nchans * b)
 
 
-def test_saturated_input_every_kernel(B, monkeypatch):
+def test_saturated_input_every_kernel(B):
     for variant in ("ws1024", "ws512", "sp1024", "plain"):
-        monkeypatch.setenv("AA_DEDISP", variant)
         w = _tiny(nchans=1024, ndms=70, nsamp=9000, chunk_len=4096, f_top=1500.0, foff=-0.2, dm_step=0.25, norm_block=1024)
         buf = B.pinned_empty(w.nbytes)
         buf.numpy()[:] = 255                         # 16-bit lanes at their limit before every flush
-        with B.Plan(w, taps=list(range(w.ndms_total))) as plan:
+        with B.Plan(w, taps=list(range(w.ndms_total)), dedisp_variant=variant) as plan:
             cands, tap = plan.run(buf)
             assert len(cands) == 0
             assert np.all(tap[:, :plan.nout[0]] == 255 * w.nchans)
@@ -200,10 +211,12 @@ def test_stream_and_chunk_invariance(B):
 
 def test_pageable_input_through_pinned_staging(B):
     """aa_run_staged (pageable observation, small pinned staging, one copy thread per stream)
-    returns exactly what aa_run returns on the pinned copy; aa_run itself keeps refusing pageable memory."""
+    equals the oracle, and returns exactly what aa_run returns on the pinned copy; aa_run itself keeps refusing
+    pageable memory."""
     w = _tiny(nchans=64, nsamp=70000, n_streams=3, chunk_len=3 * 4096, ndms=48)
     buf, x = _pinned_fill(B, w)
     taps = list(range(w.ndms_total))
+    ref, dense, geo = oracle.run(x, w, keep_dense=True)
     with B.Plan(w, taps=taps) as plan:
         want, want_tap = plan.run(buf)
         with pytest.raises(B.AAError):
@@ -216,6 +229,9 @@ def test_pageable_input_through_pinned_staging(B):
         with pytest.raises(B.AAError):
             plan.run(pageable)
         again, _ = plan.run(buf)                           # the same plan still takes pinned input directly
+    assert np.array_equal(got_tap[:, :geo["nout"][0]], dense[0])            # staged path against the oracle
+    res = compare_candidates(got, ref, w.snr_threshold)
+    assert res["only_gpu"] == 0 and res["only_oracle"] == 0 and res["width_ties"] == 0 and len(ref) > 0
     assert got.tobytes() == want.tobytes() == again.tobytes() and len(want) > 0
     assert np.array_equal(got_tap, want_tap)
 
@@ -229,6 +245,7 @@ def test_time_sharded_observation_equals_the_whole(B):
     with B.Plan(w) as plan:
         whole, _ = plan.run(buf, want_taps=False)
         info = plan.info
+    ref, _ = oracle.run(x, w)
     tail = info["halo"] - info["maxshift"]
     for world in (2, 3, 5):
         parts = []
@@ -243,6 +260,8 @@ def test_time_sharded_observation_equals_the_whole(B):
             parts.append(dist_util.merge_shards(c, shard))
         merged = np.concatenate(parts)
         merged = merged[np.lexsort((merged["t_start"], merged["dm_index"]))]
+        res = compare_candidates(merged, ref, w.snr_threshold)                 # the merged shards against the oracle
+        assert res["only_gpu"] == 0 and res["only_oracle"] == 0 and res["width_ties"] == 0 and len(ref) > 0, world
         assert merged.tobytes() == whole.tobytes() and len(whole) > 0, world
 
 

@@ -62,10 +62,13 @@ def _global_rows(w, per_range):
 
 def _check_cells(w, x, cands, tap, tapidx, cells):
     """cells: list of (range, [rows], block index)."""
+    from concurrent.futures import ThreadPoolExecutor
     geo = oracle.geometry(w)
     base = np.cumsum([0] + [rg.ndms for rg in w.ranges])
     wmax = max(w.widths)
     n_checked = n_cands = 0
+    # candidates of each tapped row, once (the list is sorted by (dm_index, t_start))
+    lo = np.searchsorted(cands["dm_index"], np.arange(int(base[-1]) + 1))
     for r, rows, k in cells:
         rg = w.ranges[r]
         Lr = w.norm_block // rg.bin
@@ -76,17 +79,60 @@ def _check_cells(w, x, cands, tap, tapidx, cells):
         nblk = min(Lr, nout - t0)
         ntau = min(Lr + wmax - 1, nout - t0)
         D = oracle.dedisperse(x, w, r, rows=rows, tau_first=t0, ntau=ntau, geo=geo)
-        for i, d in enumerate(rows):
+
+        def one(i):
+            d = rows[i]
             g = int(base[r]) + d
             got = tap[tapidx[g], t0:t0 + nblk]
             assert np.array_equal(got, D[i, :nblk]), f"dedispersed row differs: range {r} dm {d} block {k}"
             tau, ww, sn = oracle.sps_row(D[i], w, r, d_first=t0, tau_a=t0, tau_b=t0 + nblk, nout=nout)
             ref = oracle.pack_candidates(g, rg.bin, tau, ww, sn)
-            sel = (cands["dm_index"] == g) & (cands["t_start"] >= t0 * rg.bin) & (cands["t_start"] < (t0 + nblk) * rg.bin)
-            compare_candidates(cands[sel], ref, w.snr_threshold)
-            n_checked += 1
-            n_cands += len(ref)
+            row = cands[lo[g]:lo[g + 1]]
+            sel = (row["t_start"] >= t0 * rg.bin) & (row["t_start"] < (t0 + nblk) * rg.bin)
+            compare_candidates(row[sel], ref, w.snr_threshold)
+            return len(ref)
+
+        with ThreadPoolExecutor(max_workers=os.cpu_count() or 1) as ex:
+            for n in ex.map(one, range(len(rows))):
+                n_checked += 1
+                n_cands += n
     return n_checked, n_cands
+
+
+def _stratified_cells(w, subchunk_len, n_rows=64, n_seams=3, n_random_blocks=2, seed=0, max_pulses=16):
+    """SURVEY 8(d) / BASELINE.md section 3: at least `n_rows` DM rows (first and last trial, both trials at every
+    range edge, every injected DM +-1, the rest seeded-random), each checked on normalisation blocks spread over the
+    whole time span: the first block, the ragged last one, both blocks on either side of `n_seams` sub-chunk seams,
+    and `n_random_blocks` seeded-random ones.  Returns the cell list for _check_cells."""
+    geo = oracle.geometry(w)
+    rng = np.random.default_rng(2101_00941 + seed)
+    base = np.cumsum([0] + [rg.ndms for rg in w.ranges])
+    rows = set()
+    for r, rg in enumerate(w.ranges):
+        rows |= {int(base[r]), int(base[r]) + rg.ndms - 1}
+        for p in w.pulses[:max_pulses]:
+            hi = rg.dm_low + rg.dm_step * (rg.ndms - 1)
+            if rg.dm_low <= p.dm <= hi and rg.dm_step > 0:
+                d = int(round((p.dm - rg.dm_low) / rg.dm_step))
+                rows |= {int(base[r]) + min(max(d + e, 0), rg.ndms - 1) for e in (-1, 0, 1)}
+    while len(rows) < n_rows:
+        rows.add(int(rng.integers(0, base[-1])))
+    per_range = {}
+    for g in sorted(rows):
+        r = int(np.searchsorted(base, g, side="right")) - 1
+        per_range.setdefault(r, []).append(g - int(base[r]))
+    nblocks = -(-geo["t_valid"] // w.norm_block)                  # blocks on the raw time axis (the last one ragged)
+    per_sub = subchunk_len // w.norm_block
+    n_sub = -(-geo["t_valid"] // subchunk_len)
+    seams = sorted({int(v) for v in np.linspace(1, max(1, n_sub - 1), n_seams)}) if n_sub > 1 else []
+    blocks = {0, nblocks - 1}
+    for j in seams:                                               # sub-chunk j starts at block j * per_sub
+        blocks |= {j * per_sub - 1, j * per_sub}
+    while len(blocks) < 2 + 2 * len(seams) + n_random_blocks and len(blocks) < nblocks:
+        blocks.add(int(rng.integers(0, nblocks)))
+    blocks = sorted(b for b in blocks if 0 <= b < nblocks)
+    cells = [(r, rws, k) for k in blocks for r, rws in sorted(per_range.items())]
+    return cells, len(rows), blocks
 
 
 def _pulse_cells(w, geo, max_pulses=4, extra=()):
@@ -133,6 +179,11 @@ def _run_sampled(B, w, cells_extra, max_pulses=4, **plan_kw):
     buf, x = _pinned_fill(B, w)
     geo = oracle.geometry(w)
     cells = _pulse_cells(w, geo, max_pulses=max_pulses, extra=cells_extra)
+    # one oracle call per (range, block): merge the row lists of cells that share them
+    merged = {}
+    for r, rows, k in cells:
+        merged.setdefault((k, r), set()).update(rows)
+    cells = [(r, sorted(rows), k) for (k, r), rows in sorted(merged.items())]
     per_range = {}
     for r, rows, _ in cells:
         per_range.setdefault(r, set()).update(rows)
@@ -147,11 +198,14 @@ def _run_sampled(B, w, cells_extra, max_pulses=4, **plan_kw):
 
 
 def test_cfg3_full_size_sampled(B):
-    """Workload and launch configuration bench.py times: 4096 x 2^23, 2048 trials, 8 streams."""
+    """Workload and launch configuration bench.py times: 4096 x 2^23, 2048 trials, 8 streams.  >= 64 stratified DM
+    rows, each on blocks over the whole time span (first, ragged last, both sides of sub-chunk seams, random), plus
+    the block holding every injected pulse on the rows around its DM."""
     w = I.workload(3)
-    extra = [(0, [0, 1, 777, 2047], 0), (0, [5, 1023, 2046], 63), (0, [2047, 300], 127)]   # first / middle / last (ragged) block
-    cands, n_cells, n_ref, stats = _run_sampled(B, w, extra)
-    assert n_cells >= 15 and n_ref > 0
+    extra, n_rows, blocks = _stratified_cells(w, w.chunk_len // w.n_streams)
+    assert n_rows >= 64 and len(blocks) >= 9
+    cands, n_cells, n_ref, stats = _run_sampled(B, w, extra, max_pulses=len(w.pulses))
+    assert n_cells >= 64 * 9 and n_ref > 0
     assert stats["h2d_bytes"] == w.nbytes                     # every input byte crosses the link once
 
 
@@ -174,14 +228,18 @@ def test_cfg5_reduced_length_sampled_16_streams(B):
 @pytest.mark.skipif(not _full(60), reason="needs 34.4 GB pinned + headroom (AA_FULL=1 forces it)")
 def test_cfg4_full_size_sampled(B):
     w = I.workload(4)
-    extra = [(r, [0, w.ranges[r].ndms - 1], k) for r in range(6) for k in (0, 64, 127)]
-    cands, n_cells, n_ref, _ = _run_sampled(B, w, extra)
-    assert n_cells >= 36 and n_ref > 0
+    extra, n_rows, blocks = _stratified_cells(w, w.chunk_len // w.n_streams, n_seams=2, n_random_blocks=1)
+    assert n_rows >= 64 and len(blocks) >= 6
+    cands, n_cells, n_ref, _ = _run_sampled(B, w, extra, max_pulses=len(w.pulses))
+    assert n_cells >= 64 * 6 and n_ref > 0
 
 
 @pytest.mark.skipif(not _full(110), reason="needs 68.7 GB of pinned host memory + headroom (AA_FULL=1 forces it)")
 def test_cfg5_full_size_sampled(B):
     w = I.workload(5)
-    extra = [(0, [0, 2047], 0), (0, [1000], 128), (0, [1, 2046], 255)]
-    cands, n_cells, n_ref, stats = _run_sampled(B, w, extra, max_pulses=6, n_streams=8)
+    n_streams = 8
+    extra, n_rows, blocks = _stratified_cells(w, w.chunk_len // n_streams, n_seams=2, n_random_blocks=1)
+    assert n_rows >= 64 and len(blocks) >= 6
+    cands, n_cells, n_ref, stats = _run_sampled(B, w, extra, max_pulses=8, n_streams=n_streams)
+    assert n_cells >= 64 * 6 and n_ref > 0
     assert stats["h2d_bytes"] == w.nbytes

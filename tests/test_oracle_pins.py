@@ -111,7 +111,7 @@ def test_single_impulse_lands_at_t_minus_delay():
             assert np.array_equal(D[d], expect), (c, d)
 
 
-@pytest.mark.parametrize("bins", [(1,), (2,), (1, 4), (8,)])
+@pytest.mark.parametrize("bins", [(1,), (2,), (1, 4), (8,), (3,), (1, 6), (5, 10)])
 def test_dedispersion_brute_force_python_loops(bins):
     w = _tiny(nchans=6, nsamp=520, bins=bins, ndms=5, seed=len(bins))
     x = I.fill(w)
