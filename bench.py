@@ -196,6 +196,27 @@ def run_reference(args):
     return 0
 
 
+def run_microbench():
+    """The measured denominators: lane-operations per clock per SM of the integer instructions the
+    kernels use, shared-memory bytes per clock per SM, pinned host-link GB/s.  profiles/r2_microbench.md is this output."""
+    import torch
+    from paper_2101_00941_b200 import binding as B
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py --microbench needs a CUDA device")
+    torch.cuda.set_device(0)
+    B.load_library()
+    sampler = ClockSampler(0)
+    sampler.start()
+    res = B.microbench()
+    clocks = sampler.stop()
+    nsm = torch.cuda.get_device_properties(0).multi_processor_count
+    print(json.dumps({"microbench": res, "n_sm": nsm, "clocks": clocks, "gpu": torch.cuda.get_device_name(0),
+                      "units": {"arithmetic": "lane-operations per clock per SM (a full-warp instruction = 32)",
+                                "shared memory": "bytes per clock per SM, conflict-free accesses",
+                                "link": "GB/s, 1 GiB pinned copies, best of 5"}}))
+    return 0
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -212,9 +233,14 @@ def main():
                          "per rank, candidate lists gathered on rank 0); default: one observation per rank (weak)")
     ap.add_argument("--nsamp", type=int, default=0,
                     help="shorten the observation (profiling runs under ncu only; not a bench line)")
+    ap.add_argument("--microbench", action="store_true",
+                    help="measure the integer-ALU, shared-memory and host-link rates the rooflines are quoted against "
+                         "(aa_microbench), print them as one JSON line and exit")
     args = ap.parse_args()
     if args.impl == "reference":
         return run_reference(args)
+    if args.microbench:
+        return run_microbench()
 
     import torch
     from paper_2101_00941_b200 import binding as B

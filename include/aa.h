@@ -241,6 +241,20 @@ void aa_destroy(aa_plan *p);
 int  aa_host_alloc(void **p, uint64_t bytes);
 void aa_host_free(void *p);
 
+/* Micro-benchmarks of the units the hot path is bound by ("measure the real IADD3 / DP4A rates and
+ * sustained clock first"); they back the roofline denominators of bench.py and DESIGN.md, they are not on the path.
+ * aa_microbench runs kind 0 <= kind < aa_microbench_count() (aa_microbench_name: "iadd3", "lop3", "imad", "idp2a",
+ * "idp4a", "prmt", "shf", "iadd3+imad", "lds32", "lds64", "lds128", "sts128", "lds32+iadd") as one wave of
+ * ctas_per_sm (1..2) CTAs of 512 threads per SM, `trips` x 256 instructions per thread, and writes to host
+ * pointers (each may be NULL): per_clk_sm = lane-operations per clock per SM for the arithmetic kinds (a full-warp
+ * instruction counts 32), BYTES per clock per SM for the shared-memory kinds (conflict-free accesses), measured with
+ * the SMs' own cycle counters; ms = kernel time (CUDA events); sm_mhz = the clock the run saw.
+ * aa_microbench_link: pinned host <-> device copy of `bytes`, best of `reps`, in GB/s (dir 0 = H2D, 1 = D2H). */
+int aa_microbench_count(void);
+const char *aa_microbench_name(int kind);
+int aa_microbench(int kind, int ctas_per_sm, int trips, double *per_clk_sm, double *ms, double *sm_mhz);
+int aa_microbench_link(uint64_t bytes, int reps, int dir, double *gbs);
+
 const char *aa_strerror(int status);
 /* cudaError_t of the last failing CUDA call in this thread's last aa_* call (0 if none). */
 int aa_last_cuda_error(void);

@@ -25,7 +25,8 @@ CAND_DTYPE = np.dtype([("dm_index", np.uint32), ("t_start", np.uint32),
 EXPORTS = ["aa_plan_arena_bytes", "aa_plan_create", "aa_plan_query", "aa_plan_nout", "aa_plan_delays",
            "aa_plan_dedisp_variant",
            "aa_plan_geometry", "aa_run", "aa_run_staged", "aa_run_resident", "aa_get_stats", "aa_get_timeline", "aa_find_peaks", "aa_destroy", "aa_host_alloc", "aa_host_free",
-           "aa_strerror", "aa_last_cuda_error"]
+           "aa_strerror", "aa_last_cuda_error",
+           "aa_microbench_count", "aa_microbench_name", "aa_microbench", "aa_microbench_link"]
 
 
 class DMRangeC(ctypes.Structure):
@@ -121,6 +122,15 @@ def load_library() -> ctypes.CDLL:
     lib.aa_strerror.argtypes = [ctypes.c_int]
     lib.aa_last_cuda_error.restype = ctypes.c_int
     lib.aa_last_cuda_error.argtypes = []
+    lib.aa_microbench_count.restype = ctypes.c_int
+    lib.aa_microbench_count.argtypes = []
+    lib.aa_microbench_name.restype = ctypes.c_char_p
+    lib.aa_microbench_name.argtypes = [ctypes.c_int]
+    dp = ctypes.POINTER(ctypes.c_double)
+    lib.aa_microbench.restype = ctypes.c_int
+    lib.aa_microbench.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, dp, dp, dp]
+    lib.aa_microbench_link.restype = ctypes.c_int
+    lib.aa_microbench_link.argtypes = [u64, ctypes.c_int, ctypes.c_int, dp]
     _lib = lib
     return lib
 
@@ -148,6 +158,22 @@ def find_peaks(cands: np.ndarray, nthreads: int = 0) -> np.ndarray:
     n = ctypes.c_uint64(0)
     _check(lib, lib.aa_find_peaks(cands.ctypes.data, len(cands), out.ctypes.data, len(out), ctypes.byref(n), int(nthreads)))
     return out[:int(n.value)]
+
+
+def microbench(ctas_per_sm: int = 2, trips: int = 2000, link_bytes: int = 1 << 30) -> dict:
+    """aa_microbench / aa_microbench_link: measured rates of the units the hot path is bound by (per SM and clock),
+    and the pinned host link.  {name: {"per_clk_sm", "ms", "sm_mhz"}} plus "h2d_gbs" / "d2h_gbs"."""
+    lib = load_library()
+    out = {}
+    for k in range(lib.aa_microbench_count()):
+        r, ms, mhz = ctypes.c_double(), ctypes.c_double(), ctypes.c_double()
+        _check(lib, lib.aa_microbench(k, ctas_per_sm, trips, ctypes.byref(r), ctypes.byref(ms), ctypes.byref(mhz)))
+        out[lib.aa_microbench_name(k).decode()] = {"per_clk_sm": r.value, "ms": ms.value, "sm_mhz": mhz.value}
+    for d, name in ((0, "h2d_gbs"), (1, "d2h_gbs")):
+        g = ctypes.c_double()
+        _check(lib, lib.aa_microbench_link(int(link_bytes), 5, d, ctypes.byref(g)))
+        out[name] = g.value
+    return out
 
 
 def plan_geometry(w, *, n_streams: Optional[int] = None, chunk_len: Optional[int] = None) -> dict:
