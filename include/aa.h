@@ -45,7 +45,8 @@ typedef enum {
     AA_DEDISP_SP512 = 2,     /* shared-pattern kernel, 512-sample tiles */
     AA_DEDISP_SP1024 = 3,    /* ... 1024-sample tiles */
     AA_DEDISP_WS512 = 4,     /* warp-specialised shared-pattern kernel, 512-sample tiles */
-    AA_DEDISP_WS1024 = 5     /* ... 1024-sample tiles */
+    AA_DEDISP_WS1024 = 5,    /* ... 1024-sample tiles */
+    AA_DEDISP_G8 = 6         /* 8-channel shared-pattern kernel (uint8 input only): measured slower, never chosen by AUTO */
 } aa_dedisp_choice;
 
 /* One DM range of the plan: DM_i = dm_low + i*dm_step (double), i = 0..ndms-1, searched on
@@ -162,6 +163,28 @@ uint64_t aa_plan_arena_bytes(const aa_plan_desc *d);
  * creating it: no CUDA call, usable on a host without a GPU (e.g. to split an observation over ranks). */
 int aa_plan_geometry(const aa_plan_desc *d, aa_plan_info *out);
 
+/* Host-side cost model of the shared-pattern dedispersion kernels for range `range` of the plan `d` would build, from
+ * its real delay table (no CUDA call): shared-memory wavefronts (128 bytes) per CTA = per (64 trials x tile_samples)
+ * output tile, as the kernel issues them, the number of distinct delay patterns per stage, and the shared-memory
+ * room the pattern rows take.  group_channels 4 = dedisp_ws_kernel (4 channels x 64 trials per stage), 8 =
+ * dedisp_g8_kernel (8 channels x 32 trials per stage).  AA_ERR_INVALID if the range does not fit that kernel.
+ * Backs profiles/r2_cost_model.md; the binding shared-memory roofline of bench.py uses wf_* of the kernel that runs. */
+typedef struct {
+    int32_t  group_channels, block_trials, tile_samples, stages_per_cta;
+    double   wf_consumer;          /* row-word loads of the consumer warps */
+    double   wf_producer_load;     /* channel-window loads of the producer warps */
+    double   wf_producer_store;    /* pattern-row stores (both alignments) */
+    double   wf_bulk;              /* bytes landed by cp.async.bulk / 128 */
+    double   patterns_mean;
+    int32_t  patterns_max;
+    int32_t  pad;
+    double   stage_bytes_mean;
+    uint64_t stage_bytes_max;
+    uint64_t ring_bytes;           /* shared memory left for the ring of pattern rows */
+    double   shared_offset_fraction; /* consecutive trials of a consumer warp that read the very same row words */
+} aa_dedisp_model;
+int aa_plan_dedisp_model(const aa_plan_desc *d, int32_t range, int32_t group_channels, aa_dedisp_model *out);
+
 /* Allocation phase (PAPER.md:19 part 2, :41 steps 1-2, :71): validates the descriptor, builds
  * the delay tables in double (north_star formula), creates streams and events, allocates the
  * device ring, per-stream work buffers, candidate lists and pinned staging.  Nothing is
@@ -180,7 +203,7 @@ int aa_plan_delays(const aa_plan *p, int32_t r, int32_t *out);
 /* Which dedispersion kernel the plan chose for range r (the choice depends only on the delay table):
  * 0 = plain tiled kernel, 1 / 2 = shared-pattern kernel with 512 / 1024-sample tiles, 3 / 4 =
  * warp-specialised shared-pattern kernel with 512 / 1024-sample tiles, 5 = the same with 32-bit accumulators
- * (coarse time bins); AA_ERR_INVALID if r is out
+ * (coarse time bins), 6 = 8-channel shared-pattern kernel; AA_ERR_INVALID if r is out
  * of range.  Used by tests to make sure every kernel is covered. */
 int aa_plan_dedisp_variant(const aa_plan *p, int32_t r);
 

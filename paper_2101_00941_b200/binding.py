@@ -17,7 +17,7 @@ LIB_PATH = os.path.join(_HERE, "libaa.so")
 
 AA_OK, AA_ERR_INVALID, AA_ERR_NOT_PINNED, AA_ERR_OOM, AA_ERR_CUDA, AA_ERR_OVERFLOW = 0, -1, -2, -3, -4, -5
 #: aa_dedisp_choice (aa_plan_desc.dedisp_variant)
-DEDISP_CHOICE = {"auto": 0, "plain": 1, "sp512": 2, "sp1024": 3, "ws512": 4, "ws1024": 5}
+DEDISP_CHOICE = {"auto": 0, "plain": 1, "sp512": 2, "sp1024": 3, "ws512": 4, "ws1024": 5, "g8": 6}
 
 CAND_DTYPE = np.dtype([("dm_index", np.uint32), ("t_start", np.uint32),
                        ("width", np.uint32), ("snr", np.float32)])
@@ -26,7 +26,7 @@ EXPORTS = ["aa_plan_arena_bytes", "aa_plan_create", "aa_plan_query", "aa_plan_no
            "aa_plan_dedisp_variant",
            "aa_plan_geometry", "aa_run", "aa_run_staged", "aa_run_resident", "aa_get_stats", "aa_get_timeline", "aa_find_peaks", "aa_destroy", "aa_host_alloc", "aa_host_free",
            "aa_strerror", "aa_last_cuda_error",
-           "aa_microbench_count", "aa_microbench_name", "aa_microbench", "aa_microbench_link"]
+           "aa_plan_dedisp_model", "aa_microbench_count", "aa_microbench_name", "aa_microbench", "aa_microbench_link"]
 
 
 class DMRangeC(ctypes.Structure):
@@ -52,6 +52,15 @@ class PlanInfoC(ctypes.Structure):
     _fields_ = [(n, ctypes.c_uint64) for n in
                 ("maxshift", "t_valid", "halo", "subchunk_len", "n_subchunks", "ndms_total",
                  "dm_trial_samples", "arena_bytes", "pinned_bytes", "tap_row_len")]
+
+
+class DedispModelC(ctypes.Structure):
+    _fields_ = [("group_channels", ctypes.c_int32), ("block_trials", ctypes.c_int32), ("tile_samples", ctypes.c_int32),
+                ("stages_per_cta", ctypes.c_int32), ("wf_consumer", ctypes.c_double), ("wf_producer_load", ctypes.c_double),
+                ("wf_producer_store", ctypes.c_double), ("wf_bulk", ctypes.c_double), ("patterns_mean", ctypes.c_double),
+                ("patterns_max", ctypes.c_int32), ("pad", ctypes.c_int32), ("stage_bytes_mean", ctypes.c_double),
+                ("stage_bytes_max", ctypes.c_uint64), ("ring_bytes", ctypes.c_uint64),
+                ("shared_offset_fraction", ctypes.c_double)]
 
 
 class StatsC(ctypes.Structure):
@@ -110,6 +119,8 @@ def load_library() -> ctypes.CDLL:
     lib.aa_destroy.argtypes = [vp]
     lib.aa_plan_geometry.restype = ctypes.c_int
     lib.aa_plan_geometry.argtypes = [ctypes.POINTER(PlanDescC), ctypes.POINTER(PlanInfoC)]
+    lib.aa_plan_dedisp_model.restype = ctypes.c_int
+    lib.aa_plan_dedisp_model.argtypes = [ctypes.POINTER(PlanDescC), i32, i32, ctypes.POINTER(DedispModelC)]
     lib.aa_find_peaks.restype = ctypes.c_int
     lib.aa_find_peaks.argtypes = [vp, u64, vp, u64, ctypes.POINTER(u64), ctypes.c_int32]
     lib.aa_get_timeline.restype = ctypes.c_int
@@ -174,6 +185,33 @@ def microbench(ctas_per_sm: int = 2, trips: int = 2000, link_bytes: int = 1 << 3
         _check(lib, lib.aa_microbench_link(int(link_bytes), 5, d, ctypes.byref(g)))
         out[name] = g.value
     return out
+
+
+def _desc_for(w, n_streams=None, chunk_len=None):
+    ranges = (DMRangeC * len(w.ranges))(*[DMRangeC(r.dm_low, r.dm_step, r.ndms, r.bin) for r in w.ranges])
+    widths = (ctypes.c_int32 * len(w.widths))(*w.widths)
+    d = PlanDescC()
+    d.nchans, d.nsamp, d.tsamp, d.f_top, d.foff = w.nchans, w.nsamp, w.tsamp, w.f_top, w.foff
+    d.nranges, d.ranges, d.nwidths, d.widths = len(w.ranges), ranges, len(w.widths), widths
+    d.snr_threshold = float(w.snr_threshold)
+    d.n_streams = int(n_streams if n_streams is not None else w.n_streams)
+    d.chunk_len = int(chunk_len if chunk_len is not None else w.chunk_len)
+    d.norm_block = int(getattr(w, "norm_block", 65536))
+    d._keep = (ranges, widths)
+    return d
+
+
+def dedisp_model(w, r: int, group_channels: int = 4):
+    """aa_plan_dedisp_model for range r of workload w: dict of the model's fields, or None if the range does not fit
+    that kernel family (no GPU needed)."""
+    lib = load_library()
+    d = _desc_for(w)
+    m = DedispModelC()
+    rc = lib.aa_plan_dedisp_model(ctypes.byref(d), int(r), int(group_channels), ctypes.byref(m))
+    if rc == AA_ERR_INVALID:
+        return None
+    _check(lib, rc)
+    return {n: getattr(m, n) for n, _ in DedispModelC._fields_ if n != "pad"}
 
 
 def plan_geometry(w, *, n_streams: Optional[int] = None, chunk_len: Optional[int] = None) -> dict:
@@ -253,7 +291,7 @@ class Plan:
 
     def dedisp_variant(self, r: int) -> int:
         """0 plain, 1/2 shared-pattern 512/1024, 3/4 warp-specialised shared-pattern 512/1024, 5 the latter with
-        32-bit accumulators (coarse time bins)."""
+        32-bit accumulators (coarse time bins), 6 the 8-channel shared-pattern kernel."""
         v = self.lib.aa_plan_dedisp_variant(self.handle, r)
         if v < 0:
             _check(self.lib, v)

@@ -36,3 +36,23 @@ def test_report_modules_refuse_to_run_without_cuda():
         sweep.main(["--workload", "1", "--streams", "1"])
     with pytest.raises(SystemExit):
         T.main(["--workload", "1"])
+
+
+def test_dedispersion_cost_model_on_the_headline_workload():
+    """aa_plan_dedisp_model (no GPU): the consumer term is the definition (one 32-bit row word per trial, group and
+    sample pair), the pattern counts are those of the delay table, and the 8-channel variant halves the consumer term."""
+    import numpy as np
+    import oracle
+    from paper_2101_00941_b200 import binding as B, inputs as I
+    w = I.workload(3)
+    m4, m8 = B.dedisp_model(w, 0, 4), B.dedisp_model(w, 0, 8)
+    assert m4["stages_per_cta"] == w.nchans // 4 and m8["stages_per_cta"] == 2 * (w.nchans // 8)
+    assert m4["wf_consumer"] == 64 * 1024 * 2 / 128 * (w.nchans // 4)
+    assert m8["wf_consumer"] == m4["wf_consumer"] / 2
+    # distinct relative-delay vectors of one (64 trials, 4 channels) block, counted from the oracle's delay table
+    dl = oracle.delays(w, 0)
+    blk = dl[:64, 2000:2004] - dl[:64, 2000:2001]
+    assert 1 <= len(np.unique(blk, axis=0)) <= m4["patterns_max"] <= 8
+    assert 4.0 < m4["patterns_mean"] < 5.5 and m8["patterns_mean"] > m4["patterns_mean"]
+    assert m4["stage_bytes_max"] <= m4["ring_bytes"] and 0.0 <= m4["shared_offset_fraction"] < 0.1
+    assert B.dedisp_model(I.workload(4), 1, 8) is None          # the 8-channel kernel takes uint8 input only
