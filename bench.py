@@ -38,8 +38,9 @@ sys.path.insert(0, ROOT)
 
 from paper_2101_00941_b200 import inputs as I  # noqa: E402
 
-METRIC = "end-to-end DM-trial*samples/s"
+METRIC = "end-to-end DM-trial*samples/s incl. H2D/D2H; real-time factor; overlap %"
 UNIT = "DM-trial*samples/s"
+N_SM = 148
 
 
 def peaks():
@@ -51,23 +52,22 @@ def peaks():
     return {"hbm_gbs": 6650.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
 
 
-def ncu_counters(kernel_name):
-    """Per-launch counters of the dominant kernel from the committed `ncu --set full` summary of this round
-    (profiles/r1_dedisp_ws_ncu.txt, same launch shape as the bench): (dram bytes read + written, shared-memory
-    wavefronts); (None, None) if there is no summary for this kernel."""
-    path = os.path.join(ROOT, "profiles", "r1_dedisp_ws_ncu.txt")
-    if not kernel_name.startswith("dedisp_ws_kernel<1024>") or not os.path.exists(path):
-        return None, None
-    tot, wf = 0.0, None
-    scale = {"Gbyte": 1e9, "Mbyte": 1e6, "Kbyte": 1e3, "byte": 1.0}
+def ncu_profile(kernel_name):
+    """Per-launch counters of the dominant kernel from this round's committed `ncu --set full` summary
+    (profiles/r2_dedisp_ws_ncu.json, written by `python -m paper_2101_00941_b200.profile_meta`).  The summary names the
+    kernel and the sha256 of the kernel sources it was taken from; if either differs from what runs now the counters
+    are stale and (None, reason) is returned."""
+    from paper_2101_00941_b200 import profile_meta
+    path = os.path.join(ROOT, "profiles", "r2_dedisp_ws_ncu.json")
+    if not os.path.exists(path):
+        return None, "no ncu summary committed for this kernel"
     with open(path) as f:
-        for line in f:
-            c = [x.strip() for x in line.split("|")]
-            if len(c) == 3 and c[0] in ("dram__bytes_read.sum", "dram__bytes_write.sum") and c[1] in scale:
-                tot += float(c[2]) * scale[c[1]]
-            if len(c) == 3 and c[0] == "l1tex__data_pipe_lsu_wavefronts_mem_shared.sum":
-                wf = float(c[2])
-    return (tot or None), wf
+        p = json.load(f)
+    if p.get("kernel") != kernel_name:
+        return None, f"summary is for {p.get('kernel')}, the bench ran {kernel_name}"
+    if p.get("source_sha256") != profile_meta.kernel_source_hash():
+        return None, "kernel sources changed since the summary was taken"
+    return p, f"profiles/r2_dedisp_ws_ncu.json (sources {p['source_sha256'][:12]})"
 
 
 class ClockSampler:
@@ -155,15 +155,16 @@ def cpu_baseline(w, x, budget_rows=48, budget_blocks=8):
     nblocks = int(max(1, min(budget_blocks, have // L, geo["nout"][r] // L)))
     nemit = min(nblocks * L, geo["nout"][r])
     ntau = min(nemit + max(w.widths) - 1, geo["nout"][r])
+    from concurrent.futures import ThreadPoolExecutor
+    cores = oracle.num_threads()
     t0 = time.perf_counter()
-    D = oracle.dedisperse(x, w, r, rows=rows, tau_first=0, ntau=ntau, geo=geo)
-    ncand = 0
-    for k in range(len(rows)):
-        tau, _, _ = oracle.sps_row(D[k], w, r, d_first=0, tau_a=0, tau_b=nemit, nout=geo["nout"][r])
-        ncand += len(tau)
+    D = oracle.dedisperse(x, w, r, rows=rows, tau_first=0, ntau=ntau, geo=geo)         # OpenMP over DM rows
+    with ThreadPoolExecutor(max_workers=cores) as ex:                                  # one DM row per host thread
+        ncand = sum(ex.map(lambda k: len(oracle.sps_row(D[k], w, r, d_first=0, tau_a=0, tau_b=nemit, nout=geo["nout"][r])[0]),
+                           range(len(rows))))
     dt = time.perf_counter() - t0
     units = len(rows) * nemit
-    return {"value": units / dt, "unit": UNIT, "cores": oracle.num_threads(), "kind": "oracle",
+    return {"value": units / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
             "sample": f"{len(rows)} DM trials x {nemit} output samples ({nblocks} normalisation blocks) "
                       f"of {w.name}, dedispersion + SPS, {dt:.1f} s", "seconds": dt}
 
@@ -217,6 +218,90 @@ def run_microbench():
     return 0
 
 
+def _timed(fn, plan_stats, steps, warmup, barrier, dist_util):
+    """W untimed then exactly K timed calls, barrier + synchronize on both sides, CUDA events and wall clock, max over ranks."""
+    import torch
+    for _ in range(warmup):
+        fn()
+    barrier()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    t0 = time.perf_counter()
+    acc = []
+    for _ in range(steps):
+        fn()
+        acc.append(plan_stats())
+    e1.record()
+    barrier()
+    wall = time.perf_counter() - t0
+    dev = e0.elapsed_time(e1) / 1e3
+    return dist_util.max_over_ranks(max(wall, dev)), acc
+
+
+def run_config(B, k, steps, warmup, link_gbs, max_cands=1 << 24):
+    """One more BASELINE.json config end to end through aa_run (pinned host buffer, the workload's stream count):
+    the `per_config` entries of the bench line.  Own pinned buffer, released before returning."""
+    import hashlib
+    import torch
+    w = I.workload(k)
+    t0 = time.perf_counter()
+    host = B.pinned_empty(w.nbytes)
+    t_pin = time.perf_counter() - t0
+    I.fill(w, host.numpy().reshape(w.nsamp, w.nchans))
+    out = {"workload": w.name, "n_streams": w.n_streams, "pin_s": t_pin}
+    L = w.chunk_len // w.n_streams
+    last = {}
+
+    def leg(plan, fn, nsteps):
+        for _ in range(warmup):
+            fn()
+        torch.cuda.synchronize()
+        ts, sts = [], []
+        for _ in range(nsteps):
+            a = time.perf_counter()
+            fn()
+            torch.cuda.synchronize()
+            ts.append(time.perf_counter() - a)
+            sts.append(plan.stats())
+        return sum(ts) / len(ts), sts[-1]
+
+    with B.Plan(w) as plan:
+        def step():
+            last["c"], _ = plan.run(host, max_cands=max_cands, want_taps=False)
+        step_s, st = leg(plan, step, steps)
+        units = plan.info["dm_trial_samples"]
+        variants = [plan.dedisp_variant(r) for r in range(len(w.ranges))]
+    # the two things the end-to-end run overlaps, each alone: the copy of the observation, and the kernels on resident data
+    dev_in = torch.empty(w.nbytes, dtype=torch.uint8, device="cuda")
+    torch.cuda.synchronize()
+    a = time.perf_counter()
+    dev_in.copy_(host, non_blocking=True)
+    torch.cuda.synchronize()
+    xfer_s = time.perf_counter() - a
+    with B.Plan(w, n_streams=1, chunk_len=L) as plan:
+        def step_res():
+            last["r"], _ = plan.run_resident(dev_in, max_cands=max_cands, want_taps=False)
+        kern_s, st_res = leg(plan, step_res, max(1, steps - 1))
+    del dev_in
+    c = last["c"]
+    if len(last["r"]) != len(c):
+        raise RuntimeError(f"resident leg found {len(last['r'])} candidates, end-to-end leg {len(c)}")
+    out.update({
+        "steps": steps, "ms_per_step": 1e3 * step_s,
+        "e2e": {"value": units / step_s, "unit": UNIT, "h2d_bytes_per_step": st["h2d_bytes"], "d2h_bytes_per_step": st["d2h_bytes"]},
+        "real_time_factor": w.nsamp * w.tsamp / step_s,
+        "transfer_alone_s": xfer_s, "kernels_alone_s": kern_s,
+        "overlap_efficiency": max(kern_s, xfer_s) / step_s,
+        # resident leg, one stream: kernel durations from CUDA events on the launching stream, host sort inside the wall time
+        "breakdown_ms": {"dedisp": st_res["dedisp_ms"], "sps": st_res["sps_ms"], "prep": st_res["prep_ms"],
+                         "d2h": st_res["d2h_ms"], "sort": st_res["sort_ms"], "wall": st_res["wall_ms"]},
+        "dedisp_variant": variants,
+        "candidates": int(len(c)), "candidates_sha256": hashlib.sha256(c.tobytes()).hexdigest()[:16],
+    })
+    del host
+    return out
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -228,6 +313,9 @@ def main():
     ap.add_argument("--ref-rows", type=int, default=48, help="DM trials of the oracle sample")
     ap.add_argument("--ref-blocks", type=int, default=8, help="normalisation blocks of the oracle sample")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--per-config", default="auto",
+                    help="comma-separated other configs to run end to end after the main workload (3 steps each) and "
+                         "report under per_config; 'auto' = 2,4,5 for the default single-GPU run of workload 3, 'none' = skip")
     ap.add_argument("--shard-observation", action="store_true",
                     help="strong scaling: ONE observation split by time over the ranks (whole normalisation blocks + halo "
                          "per rank, candidate lists gathered on rank 0); default: one observation per rank (weak)")
@@ -250,6 +338,8 @@ def main():
         raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
     torch.cuda.set_device(local)
     from paper_2101_00941_b200 import dist_util
+    placement = dist_util.place_rank(local, world)          # NUMA node of the GPU: host threads and first touch
+    print(f"[bench] rank {rank}/{world} gpu {local}: {placement}", file=sys.stderr)
     dist_util.init("nccl", device=torch.device("cuda", local))
     B.load_library()
 
@@ -270,6 +360,9 @@ def main():
     else:
         w = dist_util.rank_workload(w, rank)
 
+    # the measured denominators of this run: shared-memory and integer rates per clock and SM, pinned link GB/s
+    mb = B.microbench(trips=500, link_bytes=1 << 28)
+
     t_gen0 = time.perf_counter()
     host = B.pinned_empty(w.nbytes)
     t_pin = time.perf_counter() - t_gen0
@@ -284,30 +377,11 @@ def main():
         dist_util.barrier()
         torch.cuda.synchronize()
 
-    def timed(fn, steps, warmup):
-        for _ in range(warmup):
-            fn()
-        barrier()
-        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-        e0.record()
-        t0 = time.perf_counter()
-        acc = []
-        for _ in range(steps):
-            fn()
-            acc.append(plan_stats())
-        e1.record()
-        barrier()
-        wall = time.perf_counter() - t0
-        dev = e0.elapsed_time(e1) / 1e3
-        t = dist_util.max_over_ranks(max(wall, dev))
-        return t, acc
-
     max_cands = 1 << 24
     sampler = ClockSampler(local)
 
     # ---- leg 1: end to end from pinned host memory -------------------------------------------
     plan = B.Plan(w, n_streams=n_streams, chunk_len=L * n_streams)
-    plan_stats = plan.stats
     info = plan.info
     units = info["dm_trial_samples"]
     if shard is not None:
@@ -323,7 +397,7 @@ def main():
         last["c"] = c
 
     sampler.start()
-    t_e2e, st_e2e = timed(step_e2e, args.steps, args.warmup)
+    t_e2e, st_e2e = _timed(step_e2e, plan.stats, args.steps, args.warmup, barrier, dist_util)
     h2d = st_e2e[-1]["h2d_bytes"]; d2h = st_e2e[-1]["d2h_bytes"]
     launches_e2e = sum(s["dedisp_launches"] + s["sps_launches"] + s["prep_launches"] for s in st_e2e)
     n_cands = last["n"]
@@ -344,7 +418,6 @@ def main():
     torch.cuda.synchronize()
     t_copy = time.perf_counter() - tc0                 # the transfers alone
     plan = B.Plan(w, n_streams=1, chunk_len=L)
-    plan_stats = plan.stats
     variant = plan.dedisp_variant(0)
     kernel_name = {0: "dedisp_kernel", 1: "dedisp_sp_kernel<512>", 2: "dedisp_sp_kernel<1024>",
                    3: "dedisp_ws_kernel<512>", 4: "dedisp_ws_kernel<1024>", 5: "dedisp_ws_kernel<512, wide>",
@@ -354,34 +427,65 @@ def main():
         c, _ = plan.run_resident(dev_in, max_cands=max_cands, want_taps=False)
         last["n_res"] = len(c)
 
-    t_res, st_res = timed(step_res, args.steps, args.warmup)
+    t_res, st_res = _timed(step_res, plan.stats, args.steps, args.warmup, barrier, dist_util)
     clocks = sampler.stop()
     plan.close()
     del dev_in
+    if shard is None and last["n_res"] != n_cands:
+        raise SystemExit(f"resident leg found {last['n_res']} candidates, end-to-end leg {n_cands}")
 
     # ---- roofline of the dominant kernel (dedispersion) ---------------------------------------
     pk, pk_src = peaks()
     d_ms = sum(s["dedisp_ms"] for s in st_res); d_n = sum(s["dedisp_launches"] for s in st_res)
     s_ms = sum(s["sps_ms"] for s in st_res); p_ms = sum(s["prep_ms"] for s in st_res)
+    s_n = sum(s["sps_launches"] for s in st_res)
     wall_ms = sum(s["wall_ms"] for s in st_res)
-    adds_per_step = sum(r.ndms * (info["t_valid"] // r.bin) for r in w.ranges) * w.nchans
-    adds_per_launch = adds_per_step * args.steps / max(d_n, 1)
     avg_launch_s = d_ms / 1e3 / max(d_n, 1)
-    achieved = adds_per_launch / avg_launch_s / 1e12              # T adds/s
-    sm_mhz = pk.get("sm_max_mhz", 1965.0)
-    peak = 148 * 128 * sm_mhz * 1e6 / 1e12                        # T lane-ops/s
-    traffic, smem_wf = ncu_counters(kernel_name)
-    roofline = {"kernel": kernel_name, "bound": "alu", "achieved": achieved, "peak": peak,
-                "unit": "T integer adds/s", "frac": achieved / peak, "traffic": traffic,
-                "peak_source": f"148 SMs x 128 lanes x {sm_mhz:.0f} MHz ({pk_src}); one add per lane-op",
-                "avg_launch_ms": avg_launch_s * 1e3, "launches": d_n,
-                "share_of_step": {"dedisp": d_ms / wall_ms, "sps": s_ms / wall_ms, "prep": p_ms / wall_ms}}
-    if smem_wf:
-        # the resource that binds this kernel: one 128-byte shared-memory wavefront per clock per SM
-        roofline["shared_memory_pipe"] = {"wavefronts_per_launch": smem_wf, "peak_per_s": 148 * sm_mhz * 1e6,
-                                          "frac": smem_wf / avg_launch_s / (148 * sm_mhz * 1e6),
-                                          "source": "ncu l1tex__data_pipe_lsu_wavefronts_mem_shared.sum (profiles/r1_dedisp_ws_ncu.txt) "
-                                                    "over the launch time measured here"}
+    sm_mhz = clocks.get("sm_mhz") or pk.get("sm_max_mhz", 1965.0)
+    # (a) the binding resource: shared-memory wavefronts the kernel issues by design (aa_plan_dedisp_model over the
+    #     plan's real tables) per launch, against the LDS rate measured in this run x the SM clock sampled in this run
+    model = B.dedisp_model(w, 0, 4) if variant in (3, 4, 5) and len(w.ranges) == 1 else None
+    nblk = -(-w.ranges[0].ndms // 64)
+    ncols = L // w.ranges[0].bin + max(w.widths) - 1
+    if model:
+        wf_cta = model["wf_consumer"] + model["wf_producer_load"] + model["wf_producer_store"] + model["wf_bulk"]
+        wf_launch = wf_cta * nblk * -(-ncols // model["tile_samples"])
+        lds_b_clk = mb["lds32"]["per_clk_sm"]
+        peak_gbs = N_SM * lds_b_clk * sm_mhz * 1e6 / 1e9
+        achieved_gbs = wf_launch * 128 / avg_launch_s / 1e9
+        prof, prof_src = ncu_profile(kernel_name)
+        roofline = {"kernel": kernel_name, "bound": "smem", "achieved": achieved_gbs, "peak": peak_gbs,
+                    "unit": "GB/s through shared memory (128-byte wavefronts)", "frac": achieved_gbs / peak_gbs,
+                    "traffic": prof["dram_bytes_per_launch"] if prof else None, "traffic_source": prof_src,
+                    "peak_source": f"measured in this run: {lds_b_clk:.1f} B/clk/SM (aa_microbench lds32) x {N_SM} SMs x "
+                                   f"{sm_mhz:.0f} MHz (median SM clock sampled during the timed region)",
+                    "algorithmic": {"wavefronts_per_launch": wf_launch, "per_cta": wf_cta,
+                                    "source": "aa_plan_dedisp_model over the plan's tables: consumer row loads + producer window "
+                                              "loads + pattern-row stores + bulk-copy landings (profiles/r2_cost_model.md)"},
+                    "avg_launch_ms": avg_launch_s * 1e3, "launches": d_n}
+        if prof:
+            roofline["ncu_wavefronts_per_launch"] = prof["smem_wavefronts_per_launch"]
+    else:
+        roofline = {"kernel": kernel_name, "bound": "alu", "achieved": None, "peak": None, "unit": "T integer adds/s", "frac": None,
+                    "traffic": None, "avg_launch_ms": avg_launch_s * 1e3, "launches": d_n}
+    # (b) the algorithmic integer work (nchans adds per DM-trial*sample) against the measured integer rate:
+    #     a work rate, not a utilisation -- the shared-pattern scheme performs about a quarter of these adds
+    adds_per_step = sum(r.ndms * (info["t_valid"] // r.bin) for r in w.ranges) * w.nchans
+    adds_rate = adds_per_step * args.steps / max(d_n, 1) / avg_launch_s / 1e12
+    lane_clk = mb["iadd3"]["per_clk_sm"] + mb["imad"]["per_clk_sm"]
+    alu_peak = N_SM * lane_clk * sm_mhz * 1e6 / 1e12
+    roofline["alu"] = {"achieved": adds_rate, "peak": alu_peak, "unit": "T integer adds/s", "frac": adds_rate / alu_peak,
+                       "peak_source": f"measured in this run: {mb['iadd3']['per_clk_sm']:.1f} (ALU pipe) + {mb['imad']['per_clk_sm']:.1f} "
+                                      f"(FMA pipe) lane-ops/clk/SM x {N_SM} SMs x {sm_mhz:.0f} MHz",
+                       "note": "algorithmic adds (nchans per unit) over time: above 1 is possible because shared pattern rows "
+                               "replace four channel adds by one; the binding resource is shared memory (frac above)"}
+    if roofline.get("frac") is None:
+        roofline.update({"achieved": adds_rate, "peak": alu_peak, "frac": adds_rate / alu_peak})
+    roofline["share_of_step"] = {"dedisp": d_ms / wall_ms, "sps": s_ms / wall_ms, "prep": p_ms / wall_ms}
+    # (c) the single-pulse-search kernel: HBM-bound by bytes (4 B read per DM-trial*sample)
+    sps_gbs = 4.0 * units * args.steps / (s_ms / 1e3) / 1e9 if s_ms > 0 else 0.0
+    roofline["sps_kernel"] = {"bound": "hbm", "achieved": sps_gbs, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": sps_gbs / pk["hbm_gbs"],
+                              "avg_launch_ms": s_ms / max(s_n, 1), "peak_source": pk_src}
 
     if rank == 0:
         value = world * units * args.steps / t_res
@@ -392,6 +496,8 @@ def main():
             "warmup": args.warmup, "ms_per_step": 1e3 * t_res / args.steps, "higher_is_better": True,
             "scaling": "strong" if shard is not None else "weak", "vs_baseline": None,
             "dtype": "u8 input, u32 exact sums, f64 S/N", "data": "synthetic",
+            "legs": {"value": "observation resident in HBM, 1 stream (aa_run_resident): kernels + D2H of candidates + host merge",
+                     "e2e": f"aa_run on the pinned host buffer, {n_streams} streams: H2D and D2H inside the timed region (the headline)"},
             "config": {"workload": w.name, "nchans": w.nchans, "nsamp": w.nsamp, "ndms": w.ndms_total,
                        "widths": list(w.widths), "n_streams_e2e": n_streams, "subchunk_len": L,
                        "chunk_len_e2e": L * n_streams, "l2": "inputs (34 GB) >> L2; no flush needed",
@@ -401,15 +507,30 @@ def main():
                     "real_time_factor": w.nsamp * w.tsamp / step_s,
                     "h2d_gbs_effective": h2d / step_s / 1e9,
                     "transfer_alone_s": t_copy, "kernels_alone_s": t_res / args.steps,
-                    "overlap_efficiency": max(t_copy, t_res / args.steps) / step_s},
+                    "overlap_efficiency": max(t_copy, t_res / args.steps) / step_s,
+                    "link": {"h2d_gbs": mb["h2d_gbs"], "d2h_gbs": mb["d2h_gbs"], "source": "aa_microbench_link, pinned, this run"}},
             "gpu_launches": int(launches_e2e),
             "candidates": n_cands, "peaks": peak_info, "clocks": clocks, "roofline": roofline,
-            "setup": {"pin_s": t_pin, "generate_s": t_gen},
+            "microbench": {k: (v["per_clk_sm"] if isinstance(v, dict) else v) for k, v in mb.items()},
+            "setup": {"pin_s": t_pin, "generate_s": t_gen, "placement": placement},
         }
         if not args.no_cpu_baseline:
             cb = cpu_baseline(w, x, budget_rows=args.ref_rows, budget_blocks=args.ref_blocks)
             cb.pop("seconds", None)
             line["cpu_baseline"] = cb
+    del host, x
+    # ---- the other configs of BASELINE.json, end to end (north_star: "the 4096-channel configs") ----
+    pcs = args.per_config
+    if pcs == "auto":
+        pcs = "2,4,5" if (world == 1 and args.workload == 3 and not args.nsamp and not args.shard_observation) else "none"
+    if rank == 0 and pcs != "none":
+        line["per_config"] = {}
+        for k in [int(v) for v in pcs.split(",") if v]:
+            try:
+                line["per_config"][f"cfg{k}"] = run_config(B, k, 3, 1, mb["h2d_gbs"])
+            except Exception as e:                      # e.g. not enough host memory to pin 68.7 GB
+                line["per_config"][f"cfg{k}"] = {"error": f"{type(e).__name__}: {e}"}
+    if rank == 0:
         print(json.dumps(line))
     dist_util.shutdown()
     return 0

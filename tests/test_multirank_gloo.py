@@ -54,14 +54,14 @@ def test_single_process_helpers_are_noops():
 
 
 # ---- one observation sharded by time over the ranks -----------------------------------------
-def _shard_setup():
+def _shard_setup(norm_block=2048):
     import math
     from paper_2101_00941_b200 import inputs as I
     import oracle
     w = I.scaled(I.workload(1), nsamp=30000, name="shardme",
                  pulses=(I.Pulse(dm=50.0, t0=7000, width=8, amp=3.0), I.Pulse(dm=90.0, t0=16380, width=16, amp=2.5),
                          I.Pulse(dm=20.0, t0=24500, width=4, amp=4.0)))
-    w = I.scaled(w, norm_block=2048)
+    w = I.scaled(w, norm_block=norm_block)
     x = I.fill(w)
     geo = oracle.geometry(w)
     bmax = max(r.bin for r in w.ranges)
@@ -86,36 +86,64 @@ def test_time_shards_partition_the_valid_span():
         assert pos == nsamp - maxshift                               # the kept spans tile [0, t_valid)
 
 
-def _shard_worker(rank, world, port, q):
+def _shard_worker(rank, world, port, q, norm_block=2048):
     os.environ.update(RANK=str(rank), WORLD_SIZE=str(world), LOCAL_RANK=str(rank),
                       MASTER_ADDR="127.0.0.1", MASTER_PORT=str(port))
     from paper_2101_00941_b200 import dist_util
     import oracle
     assert dist_util.init("gloo")
-    w, x, geo, tail = _shard_setup()
+    w, x, geo, tail = _shard_setup(norm_block)
     shard = dist_util.time_shards(w.nsamp, geo["maxshift"], w.norm_block, tail, world)[rank]
-    ws = dist_util.shard_workload(w, shard)
-    # each rank searches only its own span -- here through the oracle (CPU box); on GPUs through aa_run
-    cands, _ = oracle.run(np.ascontiguousarray(x[shard.t_first:shard.t_first + shard.nsamp]), ws)
+    if shard.nsamp == 0:
+        cands = np.empty(0, dtype=oracle.CAND_DTYPE)         # more ranks than normalisation blocks: nothing to search
+    else:
+        ws = dist_util.shard_workload(w, shard)
+        # each rank searches only its own span -- here through the oracle (CPU box); on GPUs through aa_run
+        cands, _ = oracle.run(np.ascontiguousarray(x[shard.t_first:shard.t_first + shard.nsamp]), ws)
     merged = dist_util.merge_shards(cands, shard)
     q.put((rank, None if merged is None else merged.tobytes()))
     dist_util.shutdown()
 
 
-def test_time_sharded_observation_equals_the_whole_gloo():
+import pytest
+
+
+@pytest.mark.parametrize("world,norm_block", [(2, 2048), (3, 16384)])     # 3 ranks for 2 blocks: the last shard is empty
+def test_time_sharded_observation_equals_the_whole_gloo(world, norm_block):
     import oracle
-    w, x, geo, tail = _shard_setup()
+    from paper_2101_00941_b200 import dist_util
+    w, x, geo, tail = _shard_setup(norm_block)
     whole, _ = oracle.run(x, w)
     assert len(whole) > 100
+    shards = dist_util.time_shards(w.nsamp, geo["maxshift"], w.norm_block, tail, world)
+    assert (shards[-1].nsamp == 0) == (world == 3)
     ctx = mp.get_context("spawn")
     q = ctx.Queue()
     port = _free_port()
-    ps = [ctx.Process(target=_shard_worker, args=(r, 2, port, q)) for r in range(2)]
+    ps = [ctx.Process(target=_shard_worker, args=(r, world, port, q, norm_block)) for r in range(world)]
     for p in ps:
         p.start()
     out = dict(q.get(timeout=180) for _ in ps)
     for p in ps:
         p.join(timeout=60)
         assert p.exitcode == 0
-    assert out[1] is None
+    assert all(out[r] is None for r in range(1, world))
     assert out[0] == whole.tobytes()          # bit-identical candidate list, S/N included
+
+
+def test_rank_placement_splits_the_cores_of_a_numa_node():
+    """dist_util.rank_cpus: 8 ranks on a 2-node, 64-core host get 8 cores each, inside their GPU's node, disjoint
+    among the ranks of a node; one rank alone keeps its whole node; unknown topology splits the allowed cores."""
+    from paper_2101_00941_b200 import dist_util as D
+    allowed = list(range(64))
+    nodes = [list(range(0, 32)), list(range(32, 64))]
+    got = [D.rank_cpus(r, 8, nodes[r // 4], allowed) for r in range(8)]
+    assert all(len(g) == 8 and set(g) <= set(nodes[r // 4]) for r, g in enumerate(got))
+    assert len(set(c for g in got for c in g)) == 64
+    assert D.rank_cpus(0, 1, nodes[1], allowed) == nodes[1]
+    two = [D.rank_cpus(r, 2, None, list(range(16))) for r in range(2)]
+    assert sorted(two[0] + two[1]) == list(range(16))
+    assert D._parse_cpulist("0-3,8,10-11\n") == [0, 1, 2, 3, 8, 10, 11]
+    info = D.place_rank(0, 1)                 # best effort on whatever host runs the tests; never raises
+    assert "cpus" in info
+
