@@ -9,6 +9,7 @@
 #include <algorithm>
 #include <atomic>
 #include <chrono>
+#include <condition_variable>
 #include <cmath>
 #include <cstdio>
 #include <cstdlib>
@@ -81,6 +82,8 @@ struct Stream {
     uint32_t *h_tap = nullptr;        // pinned
     uint8_t *h_stage = nullptr;       // pinned input staging (aa_run_staged), (L + halo) * nchans bytes
     std::vector<cudaEvent_t> ev;      // timing events
+    struct TapCopy { int row; uint64_t tau0, n, off; };
+    std::vector<TapCopy> tapcopies;   // capacity = ntap, reserved at plan creation; refilled per sub-chunk
     // per-run accumulators
     double h2d_ms = 0, d2h_ms = 0, prep_ms = 0, dedisp_ms = 0, sps_ms = 0, h2h_ms = 0;
     uint64_t h2d_bytes = 0, d2h_bytes = 0, dedisp_launches = 0, sps_launches = 0, prep_launches = 0, h2h_bytes = 0;
@@ -115,6 +118,41 @@ struct aa_plan {
     aa_stats stats{};
     cudaEvent_t ev_start = nullptr;           // recorded on stream 0 when a run begins: origin of the timeline
     std::vector<aa_subchunk_times> timeline;  // one entry per sub-chunk, written by its stream's thread
+
+    // Host threads are created once, here, and parked between runs (one host thread per stream; SURVEY
+    // 8(b): aa_run allocates nothing and creates nothing).  `workers[s]` serves stream s; `helpers` copy tapped rows.
+    int device = 0;
+    enum class Cmd { none, run, scatter, copyback, quit };
+    struct Job {                              // what the current aa_run call asked for
+        const uint8_t *input = nullptr;
+        int mode = 0;
+        aa_candidate *out = nullptr;
+        uint64_t max_cands = 0;
+        uint32_t *tap_out = nullptr;
+        uint64_t stored = 0;
+    } job;
+    std::vector<std::thread> workers;
+    std::mutex mu;
+    std::condition_variable cv_go, cv_done;
+    Cmd cmd = Cmd::none;
+    uint64_t seq = 0;                         // bumped with every command
+    int pending = 0, nactive = 0;
+    // helper pool for the host-to-host copies of dense planes
+    struct CopyJob { const Stream *S; uint32_t *tap_out; size_t a, b; std::atomic<int> *left; };
+    std::vector<std::thread> helpers;
+    std::mutex hmu;
+    std::condition_variable hcv;
+    std::vector<CopyJob> hq;                  // fixed capacity, reserved at plan creation
+    bool hquit = false;
+    // final ordering without a global sort: every sub-chunk's list is sorted by its stream's thread while the GPU
+    // works on, `run_cnt[j][d]` counts its records per trial, and the runs are interleaved through `scratch`
+    struct Run { uint64_t pos = 0, n = 0; };
+    std::vector<Run> runs;                    // [n_sub]
+    std::vector<uint32_t> run_cnt;            // [n_sub][ndms_total + 1] start offset of trial d inside run j
+    std::vector<uint64_t> dm_dst;             // [ndms_total + 1] first output record of trial d
+    aa_candidate *scratch = nullptr;
+    uint64_t scratch_cap = 0;
+    uint32_t ndms_total = 0;
 };
 
 namespace {
@@ -417,6 +455,24 @@ void carve(aa_plan &p)
 void destroy_plan(aa_plan *p)
 {
     if (!p) return;
+    if (!p->workers.empty()) {
+        {
+            std::lock_guard<std::mutex> lk(p->mu);
+            p->cmd = aa_plan::Cmd::quit;
+            ++p->seq;
+        }
+        p->cv_go.notify_all();
+        for (auto &t : p->workers) t.join();
+    }
+    if (!p->helpers.empty()) {
+        {
+            std::lock_guard<std::mutex> lk(p->hmu);
+            p->hquit = true;
+        }
+        p->hcv.notify_all();
+        for (auto &t : p->helpers) t.join();
+    }
+    std::free(p->scratch);
     for (auto &S : p->streams) {
         if (S.st) cudaStreamSynchronize(S.st);
         for (auto e : S.ev) if (e) cudaEventDestroy(e);
@@ -567,8 +623,8 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
         AA_W(cudaMemsetAsync(S.d_count, 0, sizeof(uint32_t), st));
 
         uint64_t tap_off = 0;
-        struct TapCopy { int row; uint64_t tau0, n, off; };
-        std::vector<TapCopy> tapcopies;
+        auto &tapcopies = S.tapcopies;
+        tapcopies.clear();                         // capacity reserved at plan creation
         for (int ri = 0; ri < nr; ++ri) {
             Range &Rg = p->ranges[ri];
             const uint64_t b = (uint64_t)Rg.r.bin;
@@ -669,34 +725,63 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
         AA_W(cudaStreamSynchronize(st));
         S.d2h_bytes += 4 + n * sizeof(aa_candidate);
 
-        // host-to-host output stage of this stream
+        // host-to-host output stage of this stream: the sub-chunk's list goes to the caller's buffer
+        // and is put in (dm_index, t_start) order right here, while the GPU works on the next sub-chunks
         p->total.fetch_add(found);
         const uint64_t pos = p->out_pos.fetch_add(n);
+        uint64_t m = 0;
         if (pos < max_cands) {
-            const uint64_t m = std::min<uint64_t>(n, max_cands - pos);
-            if (m) std::memcpy(out + pos, S.h_cands, m * sizeof(aa_candidate));
+            m = std::min<uint64_t>(n, max_cands - pos);
+            if (m) {
+                std::memcpy(out + pos, S.h_cands, m * sizeof(aa_candidate));
+                std::sort(out + pos, out + pos + m, [](const aa_candidate &a, const aa_candidate &b) {
+                    return a.dm_index != b.dm_index ? a.dm_index < b.dm_index : a.t_start < b.t_start;
+                });
+            }
+        }
+        {
+            // where each trial starts inside this run
+            p->runs[j].pos = pos < max_cands ? pos : max_cands;
+            p->runs[j].n = m;
+            uint32_t *cnt = &p->run_cnt[j * (uint64_t)(p->ndms_total + 1)];
+            uint64_t i = 0;
+            for (uint32_t d = 0; d <= p->ndms_total; ++d) {
+                while (i < m && out[pos + i].dm_index < d) ++i;
+                cnt[d] = (uint32_t)i;
+            }
         }
         if (tap_out && !tapcopies.empty()) {
             // host-to-host copy of the tapped rows; a dense plane is hundreds of MB per sub-chunk,
-            // so the stream's thread takes helpers when the machine has cores to spare
+            // so the stream's thread shares it with the plan's helper threads (created at plan creation)
             auto copy_rows = [&](size_t a, size_t b) {
                 for (size_t i = a; i < b; ++i) {
-                    const TapCopy &tc = tapcopies[i];
+                    const Stream::TapCopy &tc = tapcopies[i];
                     std::memcpy(tap_out + (uint64_t)tc.row * p->tap_row_len + tc.tau0, S.h_tap + tc.off, tc.n * 4);
                 }
             };
             const uint64_t bytes = tap_off * 4;
-            const unsigned hw = std::max(1u, std::thread::hardware_concurrency());
-            const size_t K = bytes < (64ull << 20) ? 1 : std::min<size_t>(std::max<size_t>(hw / (unsigned)p->n_streams, 1), 4);
+            const size_t K = bytes < (64ull << 20) || p->helpers.empty()
+                                 ? 1 : std::min<size_t>(1 + p->helpers.size() / (size_t)p->nactive, 4);
             if (K == 1) {
                 copy_rows(0, tapcopies.size());
             } else {
-                std::vector<std::thread> helpers;
                 const size_t per = (tapcopies.size() + K - 1) / K;
-                for (size_t k = 1; k < K; ++k)
-                    helpers.emplace_back(copy_rows, std::min(k * per, tapcopies.size()), std::min((k + 1) * per, tapcopies.size()));
+                std::atomic<int> left{0};
+                size_t inline_from = tapcopies.size();      // parts the queue has no room for are copied here
+                {
+                    std::lock_guard<std::mutex> lk(p->hmu);
+                    for (size_t k = 1; k < K; ++k) {
+                        const size_t a = std::min(k * per, tapcopies.size()), b = std::min((k + 1) * per, tapcopies.size());
+                        if (a >= b) break;
+                        if (p->hq.size() == p->hq.capacity()) { inline_from = a; break; }
+                        left.fetch_add(1);
+                        p->hq.push_back({&S, tap_out, a, b, &left});
+                    }
+                }
+                p->hcv.notify_all();
                 copy_rows(0, std::min(per, tapcopies.size()));
-                for (auto &h : helpers) h.join();
+                copy_rows(inline_from, tapcopies.size());
+                while (left.load(std::memory_order_acquire) > 0) std::this_thread::yield();
             }
         }
 
@@ -721,6 +806,88 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
             cudaEventElapsedTime(&ms, S.ev[kEvFixed + 3 * ri], S.ev[kEvFixed + 3 * ri + 1]); T.dedisp_ms += ms;
             cudaEventElapsedTime(&ms, S.ev[kEvFixed + 3 * ri + 1], S.ev[kEvFixed + 3 * ri + 2]); T.sps_ms += ms;
         }
+    }
+}
+
+// Sends one command to every active worker thread and waits until all of them are done with it.
+void command(aa_plan *p, aa_plan::Cmd c)
+{
+    std::unique_lock<std::mutex> lk(p->mu);
+    p->cmd = c;
+    p->pending = p->nactive;
+    ++p->seq;
+    p->cv_go.notify_all();
+    p->cv_done.wait(lk, [&] { return p->pending == 0; });
+}
+
+// Pieces of the final interleave: worker s of nactive takes every nactive-th trial (scatter) / an equal slice (copy back)
+void merge_scatter(aa_plan *p, int s)
+{
+    const uint64_t W = (uint64_t)p->ndms_total + 1;
+    const aa_candidate *out = p->job.out;
+    for (uint32_t d = (uint32_t)s; d < p->ndms_total; d += (uint32_t)p->nactive) {
+        uint64_t dst = p->dm_dst[d];
+        for (uint64_t j = 0; j < p->n_sub; ++j) {
+            const uint32_t a = p->run_cnt[j * W + d], b = p->run_cnt[j * W + d + 1];
+            if (b > a) {
+                std::memcpy(p->scratch + dst, out + p->runs[j].pos + a, (uint64_t)(b - a) * sizeof(aa_candidate));
+                dst += b - a;
+            }
+        }
+    }
+}
+
+void merge_copyback(aa_plan *p, int s)
+{
+    const uint64_t n = p->job.stored, per = (n + (uint64_t)p->nactive - 1) / (uint64_t)p->nactive;
+    const uint64_t a = std::min(n, per * (uint64_t)s), b = std::min(n, a + per);
+    if (b > a) std::memcpy(p->job.out + a, p->scratch + a, (b - a) * sizeof(aa_candidate));
+}
+
+// Body of the persistent host thread of stream s: parked on the condition variable between commands.
+void worker_main(aa_plan *p, int s)
+{
+    cudaSetDevice(p->device);
+    uint64_t seen = 0;
+    for (;;) {
+        aa_plan::Cmd c;
+        {
+            std::unique_lock<std::mutex> lk(p->mu);
+            p->cv_go.wait(lk, [&] { return p->seq != seen; });
+            seen = p->seq;
+            c = p->cmd;
+        }
+        if (c == aa_plan::Cmd::quit) return;
+        if (c == aa_plan::Cmd::run)
+            worker(p, s, p->job.input, (Input)p->job.mode, p->job.out, p->job.max_cands, p->job.tap_out);
+        else if (c == aa_plan::Cmd::scatter)
+            merge_scatter(p, s);
+        else if (c == aa_plan::Cmd::copyback)
+            merge_copyback(p, s);
+        {
+            std::lock_guard<std::mutex> lk(p->mu);
+            if (--p->pending == 0) p->cv_done.notify_all();
+        }
+    }
+}
+
+// Body of a helper thread: host-to-host copies of tapped rows handed over by the stream threads.
+void helper_main(aa_plan *p)
+{
+    for (;;) {
+        aa_plan::CopyJob jb;
+        {
+            std::unique_lock<std::mutex> lk(p->hmu);
+            p->hcv.wait(lk, [&] { return p->hquit || !p->hq.empty(); });
+            if (p->hq.empty()) return;           // quit
+            jb = p->hq.back();
+            p->hq.pop_back();
+        }
+        for (size_t i = jb.a; i < jb.b; ++i) {
+            const Stream::TapCopy &tc = jb.S->tapcopies[i];
+            std::memcpy(jb.tap_out + (uint64_t)tc.row * p->tap_row_len + tc.tau0, jb.S->h_tap + tc.off, tc.n * 4);
+        }
+        jb.left->fetch_sub(1, std::memory_order_release);
     }
 }
 
@@ -751,11 +918,10 @@ int run_impl(aa_plan *p, const uint8_t *input, Input mode, aa_candidate *out, ui
         S.h2d_bytes = S.d2h_bytes = S.dedisp_launches = S.sps_launches = S.prep_launches = S.h2h_bytes = 0;
     }
     if (cudaEventRecord(p->ev_start, p->streams[0].st) != cudaSuccess) { g_last_cuda_error = (int)cudaGetLastError(); return AA_ERR_CUDA; }
-    const int nthreads = (int)std::min<uint64_t>((uint64_t)p->n_streams, p->n_sub);
-    std::vector<std::thread> th;
-    for (int s = 1; s < nthreads; ++s) th.emplace_back(worker, p, s, input, mode, out, max_cands, tap_out);
-    worker(p, 0, input, mode, out, max_cands, tap_out);
-    for (auto &t : th) t.join();
+    // wake the plan's worker threads (one per stream, created at plan creation) and wait for them
+    p->job.input = input; p->job.mode = (int)mode; p->job.out = out; p->job.max_cands = max_cands; p->job.tap_out = tap_out;
+    for (uint64_t j = 0; j < p->n_sub; ++j) p->runs[j] = aa_plan::Run{};
+    command(p, aa_plan::Cmd::run);
     if (p->error.load()) {
         for (auto &S : p->streams) cudaStreamSynchronize(S.st);
         g_last_cuda_error = p->error.load();
@@ -765,9 +931,26 @@ int run_impl(aa_plan *p, const uint8_t *input, Input mode, aa_candidate *out, ui
     const uint64_t total = p->total.load();
     const uint64_t stored = std::min<uint64_t>(p->out_pos.load(), max_cands);
     const auto t1 = std::chrono::steady_clock::now();
-    std::sort(out, out + stored, [](const aa_candidate &a, const aa_candidate &b) {
-        return a.dm_index != b.dm_index ? a.dm_index < b.dm_index : a.t_start < b.t_start;
-    });
+    // Every sub-chunk's run is already sorted, and the runs of one trial follow each other in time, so the final
+    // order is: for every trial, its piece of run 0, of run 1, ...  Two parallel passes through the scratch buffer.
+    if (stored > 1) {
+        if (stored <= p->scratch_cap) {
+            const uint64_t W = (uint64_t)p->ndms_total + 1;
+            uint64_t acc = 0;
+            for (uint32_t d = 0; d < p->ndms_total; ++d) {
+                p->dm_dst[d] = acc;
+                for (uint64_t j = 0; j < p->n_sub; ++j) acc += p->run_cnt[j * W + d + 1] - p->run_cnt[j * W + d];
+            }
+            p->dm_dst[p->ndms_total] = acc;
+            p->job.stored = stored;
+            command(p, aa_plan::Cmd::scatter);
+            command(p, aa_plan::Cmd::copyback);
+        } else {
+            std::sort(out, out + stored, [](const aa_candidate &a, const aa_candidate &b) {
+                return a.dm_index != b.dm_index ? a.dm_index < b.dm_index : a.t_start < b.t_start;
+            });
+        }
+    }
     const auto t2 = std::chrono::steady_clock::now();
     *n_cands = total;
 
@@ -870,6 +1053,29 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
     p->done.reset(new std::atomic<int>[p->n_sub]);
     p->dedisp_issued.reset(new std::atomic<int>[p->n_sub]);
     p->copied.reset(new std::atomic<int>[p->n_streams]);
+    // host side of the runs to come: threads, helper pool, tap lists, run tables, merge scratch -- all of it now
+    if (cudaGetDevice(&p->device) != cudaSuccess) return fail(AA_ERR_CUDA, cudaGetLastError());
+    p->ndms_total = 0;
+    for (auto &R : p->ranges) p->ndms_total += (uint32_t)R.r.ndms;
+    p->nactive = (int)std::min<uint64_t>((uint64_t)p->n_streams, p->n_sub);
+    try {
+        for (auto &S : p->streams) S.tapcopies.reserve((size_t)std::max(1, d->ntap));
+        p->runs.assign(p->n_sub, aa_plan::Run{});
+        p->run_cnt.assign(p->n_sub * (uint64_t)(p->ndms_total + 1), 0u);
+        p->dm_dst.assign((size_t)p->ndms_total + 1, 0);
+        p->hq.reserve((size_t)p->nactive * 3);
+        p->scratch_cap = std::min<uint64_t>(p->n_sub * p->cap, 1ull << 24);
+        p->scratch = static_cast<aa_candidate *>(std::malloc(p->scratch_cap * sizeof(aa_candidate)));   // touched only as far as a run needs
+        if (!p->scratch) p->scratch_cap = 0;                   // the final order then comes from one std::sort
+        for (int s = 0; s < p->nactive; ++s) p->workers.emplace_back(worker_main, p, s);
+        if (p->tap_stage_elems * 4 >= (64ull << 20)) {
+            const int hw = (int)std::max(1u, std::thread::hardware_concurrency());
+            const int nh = std::max(0, std::min(hw - p->nactive, 3 * p->nactive));
+            for (int k = 0; k < nh; ++k) p->helpers.emplace_back(helper_main, p);
+        }
+    } catch (...) {
+        return fail(AA_ERR_OOM, cudaSuccess);
+    }
     for (auto &R : p->ranges) {
         if ((e = cudaMemcpy(R.d_delays, R.h_delays.data(), R.h_delays.size() * 4, cudaMemcpyHostToDevice)) != cudaSuccess)
             return fail(AA_ERR_CUDA, e);
