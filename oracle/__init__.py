@@ -45,6 +45,8 @@ def _load():
         lib.aaor_delays.argtypes = [i32, dbl, dbl, dbl, i32, dbl, dbl, i32, vp]
         lib.aaor_bin.restype = i32
         lib.aaor_bin.argtypes = [vp, u64, i32, i32, u64, u64, vp]
+        lib.aaor_bin_u16.restype = i32
+        lib.aaor_bin_u16.argtypes = [vp, u64, i32, i32, u64, u64, vp]
         lib.aaor_dedisperse.restype = i32
         lib.aaor_dedisperse.argtypes = [vp, i32, u64, u64, vp, i32, u64, u64, vp]
         lib.aaor_block_stats.restype = None
@@ -85,6 +87,26 @@ def geometry(w) -> Dict:
             "nout": [t_valid // rg.bin for rg in w.ranges], "delays": dl}
 
 
+def unpack(x: np.ndarray, w) -> np.ndarray:
+    """The samples of the packed filterbank buffer `x` as an array [nsamp][nchans] (reading A19):
+    nbits 8: `x` itself (uint8); nbits 16: little-endian uint16 words; nbits 4: two samples per byte, the even
+    channel in the low nibble, widened to uint16."""
+    nbits = int(getattr(w, "nbits", 8) or 8)
+    if nbits == 8:
+        assert x.dtype == np.uint8 and x.shape == (w.nsamp, w.nchans)
+        return x
+    if nbits == 16:
+        assert x.dtype == np.uint8 and x.shape == (w.nsamp, 2 * w.nchans)
+        return (x[:, 0::2].astype(np.uint16) | (x[:, 1::2].astype(np.uint16) << 8))
+    if nbits == 4:
+        assert x.dtype == np.uint8 and w.nchans % 2 == 0 and x.shape == (w.nsamp, w.nchans // 2)
+        out = np.empty((w.nsamp, w.nchans), dtype=np.uint16)
+        out[:, 0::2] = x & 15
+        out[:, 1::2] = x >> 4
+        return out
+    raise ValueError("nbits must be 4, 8 or 16")
+
+
 # ---- steps 4-5 ---------------------------------------------------------------
 def dedisperse(x: np.ndarray, w, r: int, rows: Optional[Sequence[int]] = None,
                tau_first: int = 0, ntau: Optional[int] = None, geo: Optional[Dict] = None) -> np.ndarray:
@@ -97,11 +119,13 @@ def dedisperse(x: np.ndarray, w, r: int, rows: Optional[Sequence[int]] = None,
         dl = np.ascontiguousarray(dl[np.asarray(rows, dtype=np.int64)])
     if ntau is None:
         ntau = geo["nout"][r] - tau_first
-    assert x.dtype == np.uint8 and x.shape == (w.nsamp, w.nchans)
-    assert 255 * w.nchans * rg.bin < 2 ** 32
+    x = unpack(x, w)
+    x = np.ascontiguousarray(x)
+    assert (2 ** int(getattr(w, "nbits", 8) or 8) - 1) * w.nchans * rg.bin < 2 ** 32
     span = ntau + int(dl.max())                       # binned samples needed from tau_first on
     y = np.empty((w.nchans, span), dtype=np.uint32)
-    if lib.aaor_bin(x.ctypes.data, w.nsamp, w.nchans, rg.bin, tau_first, span, y.ctypes.data) != 0:
+    fn = lib.aaor_bin if x.dtype == np.uint8 else lib.aaor_bin_u16
+    if fn(x.ctypes.data, w.nsamp, w.nchans, rg.bin, tau_first, span, y.ctypes.data) != 0:
         raise ValueError("binned span runs past the observation")
     D = np.empty((dl.shape[0], ntau), dtype=np.uint32)
     rc = lib.aaor_dedisperse(y.ctypes.data, w.nchans, tau_first, span, dl.ctypes.data, dl.shape[0],

@@ -80,6 +80,24 @@ int aaor_bin(const uint8_t *x, uint64_t nsamp, int nchans, int bin,
     return 0;
 }
 
+/* The same for 16-bit samples (x time-major [nsamp][nchans] uint16): inputs of other bit depths (DESIGN.md reading
+ * A19: 4-bit samples packed two per byte, low nibble = even channel; 16-bit little-endian words) are widened to
+ * uint16 by the caller and binned here.  Sums stay below 2^32 (65535 * bin, bin <= 128). */
+int aaor_bin_u16(const uint16_t *x, uint64_t nsamp, int nchans, int bin,
+                 uint64_t tau_first, uint64_t ntau, uint32_t *y)
+{
+    if ((tau_first + ntau) * (uint64_t)bin > nsamp) return -1;
+    #pragma omp parallel for schedule(static)
+    for (int c = 0; c < nchans; ++c)
+        for (uint64_t k = 0; k < ntau; ++k) {
+            uint32_t s = 0;
+            for (int i = 0; i < bin; ++i)
+                s += x[((tau_first + k) * (uint64_t)bin + (uint64_t)i) * (uint64_t)nchans + (uint64_t)c];
+            y[(size_t)c * ntau + k] = s;
+        }
+    return 0;
+}
+
 /* ---- step 5: dedispersion ---------------------------------------------------
  * D[i][k] = sum_c y[c][(tau_first + k) + delta(c,i) - y_first],  k = 0..ntau-1,
  * where row c of y holds binned samples y_first .. y_first+ny-1.
@@ -115,7 +133,7 @@ int aaor_dedisperse(const uint32_t *y, int nchans, uint64_t y_first, uint64_t ny
  * Each (mu, sigma) comes from exact integer sums m = #, S1 = sum x, S2 = sum x^2:
  *     mu = S1/m,   sigma = sqrt( (m*S2 - S1^2) / (m*m) )
  * with m*S2 - S1^2 formed exactly in 128-bit integers and rounded once. */
-static void moments(uint64_t m, uint64_t S1, uint64_t S2, double *mu, double *sigma)
+static void moments(uint64_t m, uint64_t S1, unsigned __int128 S2, double *mu, double *sigma)
 {
     unsigned __int128 N = (unsigned __int128)m * S2 - (unsigned __int128)S1 * S1;
     double dm = (double)m;
@@ -126,7 +144,10 @@ static void moments(uint64_t m, uint64_t S1, uint64_t S2, double *mu, double *si
 void aaor_block_stats(const uint32_t *d, uint64_t n, double *mu_out, double *sigma_out,
                       uint64_t *nsel_out)
 {
-    uint64_t m = 0, S1 = 0, S2 = 0;
+    /* the sum of squares is kept in 128 bits: 16-bit input on thousands of channels passes 2^64 (65536 samples of
+     * 2^28 each); wherever it stays below 2^64 the value is the same as before */
+    uint64_t m = 0, S1 = 0;
+    unsigned __int128 S2 = 0;
     double mu = 0.0, sigma = 0.0;
     for (uint64_t k = 0; k < n; ++k) { m++; S1 += d[k]; S2 += (uint64_t)d[k] * d[k]; }
     if (m) moments(m, S1, S2, &mu, &sigma);

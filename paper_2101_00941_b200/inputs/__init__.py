@@ -78,14 +78,19 @@ class Workload:
     noise_seed: int
     pulses: Tuple[Pulse, ...]
     norm_block: int = 65536
+    nbits: int = 8          # bits per input sample: 8 (BASELINE.json configs), 4 or 16 (reading A19)
 
     @property
     def ndms_total(self) -> int:
         return sum(r.ndms for r in self.ranges)
 
     @property
+    def row_bytes(self) -> int:
+        return self.nchans * self.nbits // 8
+
+    @property
     def nbytes(self) -> int:
-        return self.nchans * self.nsamp
+        return self.row_bytes * self.nsamp
 
 
 def _pow2_upto(n: int) -> Tuple[int, ...]:
@@ -245,11 +250,34 @@ def pulse_offsets(w: Workload, dm: float) -> np.ndarray:
     return np.rint(_K_DISP * dm * (f ** -2.0 - w.f_top ** -2.0) / w.tsamp).astype(np.int64)
 
 
+def _fill_packed(w: Workload, out: Optional[np.ndarray], t_first: int, n: int) -> np.ndarray:
+    """Other bit depths, derived from the seeded 8-bit stream so that the pulses stay where they are:
+    4 bits: the 8-bit sample >> 4 (0..15, mean 8), two per byte, even channel in the low nibble;
+    16 bits: 256 * (8-bit sample) + a second seeded 8-bit noise stream, little-endian words (mean 32896, sigma 4097)."""
+    w8 = dataclasses.replace(w, nbits=8)
+    hi = fill_span(w8, t_first, n)
+    if out is None:
+        out = np.empty((n, w.row_bytes), dtype=np.uint8)
+    assert out.dtype == np.uint8 and out.shape == (n, w.row_bytes) and out.flags.c_contiguous
+    if w.nbits == 4:
+        assert w.nchans % 2 == 0
+        np.bitwise_or(hi[:, 0::2] >> 4, hi[:, 1::2] & 0xF0, out=out)
+    elif w.nbits == 16:
+        lo = fill_span(dataclasses.replace(w8, noise_seed=w.noise_seed + 7777, pulses=()), t_first, n)
+        out[:, 0::2] = lo
+        out[:, 1::2] = hi
+    else:
+        raise ValueError("nbits must be 4, 8 or 16")
+    return out
+
+
 def fill(w: Workload, out: Optional[np.ndarray] = None) -> np.ndarray:
-    """Write workload `w`'s filterbank into `out` (uint8, shape [nsamp, nchans]); returns it.
+    """Write workload `w`'s filterbank into `out` (uint8, shape [nsamp, row_bytes]); returns it.
 
     `out` may be a view of pinned host memory; it is written in place.
     """
+    if w.nbits != 8:
+        return _fill_packed(w, out, 0, w.nsamp)
     lib = _load()
     if out is None:
         out = np.empty((w.nsamp, w.nchans), dtype=np.uint8)
@@ -265,8 +293,10 @@ def fill(w: Workload, out: Optional[np.ndarray] = None) -> np.ndarray:
 def fill_span(w: Workload, t_first: int, n: int, out: Optional[np.ndarray] = None) -> np.ndarray:
     """Rows [t_first, t_first + n) of workload `w`'s filterbank (what `fill(w)[t_first:t_first+n]` holds) without
     generating the rest: the generator is counter-based, so a rank of a time-sharded run makes only its span."""
-    lib = _load()
     assert 0 <= t_first and t_first + n <= w.nsamp
+    if w.nbits != 8:
+        return _fill_packed(w, out, t_first, n)
+    lib = _load()
     if out is None:
         out = np.empty((n, w.nchans), dtype=np.uint8)
     assert out.dtype == np.uint8 and out.shape == (n, w.nchans) and out.flags.c_contiguous

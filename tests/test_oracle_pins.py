@@ -159,6 +159,49 @@ def test_total_is_conserved_away_from_edges():
     assert np.all(D.sum(axis=1, dtype=np.uint64) == x.sum(dtype=np.uint64))
 
 
+# --------------------------------------------------------------------------- other input bit depths (reading A19)
+def test_unpack_hand_made_bytes():
+    class W4: nsamp = 2; nchans = 4; nbits = 4
+    x = np.array([[0x21, 0xF0], [0x0A, 0x37]], dtype=np.uint8)
+    assert oracle.unpack(x, W4).tolist() == [[1, 2, 0, 15], [10, 0, 7, 3]]        # even channel = low nibble
+    class W16: nsamp = 1; nchans = 2; nbits = 16
+    x = np.array([[0x34, 0x12, 0xFF, 0xFF]], dtype=np.uint8)
+    assert oracle.unpack(x, W16).tolist() == [[0x1234, 0xFFFF]]                    # little-endian words
+
+
+@pytest.mark.parametrize("nbits,bins", [(4, (1, 2)), (16, (1,)), (16, (3,))])
+def test_other_bit_depths_brute_force_and_linearity(nbits, bins):
+    w = I.scaled(_tiny(nchans=6, nsamp=520, bins=bins, ndms=5, seed=nbits), nbits=nbits)
+    x = I.fill(w)
+    u = oracle.unpack(x, w).astype(np.int64)
+    geo = oracle.geometry(w)
+    for r, rg in enumerate(w.ranges):
+        D = oracle.dedisperse(x, w, r, geo=geo)
+        dl = geo["delays"][r]
+        for d in range(rg.ndms):
+            for tau in range(0, geo["nout"][r], 11):                                # python loops over the definition
+                assert D[d, tau] == sum(int(u[rg.bin * (tau + dl[d, c]) + i, c]) for c in range(w.nchans) for i in range(rg.bin))
+        # dedispersion is linear: the 16-bit result is 256 x (high bytes) + (low bytes), the 4-bit one that of the nibbles as bytes
+        w8 = I.scaled(w, nbits=8)
+        if nbits == 16:
+            hi = oracle.dedisperse(np.ascontiguousarray(x[:, 1::2]), w8, r, geo=geo).astype(np.uint64)
+            lo = oracle.dedisperse(np.ascontiguousarray(x[:, 0::2]), w8, r, geo=geo).astype(np.uint64)
+            assert np.array_equal(D.astype(np.uint64), 256 * hi + lo)
+        else:
+            assert np.array_equal(D, oracle.dedisperse(u.astype(np.uint8), w8, r, geo=geo))
+
+
+def test_stats_with_sums_of_squares_beyond_64_bits():
+    """16-bit input on thousands of channels: 65536 samples near 2^28 have a sum of squares near 2^72."""
+    rng = np.random.default_rng(5)
+    d = (rng.integers(0, 1 << 20, size=70000) + (1 << 28)).astype(np.int64)
+    d[rng.integers(0, d.size, 40)] += 1 << 27
+    mu, sg, n = oracle.block_stats(d.astype(np.uint32))
+    pm, ps, pn = _py_stats(d)
+    assert sum(int(v) * int(v) for v in d) > 2 ** 64
+    assert n == pn and mu == pm and abs(sg - ps) <= 1e-12 * ps
+
+
 # --------------------------------------------------------------------------- statistics
 def _py_stats(d):
     """Python restatement with exact integers (fractions) and numpy selection."""
