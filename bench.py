@@ -247,7 +247,7 @@ def run_config(B, k, steps, warmup, link_gbs, max_cands=1 << 24):
     t0 = time.perf_counter()
     host = B.pinned_empty(w.nbytes)
     t_pin = time.perf_counter() - t0
-    I.fill(w, host.numpy().reshape(w.nsamp, w.nchans))
+    I.fill(w, host.numpy().reshape(w.nsamp, w.row_bytes))
     out = {"workload": w.name, "n_streams": w.n_streams, "pin_s": t_pin}
     L = w.chunk_len // w.n_streams
     last = {}
@@ -319,6 +319,8 @@ def main():
     ap.add_argument("--shard-observation", action="store_true",
                     help="strong scaling: ONE observation split by time over the ranks (whole normalisation blocks + halo "
                          "per rank, candidate lists gathered on rank 0); default: one observation per rank (weak)")
+    ap.add_argument("--nbits", type=int, default=8, choices=[4, 8, 16],
+                    help="bits per input sample (DESIGN.md reading A19); 8 is the BASELINE.json workload")
     ap.add_argument("--nsamp", type=int, default=0,
                     help="shorten the observation (profiling runs under ncu only; not a bench line)")
     ap.add_argument("--microbench", action="store_true",
@@ -347,6 +349,9 @@ def main():
     if args.nsamp:
         w = I.scaled(w, nsamp=args.nsamp, name=w.name + f"_nsamp{args.nsamp}")
         note = "shortened observation for profiling; not a bench line"
+    if args.nbits != 8:
+        w = I.scaled(w, nbits=args.nbits, name=w.name + f"_{args.nbits}bit")
+        note = f"{args.nbits}-bit input derived from the seeded 8-bit stream; not the BASELINE.json workload"
     n_streams = args.streams or w.n_streams
     L = w.chunk_len // w.n_streams                     # sub-chunk length of both legs
     shard = None
@@ -366,7 +371,7 @@ def main():
     t_gen0 = time.perf_counter()
     host = B.pinned_empty(w.nbytes)
     t_pin = time.perf_counter() - t_gen0
-    x = host.numpy().reshape(w.nsamp, w.nchans)
+    x = host.numpy().reshape(w.nsamp, w.row_bytes)
     if shard is not None:
         I.fill_span(w_full, shard.t_first, shard.nsamp, x)
     else:
@@ -498,7 +503,7 @@ def main():
             "dtype": "u8 input, u32 exact sums, f64 S/N", "data": "synthetic",
             "legs": {"value": "observation resident in HBM, 1 stream (aa_run_resident): kernels + D2H of candidates + host merge",
                      "e2e": f"aa_run on the pinned host buffer, {n_streams} streams: H2D and D2H inside the timed region (the headline)"},
-            "config": {"workload": w.name, "nchans": w.nchans, "nsamp": w.nsamp, "ndms": w.ndms_total,
+            "config": {"workload": w.name, "nchans": w.nchans, "nsamp": w.nsamp, "nbits": w.nbits, "ndms": w.ndms_total,
                        "widths": list(w.widths), "n_streams_e2e": n_streams, "subchunk_len": L,
                        "chunk_len_e2e": L * n_streams, "l2": "inputs (34 GB) >> L2; no flush needed",
                        "note": note},
@@ -522,7 +527,8 @@ def main():
     # ---- the other configs of BASELINE.json, end to end (north_star: "the 4096-channel configs") ----
     pcs = args.per_config
     if pcs == "auto":
-        pcs = "2,4,5" if (world == 1 and args.workload == 3 and not args.nsamp and not args.shard_observation) else "none"
+        pcs = "2,4,5" if (world == 1 and args.workload == 3 and not args.nsamp and not args.shard_observation
+                          and args.nbits == 8) else "none"
     if rank == 0 and pcs != "none":
         line["per_config"] = {}
         for k in [int(v) for v in pcs.split(",") if v]:

@@ -67,7 +67,7 @@ typedef struct {
 } aa_candidate;
 
 typedef struct {
-    /* filterbank: x[t][c] uint8, time-major, channel 0 centred on f_top, foff < 0 (A1, A2) */
+    /* filterbank: x[t][c], time-major, channel 0 centred on f_top, foff < 0 (A1, A2); uint8 unless nbits says otherwise */
     int32_t  nchans;
     uint64_t nsamp;
     double   tsamp;            /* seconds */
@@ -106,6 +106,11 @@ typedef struct {
      * forced kernel cannot serve (tables do not fit) runs on the plain kernel.  Unknown values: AA_ERR_INVALID.  All
      * kernels compute the same exact sums; tests force each one against the oracle. */
     int32_t  dedisp_variant;
+    /* Bits per input sample (reading A19): 0 or 8 = uint8 [nsamp][nchans]; 4 = two samples per byte, the
+     * even channel in the low nibble, [nsamp][nchans / 2] bytes (nchans even); 16 = little-endian uint16,
+     * [nsamp][2 nchans] bytes.  4-bit samples are unpacked on the device; 16-bit samples are split into a low-byte and
+     * a high-byte plane, both dedispersed by the 8-bit kernels and joined as D = D(low) + 256 D(high) (exact). */
+    int32_t  nbits;
 } aa_plan_desc;
 
 typedef struct {
@@ -212,7 +217,8 @@ int aa_plan_dedisp_variant(const aa_plan *p, int32_t r);
  * async H2D of the new input rows -> corner turn into the device ring -> per range: (binning,)
  * dedispersion, block statistics + boxcar S/N + candidate compaction -> D2H of the candidate
  * list into pinned staging; one host thread per stream copies staging into `out`.
- *   host_input : PINNED host, uint8 [nsamp][nchans]           (AA_ERR_NOT_PINNED otherwise)
+ *   host_input : PINNED host, uint8 [nsamp][nchans] (nbits 8; [nsamp][nchans * nbits / 8] bytes in general)
+ *                (AA_ERR_NOT_PINNED otherwise)
  *   out        : host (pageable ok), room for max_cands records; sorted by (dm_index, t_start)
  *   n_cands    : host, receives the true number found; if it exceeds max_cands or a sub-chunk's
  *                device list overflowed the call returns AA_ERR_OVERFLOW and aa_stats.n_stored

@@ -45,7 +45,7 @@ class PlanDescC(ctypes.Structure):
                 ("streams", ctypes.POINTER(ctypes.c_void_p)),
                 ("ntap", ctypes.c_int32), ("tap_dm_indices", ctypes.POINTER(ctypes.c_uint32)),
                 ("max_cands_per_subchunk", ctypes.c_uint64), ("stage_input", ctypes.c_int32),
-                ("dedisp_variant", ctypes.c_int32)]
+                ("dedisp_variant", ctypes.c_int32), ("nbits", ctypes.c_int32)]
 
 
 class PlanInfoC(ctypes.Structure):
@@ -197,6 +197,7 @@ def _desc_for(w, n_streams=None, chunk_len=None):
     d.n_streams = int(n_streams if n_streams is not None else w.n_streams)
     d.chunk_len = int(chunk_len if chunk_len is not None else w.chunk_len)
     d.norm_block = int(getattr(w, "norm_block", 65536))
+    d.nbits = int(getattr(w, "nbits", 8))
     d._keep = (ranges, widths)
     return d
 
@@ -218,15 +219,7 @@ def plan_geometry(w, *, n_streams: Optional[int] = None, chunk_len: Optional[int
     """aa_plan_geometry: maxshift, halo, sub-chunks, work units and memory of the plan for workload `w`, without
     creating it (no GPU needed)."""
     lib = load_library()
-    ranges = (DMRangeC * len(w.ranges))(*[DMRangeC(r.dm_low, r.dm_step, r.ndms, r.bin) for r in w.ranges])
-    widths = (ctypes.c_int32 * len(w.widths))(*w.widths)
-    d = PlanDescC()
-    d.nchans, d.nsamp, d.tsamp, d.f_top, d.foff = w.nchans, w.nsamp, w.tsamp, w.f_top, w.foff
-    d.nranges, d.ranges, d.nwidths, d.widths = len(w.ranges), ranges, len(w.widths), widths
-    d.snr_threshold = float(w.snr_threshold)
-    d.n_streams = int(n_streams if n_streams is not None else w.n_streams)
-    d.chunk_len = int(chunk_len if chunk_len is not None else w.chunk_len)
-    d.norm_block = int(getattr(w, "norm_block", 65536))
+    d = _desc_for(w, n_streams, chunk_len)
     info = PlanInfoC()
     _check(lib, lib.aa_plan_geometry(ctypes.byref(d), ctypes.byref(info)))
     return {n: int(getattr(info, n)) for n, _ in PlanInfoC._fields_}
@@ -261,6 +254,7 @@ class Plan:
         d.max_cands_per_subchunk = int(max_cands_per_subchunk)
         d.stage_input = 1 if stage_input else 0
         d.dedisp_variant = DEDISP_CHOICE[dedisp_variant] if isinstance(dedisp_variant, str) else int(dedisp_variant)
+        d.nbits = int(getattr(w, "nbits", 8))
         self._arena = None
         self._streams = None
         if torch_resources:

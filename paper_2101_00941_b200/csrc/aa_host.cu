@@ -75,6 +75,7 @@ struct Stream {
     uint8_t *d_raw = nullptr;
     std::vector<uint16_t *> d_binned;
     uint32_t *d_D = nullptr;
+    uint32_t *d_D2 = nullptr;         // 16-bit input: dedispersed high-byte plane of the current range
     aa_candidate *d_cands = nullptr;
     uint32_t *d_count = nullptr;
     uint32_t *h_count = nullptr;      // pinned
@@ -104,11 +105,15 @@ struct aa_plan {
     uint64_t pitchD = 0, d_rows = 0, cap = 0, tap_row_len = 0, tap_stage_elems = 0;
     std::vector<uint64_t> pitch_b;
     uint32_t norm_block = 65536;
+    int nbits = 8, planes = 1;        // planes: 8-bit planes the input is processed as (2 for 16-bit samples)
+    uint64_t row_bytes = 0;           // bytes of one input time sample (all channels)
+    bool big = false;                 // a block's sum of squares may pass 2^63: 128-bit statistics
     int n_streams = 1;
     uint64_t arena_bytes = 0, pinned_bytes = 0;
     void *arena = nullptr;
     bool own_arena = false;
     uint8_t *d_ring = nullptr;
+    uint64_t ring_plane_bytes = 0;    // distance of the high-byte ring from the low-byte ring
     std::vector<Stream> streams;
     std::vector<cudaEvent_t> ev_loaded, ev_dedisp, ev_copied;
     std::unique_ptr<std::atomic<int>[]> loaded, done, dedisp_issued, copied;
@@ -189,6 +194,12 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
     p.desc.tap_dm_indices = p.taps_in.data();
     p.n_streams = d->n_streams;
     p.norm_block = d->norm_block ? d->norm_block : 65536u;
+    p.nbits = d->nbits ? d->nbits : 8;
+    if (p.nbits != 4 && p.nbits != 8 && p.nbits != 16) return AA_ERR_INVALID;
+    if (p.nbits == 4 && (d->nchans & 1)) return AA_ERR_INVALID;
+    p.planes = p.nbits == 16 ? 2 : 1;
+    p.row_bytes = (uint64_t)d->nchans * (uint64_t)p.nbits / 8;
+    const uint64_t maxsample = (1ull << p.nbits) - 1;
 
     for (int j = 0; j < d->nwidths; ++j) {
         if (p.widths[j] < 1 || (j && p.widths[j] <= p.widths[j - 1])) return AA_ERR_INVALID;
@@ -203,15 +214,17 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         if (r.ndms < 1 || r.ndms > 65535 || r.bin < 1 || r.bin > 128 || !(r.dm_step >= 0) || !(r.dm_low >= 0))
             return AA_ERR_INVALID;
         if (p.norm_block % r.bin) return AA_ERR_INVALID;
-        if (255ull * d->nchans * r.bin >= (1ull << 32)) return AA_ERR_INVALID;
+        if (maxsample * d->nchans * r.bin >= (1ull << 32)) return AA_ERR_INVALID;
         lcm = lcm / gcd64(lcm, r.bin) * r.bin;
         bin_max = std::max(bin_max, r.bin);
     }
     if (p.norm_block % kAlign || p.norm_block % lcm) return AA_ERR_INVALID;
     // exact 64-bit sum of squares per block: norm_block*bin*(255*nchans)^2 < 2^63
     {
-        long double bound = (long double)p.norm_block * bin_max * 255.0L * 255.0L * d->nchans * d->nchans;
-        if (bound >= 9.2e18L) return AA_ERR_INVALID;
+        // beyond it (16-bit input on thousands of channels) the statistics take 128-bit sums, in the generic SPS kernel
+        long double bound = (long double)p.norm_block * bin_max * (long double)maxsample * (long double)maxsample * d->nchans * d->nchans;
+        p.big = bound >= 9.2e18L;
+        if (p.big && p.nbits != 16) return AA_ERR_INVALID;
     }
 
     // delay tables: delta(c,i) = floor(((4.148808e3*DM_i)*(1/f_c^2 - 1/f_top^2))/(tsamp*bin) + 0.5)
@@ -287,8 +300,8 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         R.in16 = R.r.bin > 1;
         R.flush_ch = (int)((65535 / (255 * R.r.bin)) & ~1);
         if (R.flush_ch < 2) return AA_ERR_INVALID;
-        R.wide = 255ull * d->nchans * R.r.bin * p.wmax >= (1ull << 32);
-        R.small31 = 255ull * d->nchans * R.r.bin * p.wmax < (1ull << 31);
+        R.wide = (long double)maxsample * d->nchans * R.r.bin * p.wmax >= 4294967296.0L;
+        R.small31 = (long double)maxsample * d->nchans * R.r.bin * p.wmax < 2147483648.0L;
         if (R.in16) {
             auto it = std::find(p.bins.begin(), p.bins.end(), R.r.bin);
             if (it == p.bins.end()) { p.bins.push_back(R.r.bin); R.bin_slot = (int)p.bins.size() - 1; }
@@ -410,22 +423,25 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
     // arena layout (256-byte aligned bump allocation, computed identically in carve())
     uint64_t off = 0;
     auto take = [&](uint64_t bytes) { off = round_up(off, 256) + bytes; };
-    take(round_up((uint64_t)d->nchans, kG8) * p.ring_pitch);    // zero rows pad the channels to a multiple of 8
+    p.ring_plane_bytes = round_up(round_up((uint64_t)d->nchans, kG8) * p.ring_pitch, 256);
+    take(p.ring_plane_bytes * (uint64_t)p.planes);              // zero rows pad the channels to a multiple of 8
     for (auto &R : p.ranges) {
         take((uint64_t)R.r.ndms * d->nchans * 4);
         take((uint64_t)R.h_dtiles.size() * 4);
         take((uint64_t)R.sp_table_bytes());
     }
     for (int s = 0; s < p.n_streams; ++s) {
-        take((p.L + p.halo) * (uint64_t)d->nchans);
-        for (size_t k = 0; k < p.bins.size(); ++k) take(round_up((uint64_t)d->nchans, kSpG) * p.pitch_b[k] * 2);
+        take((p.L + p.halo) * p.row_bytes);
+        for (int pl = 0; pl < p.planes; ++pl)
+            for (size_t k = 0; k < p.bins.size(); ++k) take(round_up((uint64_t)d->nchans, kSpG) * p.pitch_b[k] * 2);
         take(p.d_rows * p.pitchD * 4);
+        if (p.planes == 2) take(p.d_rows * p.pitchD * 4);
         take(p.cap * sizeof(aa_candidate));
         take(256);
     }
     p.arena_bytes = round_up(off, 256);
     p.pinned_bytes = (uint64_t)p.n_streams * (256 + p.cap * sizeof(aa_candidate) + p.tap_stage_elems * 4 +
-                                              (d->stage_input ? (p.L + p.halo) * (uint64_t)d->nchans : 0));
+                                              (d->stage_input ? (p.L + p.halo) * p.row_bytes : 0));
     return AA_OK;
 }
 
@@ -435,18 +451,21 @@ void carve(aa_plan &p)
     uint64_t off = 0;
     auto take = [&](uint64_t bytes) { off = round_up(off, 256); uint8_t *q = base + off; off += bytes; return q; };
     const int nchans = p.desc.nchans;
-    p.d_ring = take(round_up((uint64_t)nchans, kG8) * p.ring_pitch);
+    p.d_ring = take(p.ring_plane_bytes * (uint64_t)p.planes);
     for (auto &R : p.ranges) {
         R.d_delays = reinterpret_cast<int32_t *>(take((uint64_t)R.r.ndms * nchans * 4));
         R.d_dtiles = reinterpret_cast<int32_t *>(take((uint64_t)R.h_dtiles.size() * 4));
         R.d_sp = take((uint64_t)R.sp_table_bytes());
     }
     for (auto &S : p.streams) {
-        S.d_raw = take((p.L + p.halo) * (uint64_t)nchans);
-        S.d_binned.resize(p.bins.size());
-        for (size_t k = 0; k < p.bins.size(); ++k)
-            S.d_binned[k] = reinterpret_cast<uint16_t *>(take(round_up((uint64_t)nchans, kSpG) * p.pitch_b[k] * 2));
+        S.d_raw = take((p.L + p.halo) * p.row_bytes);
+        S.d_binned.resize(p.bins.size() * (size_t)p.planes);          // [plane][bin slot]
+        for (int pl = 0; pl < p.planes; ++pl)
+            for (size_t k = 0; k < p.bins.size(); ++k)
+                S.d_binned[(size_t)pl * p.bins.size() + k] =
+                    reinterpret_cast<uint16_t *>(take(round_up((uint64_t)nchans, kSpG) * p.pitch_b[k] * 2));
         S.d_D = reinterpret_cast<uint32_t *>(take(p.d_rows * p.pitchD * 4));
+        if (p.planes == 2) S.d_D2 = reinterpret_cast<uint32_t *>(take(p.d_rows * p.pitchD * 4));
         S.d_cands = reinterpret_cast<aa_candidate *>(take(p.cap * sizeof(aa_candidate)));
         S.d_count = reinterpret_cast<uint32_t *>(take(256));
     }
@@ -536,9 +555,9 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
         new_rows(j, t_first, nt);
         if (!nt) return;
         const auto c0 = std::chrono::steady_clock::now();
-        std::memcpy(S.h_stage, input + t_first * (uint64_t)nchans, nt * (uint64_t)nchans);
+        std::memcpy(S.h_stage, input + t_first * p->row_bytes, nt * p->row_bytes);
         S.h2h_ms += std::chrono::duration<double, std::milli>(std::chrono::steady_clock::now() - c0).count();
-        S.h2h_bytes += nt * (uint64_t)nchans;
+        S.h2h_bytes += nt * p->row_bytes;
     };
     if (staged && (uint64_t)s < p->n_sub) stage((uint64_t)s);
 
@@ -548,7 +567,7 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
 
         uint64_t t_first, nt;
         new_rows(j, t_first, nt);
-        const uint8_t *src = staged ? S.h_stage : input + t_first * (uint64_t)nchans;
+        const uint8_t *src = staged ? S.h_stage : input + t_first * p->row_bytes;
 
         // First round only (every stream is idle and would start its copy at once): the copies take the link one
         // after the other in sub-chunk order, so that sub-chunk 0 is complete after 1/n_streams of the time.
@@ -559,8 +578,8 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
         }
         AA_W(cudaEventRecord(S.ev[0], st));
         if (!resident && nt) {
-            AA_W(cudaMemcpyAsync(S.d_raw, src, nt * (uint64_t)nchans, cudaMemcpyHostToDevice, st));
-            S.h2d_bytes += nt * (uint64_t)nchans;
+            AA_W(cudaMemcpyAsync(S.d_raw, src, nt * p->row_bytes, cudaMemcpyHostToDevice, st));
+            S.h2d_bytes += nt * p->row_bytes;
             src = S.d_raw;
         }
         AA_W(cudaEventRecord(S.ev[1], st));
@@ -568,8 +587,8 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
             AA_W(cudaEventRecord(p->ev_copied[j], st));
             p->copied[j].store(1, std::memory_order_release);
         }
-        AA_W(launch_corner_turn(src, (int64_t)nt, nchans, (int64_t)t_first, p->d_ring, (int64_t)p->ring_pitch,
-                                (int64_t)R, (int64_t)halo, st));
+        AA_W(launch_corner_turn(src, (int64_t)nt, nchans, p->nbits, (int64_t)t_first, p->d_ring, p->d_ring + p->ring_plane_bytes,
+                                (int64_t)p->ring_pitch, (int64_t)R, (int64_t)halo, st));
         S.prep_launches += nt ? 1 : 0;
         AA_W(cudaEventRecord(S.ev[2], st));
         AA_W(cudaEventRecord(p->ev_loaded[j], st));
@@ -591,8 +610,10 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
         const uint64_t in_len = std::min<uint64_t>(L + halo, nsamp - j * L);
 
         AA_W(cudaEventRecord(S.ev[3], st));
-        {
+        for (int pl = 0; pl < p->planes; ++pl) {
             // power-of-two bins up to 32 share one pass over the ring; anything else is binned on its own
+            const uint8_t *ring_pl = p->d_ring + (uint64_t)pl * p->ring_plane_bytes;
+            uint16_t *const *binned = &S.d_binned[(size_t)pl * p->bins.size()];
             BinMultiArgs ba{};
             bool any = false;
             for (size_t k = 0; k < p->bins.size(); ++k) {
@@ -600,18 +621,18 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
                 int l = -1;
                 for (int q = 0; q < 5; ++q) if (b == (2 << q)) l = q;
                 if (l >= 0 && col0 % 16 == 0 && p->pitch_b[k] % 16 == 0) {
-                    ba.out[l] = S.d_binned[k];
+                    ba.out[l] = binned[k];
                     ba.pitch[l] = (int64_t)p->pitch_b[k];
                     ba.nbinned[l] = (int64_t)(in_len / b);
                     any = true;
                 } else {
-                    AA_W(launch_bin(p->d_ring, (int64_t)p->ring_pitch, (int64_t)col0, nchans, b, (int64_t)(in_len / b),
-                                    S.d_binned[k], (int64_t)p->pitch_b[k], st));
+                    AA_W(launch_bin(ring_pl, (int64_t)p->ring_pitch, (int64_t)col0, nchans, b, (int64_t)(in_len / b),
+                                    binned[k], (int64_t)p->pitch_b[k], st));
                     S.prep_launches++;
                 }
             }
             if (any) {
-                ba.ring = p->d_ring;
+                ba.ring = ring_pl;
                 ba.ring_pitch = (int64_t)p->ring_pitch;
                 ba.col0 = (int64_t)col0;
                 ba.ngroups = (int64_t)((in_len + 31) / 32);
@@ -635,28 +656,33 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
                 const uint64_t left = Rg.nout - tau0;
                 const uint64_t nemit = std::min<uint64_t>(L / b, left);
                 const uint64_t ncols = std::min<uint64_t>(L / b + p->wmax - 1, left);
-                DedispArgs da{};
-                da.in = Rg.in16 ? (const void *)S.d_binned[Rg.bin_slot] : (const void *)p->d_ring;
-                da.pitch_in = Rg.in16 ? (int64_t)p->pitch_b[Rg.bin_slot] : (int64_t)p->ring_pitch;
-                da.col0 = Rg.in16 ? 0 : (int64_t)col0;
-                da.delays = Rg.d_delays;
-                da.dtiles = Rg.d_dtiles;
-                da.nchans = nchans;
-                da.ndms = Rg.r.ndms;
-                da.ncols = (int32_t)ncols;
-                da.out = S.d_D;
-                da.pitch_out = (int64_t)p->pitchD;
-                da.row = Rg.row;
-                da.flush_ch = Rg.flush_ch;
-                da.sp_tab = Rg.d_sp;
-                da.sp_rows = Rg.sp_rows;
-                da.sp_pbytes = Rg.sp_pbytes;
-                da.sp_flush = Rg.sp_flush;
-                if (Rg.g8) AA_W(launch_dedisp_g8(da, st));
-                else if (Rg.ws) AA_W(launch_dedisp_ws(da, Rg.sp_tb, Rg.in16, Rg.ws_wide, st));
-                else if (Rg.sp_tb) AA_W(launch_dedisp_sp(da, Rg.sp_tb, st));
-                else AA_W(launch_dedisp(da, Rg.in16, Rg.dpw, st));
-                S.dedisp_launches++;
+                for (int pl = 0; pl < p->planes; ++pl) {
+                    DedispArgs da{};
+                    da.in = Rg.in16 ? (const void *)S.d_binned[(size_t)pl * p->bins.size() + Rg.bin_slot]
+                                    : (const void *)(p->d_ring + (uint64_t)pl * p->ring_plane_bytes);
+                    da.pitch_in = Rg.in16 ? (int64_t)p->pitch_b[Rg.bin_slot] : (int64_t)p->ring_pitch;
+                    da.col0 = Rg.in16 ? 0 : (int64_t)col0;
+                    da.delays = Rg.d_delays;
+                    da.dtiles = Rg.d_dtiles;
+                    da.nchans = nchans;
+                    da.ndms = Rg.r.ndms;
+                    da.ncols = (int32_t)ncols;
+                    da.out = pl ? S.d_D2 : S.d_D;
+                    da.pitch_out = (int64_t)p->pitchD;
+                    da.row = Rg.row;
+                    da.flush_ch = Rg.flush_ch;
+                    da.sp_tab = Rg.d_sp;
+                    da.sp_rows = Rg.sp_rows;
+                    da.sp_pbytes = Rg.sp_pbytes;
+                    da.sp_flush = Rg.sp_flush;
+                    if (Rg.g8) AA_W(launch_dedisp_g8(da, st));
+                    else if (Rg.ws) AA_W(launch_dedisp_ws(da, Rg.sp_tb, Rg.in16, Rg.ws_wide, st));
+                    else if (Rg.sp_tb) AA_W(launch_dedisp_sp(da, Rg.sp_tb, st));
+                    else AA_W(launch_dedisp(da, Rg.in16, Rg.dpw, st));
+                    S.dedisp_launches++;
+                }
+                // 16-bit input: D = D(low bytes) + 256 D(high bytes)
+                if (p->planes == 2) AA_W(launch_combine_planes(S.d_D, S.d_D2, (int64_t)p->pitchD, Rg.r.ndms, (int32_t)ncols, st));
                 AA_W(cudaEventRecord(e1, st));
                 if (ri == nr - 1) {
                     AA_W(cudaEventRecord(p->ev_dedisp[j], st));
@@ -679,7 +705,7 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
                 sa.cands = S.d_cands;
                 sa.count = S.d_count;
                 sa.cap = (uint32_t)p->cap;
-                AA_W(launch_sps(sa, p->wt, Rg.wide, Rg.small31, st));
+                AA_W(launch_sps(sa, p->wt, Rg.wide, Rg.small31, p->big, st));
                 S.sps_launches++;
                 AA_W(cudaEventRecord(e2, st));
                 // tapped rows: runs of consecutive trials leave in one strided copy (all rows tapped = the dense
@@ -1025,18 +1051,22 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
         if (p->tap_stage_elems)
             if ((e = cudaHostAlloc((void **)&S.h_tap, p->tap_stage_elems * 4, cudaHostAllocDefault)) != cudaSuccess) { cudaGetLastError(); return fail(AA_ERR_OOM, e); }
         if (d->stage_input)
-            if ((e = cudaHostAlloc((void **)&S.h_stage, (p->L + p->halo) * (uint64_t)d->nchans, cudaHostAllocDefault)) != cudaSuccess) { cudaGetLastError(); return fail(AA_ERR_OOM, e); }
+            if ((e = cudaHostAlloc((void **)&S.h_stage, (p->L + p->halo) * p->row_bytes, cudaHostAllocDefault)) != cudaSuccess) { cudaGetLastError(); return fail(AA_ERR_OOM, e); }
     }
     carve(*p);
     {
         const uint64_t ring_pad = round_up((uint64_t)d->nchans, kG8) - (uint64_t)d->nchans;
         const uint64_t pad_rows = round_up((uint64_t)d->nchans, kSpG) - (uint64_t)d->nchans;
-        if (ring_pad && (e = cudaMemset(p->d_ring + (uint64_t)d->nchans * p->ring_pitch, 0, ring_pad * p->ring_pitch)) != cudaSuccess)
-            return fail(AA_ERR_CUDA, e);
+        for (int pl = 0; ring_pad && pl < p->planes; ++pl)
+            if ((e = cudaMemset(p->d_ring + (uint64_t)pl * p->ring_plane_bytes + (uint64_t)d->nchans * p->ring_pitch, 0,
+                                ring_pad * p->ring_pitch)) != cudaSuccess)
+                return fail(AA_ERR_CUDA, e);
         for (auto &S : p->streams)
-            for (size_t k = 0; pad_rows && k < p->bins.size(); ++k)
-                if ((e = cudaMemset(S.d_binned[k] + (uint64_t)d->nchans * p->pitch_b[k], 0, pad_rows * p->pitch_b[k] * 2)) != cudaSuccess)
+            for (size_t k = 0; pad_rows && k < S.d_binned.size(); ++k) {
+                const uint64_t pitch = p->pitch_b[k % p->bins.size()];
+                if ((e = cudaMemset(S.d_binned[k] + (uint64_t)d->nchans * pitch, 0, pad_rows * pitch * 2)) != cudaSuccess)
                     return fail(AA_ERR_CUDA, e);
+            }
     }
     p->ev_loaded.assign(p->n_sub, nullptr);
     for (auto &ev : p->ev_loaded)

@@ -175,9 +175,13 @@ constexpr int kMaxWidths = 32;
 struct WidthTable { int32_t w[kMaxWidths]; };
 
 // ---- kernel launchers (each returns cudaGetLastError()) -------------------------------------
-cudaError_t launch_corner_turn(const uint8_t *src, int64_t nt, int32_t nchans, int64_t t_abs0,
-                               uint8_t *ring, int64_t ring_pitch, int64_t ring_len, int64_t mirror,
+// nbits 8: uint8 rows; 4: two samples per byte (even channel low), unpacked into the ring; 16: little-endian words,
+// low bytes into `ring`, high bytes into `ring_hi`
+cudaError_t launch_corner_turn(const uint8_t *src, int64_t nt, int32_t nchans, int32_t nbits, int64_t t_abs0,
+                               uint8_t *ring, uint8_t *ring_hi, int64_t ring_pitch, int64_t ring_len, int64_t mirror,
                                cudaStream_t st);
+// 16-bit input: D += Dhi << 8 over [ndms][ncols]
+cudaError_t launch_combine_planes(uint32_t *D, const uint32_t *Dhi, int64_t pitch, int32_t ndms, int32_t ncols, cudaStream_t st);
 cudaError_t launch_bin(const uint8_t *ring, int64_t ring_pitch, int64_t col0, int32_t nchans,
                        int32_t bin, int64_t nbinned, uint16_t *out, int64_t out_pitch, cudaStream_t st);
 // every power-of-two bin 2, 4, .., 32 the plan uses, in one pass (level l = bin 2^(l+1); out[l] == nullptr: not wanted)
@@ -195,8 +199,9 @@ cudaError_t launch_dedisp(const DedispArgs &a, bool in16, int dpw, cudaStream_t 
 size_t dedisp_smem_bytes(bool in16, int dpw, int row);
 int dedisp_stage_channels(bool in16);
 cudaError_t dedisp_configure();   // opt in to large dynamic shared memory (once per process)
-// wide: boxcar sums need 64 bits (255 nchans bin wmax >= 2^32); small31: they stay below 2^31
-cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, bool small31, cudaStream_t st);
+// wide: boxcar sums need 64 bits (maxsample nchans bin wmax >= 2^32); small31: they stay below 2^31;
+// big: a block's sum of squares may pass 2^63 (16-bit input on many channels): 128-bit sums in the generic kernel
+cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, bool small31, bool big, cudaStream_t st);
 cudaError_t sps_configure();
 
 }  // namespace aa

@@ -1,6 +1,8 @@
 // Preparation kernels of a sub-chunk: corner turn of the freshly copied
 // time-major rows into the channel-major device ring, and per-range time binning.
 // Both are plain HBM-bound data movement (2 B and ~1+2/b B per input sample).
+#include <algorithm>
+
 #include "aa_internal.h"
 
 namespace aa {
@@ -101,11 +103,88 @@ __global__ void __launch_bounds__(256) corner_turn_vec_kernel(const uint8_t *__r
     }
 }
 
-cudaError_t launch_corner_turn(const uint8_t *src, int64_t nt, int32_t nchans, int64_t t_abs0,
-                               uint8_t *ring, int64_t ring_pitch, int64_t ring_len, int64_t mirror,
+// Other input bit depths (reading A19), same tiling as corner_turn_kernel:
+//   NBITS 4 : a row holds nchans / 2 bytes, even channel in the low nibble; the ring receives the nibbles as bytes;
+//   NBITS 16: a row holds nchans little-endian words; the low bytes go to `ring`, the high bytes to `ring_hi` (two
+//             8-bit planes: dedispersion is linear, D = D(low) + 256 D(high), so the 8-bit kernels serve both).
+template <int NBITS>
+__global__ void __launch_bounds__(256) corner_turn_packed_kernel(const uint8_t *__restrict__ src, int64_t nt, int32_t nchans,
+                                                                 int64_t t_abs0, uint8_t *__restrict__ ring,
+                                                                 uint8_t *__restrict__ ring_hi, int64_t ring_pitch,
+                                                                 int64_t ring_len, int64_t mirror)
+{
+    __shared__ uint8_t tile[2][64][64 + 4];
+    const int tx = threadIdx.x & 63, ty = threadIdx.x >> 6;   // 64 x 4
+    const int64_t tb = (int64_t)blockIdx.x * 64;
+    const int32_t cb = blockIdx.y * 64;
+    const int64_t row_bytes = NBITS == 4 ? nchans / 2 : 2 * (int64_t)nchans;
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const int64_t t = tb + ty + 4 * k;
+        const int32_t c = cb + tx;
+        uint8_t lo = 0, hi = 0;
+        if (t < nt && c < nchans) {
+            if (NBITS == 4) {
+                const uint8_t b = src[t * row_bytes + (c >> 1)];
+                lo = (c & 1) ? (uint8_t)(b >> 4) : (uint8_t)(b & 15);
+            } else {
+                const uint16_t v = *reinterpret_cast<const uint16_t *>(src + t * row_bytes + 2 * (int64_t)c);
+                lo = (uint8_t)(v & 0xFF);
+                hi = (uint8_t)(v >> 8);
+            }
+        }
+        tile[0][ty + 4 * k][tx] = lo;
+        if (NBITS == 16) tile[1][ty + 4 * k][tx] = hi;
+    }
+    __syncthreads();
+#pragma unroll
+    for (int k = 0; k < 16; ++k) {
+        const int32_t c = cb + ty + 4 * k;
+        const int64_t t = tb + tx;
+        if (t < nt && c < nchans) {
+            const int64_t col = (t_abs0 + t) % ring_len;
+            const uint8_t v = tile[0][tx][ty + 4 * k];
+            ring[c * ring_pitch + col] = v;
+            if (col < mirror) ring[c * ring_pitch + ring_len + col] = v;
+            if (NBITS == 16) {
+                const uint8_t h = tile[1][tx][ty + 4 * k];
+                ring_hi[c * ring_pitch + col] = h;
+                if (col < mirror) ring_hi[c * ring_pitch + ring_len + col] = h;
+            }
+        }
+    }
+}
+
+// 16-bit input: D <- D(low bytes) + 256 * D(high bytes), element by element over the sub-chunk's output tile
+__global__ void __launch_bounds__(256) combine_planes_kernel(uint32_t *__restrict__ D, const uint32_t *__restrict__ Dhi,
+                                                             int64_t pitch, int32_t ncols)
+{
+    const int64_t row = (int64_t)blockIdx.y * pitch;
+    for (int32_t i = blockIdx.x * blockDim.x + threadIdx.x; i < ncols; i += gridDim.x * blockDim.x)
+        D[row + i] += Dhi[row + i] << 8;
+}
+
+cudaError_t launch_combine_planes(uint32_t *D, const uint32_t *Dhi, int64_t pitch, int32_t ndms, int32_t ncols, cudaStream_t st)
+{
+    if (ndms <= 0 || ncols <= 0) return cudaSuccess;
+    dim3 grid((unsigned)std::min<int64_t>((ncols + 255) / 256, 64), (unsigned)ndms);
+    combine_planes_kernel<<<grid, 256, 0, st>>>(D, Dhi, pitch, ncols);
+    return cudaGetLastError();
+}
+
+cudaError_t launch_corner_turn(const uint8_t *src, int64_t nt, int32_t nchans, int32_t nbits, int64_t t_abs0,
+                               uint8_t *ring, uint8_t *ring_hi, int64_t ring_pitch, int64_t ring_len, int64_t mirror,
                                cudaStream_t st)
 {
     if (nt <= 0) return cudaSuccess;
+    if (nbits != 8) {
+        dim3 grid((unsigned)((nt + 63) / 64), (unsigned)((nchans + 63) / 64));
+        if (nbits == 4)
+            corner_turn_packed_kernel<4><<<grid, 256, 0, st>>>(src, nt, nchans, t_abs0, ring, ring_hi, ring_pitch, ring_len, mirror);
+        else
+            corner_turn_packed_kernel<16><<<grid, 256, 0, st>>>(src, nt, nchans, t_abs0, ring, ring_hi, ring_pitch, ring_len, mirror);
+        return cudaGetLastError();
+    }
     // 16-sample pieces must not straddle the end of the ring, the mirror boundary or the end of the data
     const bool vec = nchans % 4 == 0 && nt % 16 == 0 && t_abs0 % 16 == 0 && ring_len % 16 == 0 && mirror % 16 == 0 &&
                      ring_pitch % 16 == 0 && (reinterpret_cast<uintptr_t>(src) & 3) == 0 &&

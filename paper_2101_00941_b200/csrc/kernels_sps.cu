@@ -41,7 +41,7 @@ __device__ __forceinline__ uint64_t warp_sum(uint64_t v)
 }
 
 struct Shared {
-    uint64_t red[3][NT / 32];
+    uint64_t red[5][NT / 32];
     double mu, sigma;
     uint64_t m;
     long long bthr[kMaxWidths];
@@ -50,7 +50,9 @@ struct Shared {
     int w[kMaxWidths];        // widths (a dynamically indexed kernel parameter would go through the ADU pipe)
 };
 
-template <typename ACC>
+// BIG: the block's sum of squares may pass 2^64 (16-bit input on thousands of channels): every thread keeps its part
+// as (low 64 bits, carries), the parts are added as three sums that cannot overflow and joined in 128 bits.
+template <typename ACC, bool BIG = false>
 __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const __grid_constant__ WidthTable wt)
 {
     extern __shared__ __align__(16) uint8_t dyn[];
@@ -71,25 +73,40 @@ __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const __grid_c
     double mu = 0.0, sigma = 0.0;
     for (int pass = 0; pass < 4; ++pass) {
         const double lim = __dmul_rn(3.0, sigma);
-        uint64_t m = 0, S1 = 0, S2 = 0;
+        uint64_t m = 0, S1 = 0, S2 = 0, carry = 0;
         for (int64_t i = b0 + tid; i < b1; i += NT) {
             const uint32_t x = row[i];
             const bool sel = (pass == 0) || (fabs(__dsub_rn((double)x, mu)) <= lim);
             if (sel) {
                 m += 1;
                 S1 += x;
-                S2 += (uint64_t)x * x;
+                const uint64_t sq = (uint64_t)x * x;
+                S2 += sq;
+                if (BIG) carry += S2 < sq;
             }
         }
-        m = warp_sum(m); S1 = warp_sum(S1); S2 = warp_sum(S2);
-        if (lane == 0) { sh.red[0][warp] = m; sh.red[1][warp] = S1; sh.red[2][warp] = S2; }
+        m = warp_sum(m); S1 = warp_sum(S1);
+        if (BIG) {
+            const uint64_t lo = warp_sum(S2 & 0xFFFFFFFFull), hi = warp_sum(S2 >> 32);
+            carry = warp_sum(carry);
+            if (lane == 0) { sh.red[2][warp] = lo; sh.red[3][warp] = hi; sh.red[4][warp] = carry; }
+        } else {
+            S2 = warp_sum(S2);
+            if (lane == 0) sh.red[2][warp] = S2;
+        }
+        if (lane == 0) { sh.red[0][warp] = m; sh.red[1][warp] = S1; }
         __syncthreads();
         if (tid == 0) {
-            m = S1 = S2 = 0;
-            for (int w = 0; w < NT / 32; ++w) { m += sh.red[0][w]; S1 += sh.red[1][w]; S2 += sh.red[2][w]; }
+            m = S1 = 0;
+            unsigned __int128 S2w = 0;
+            for (int w = 0; w < NT / 32; ++w) {
+                m += sh.red[0][w]; S1 += sh.red[1][w];
+                S2w += sh.red[2][w];
+                if (BIG) S2w += ((unsigned __int128)sh.red[3][w] << 32) + ((unsigned __int128)sh.red[4][w] << 64);
+            }
             sh.m = m;
             if (m) {
-                const unsigned __int128 N = (unsigned __int128)m * S2 - (unsigned __int128)S1 * S1;
+                const unsigned __int128 N = (unsigned __int128)m * S2w - (unsigned __int128)S1 * S1;
                 const double dm = __ull2double_rn(m);
                 sh.mu = __ddiv_rn(__ull2double_rn(S1), dm);
                 sh.sigma = __dsqrt_rn(__ddiv_rn(u128_to_double(N), __dmul_rn(dm, dm)));
@@ -641,17 +658,21 @@ cudaError_t sps_configure()
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(sps_kernel<uint64_t>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(sps_kernel<uint64_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(sps_kernel<uint32_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
+    if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(sps_cluster_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(sps_cluster_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
 }
 
-cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, bool small31, cudaStream_t st)
+cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, bool small31, bool big, cudaStream_t st)
 {
     if (a.nemit <= 0 || a.ndms <= 0) return cudaSuccess;
     const unsigned nblk = (unsigned)((a.nemit + a.block_len - 1) / a.block_len);
     int C = 1, seg = 0;
-    if (sps_cluster_shape(a, wide, C, seg)) {
+    if (!big && sps_cluster_shape(a, wide, C, seg)) {
         cudaLaunchConfig_t cfg{};
         cfg.gridDim = dim3(nblk * (unsigned)C, (unsigned)a.ndms);
         cfg.blockDim = dim3(NT2);
@@ -668,8 +689,12 @@ cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, bool s
                        : cudaLaunchKernelEx(&cfg, sps_cluster_kernel<false>, a, wt, C, seg);
     }
     dim3 grid(nblk, (unsigned)a.ndms);
-    if (wide)
+    if (wide && big)
+        sps_kernel<uint64_t, true><<<grid, NT, sps_smem(a, true), st>>>(a, wt);
+    else if (wide)
         sps_kernel<uint64_t><<<grid, NT, sps_smem(a, true), st>>>(a, wt);
+    else if (big)
+        sps_kernel<uint32_t, true><<<grid, NT, sps_smem(a, false), st>>>(a, wt);
     else
         sps_kernel<uint32_t><<<grid, NT, sps_smem(a, false), st>>>(a, wt);
     return cudaGetLastError();

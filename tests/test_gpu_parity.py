@@ -18,7 +18,7 @@ def B():
 
 def _pinned_fill(B, w):
     buf = B.pinned_empty(w.nbytes)
-    x = buf.numpy().reshape(w.nsamp, w.nchans)
+    x = buf.numpy().reshape(w.nsamp, w.row_bytes)
     I.fill(w, x)
     return buf, x
 
@@ -166,6 +166,34 @@ def test_binned_input_on_the_shared_pattern_kernel(B, variant, code, case):
         base += rg.ndms
     res = compare_candidates(cands, ref, w.snr_threshold)
     assert res["only_gpu"] == 0 and res["only_oracle"] == 0
+
+
+@pytest.mark.parametrize("nbits,case", [
+    (4, dict(nchans=16, nsamp=20000)),                                                    # plain kernel
+    (4, dict(nchans=30, nsamp=20011, ndms=33, bins=(1, 2))),                              # ragged, binned
+    (4, dict(nchans=302, ndms=100, nsamp=21000, chunk_len=8192, foff=-0.5, dm_step=0.25, norm_block=1024)),   # shared-pattern kernel
+    (16, dict(nchans=16, nsamp=20000)),
+    (16, dict(nchans=24, ndms=37, nsamp=15001, bins=(1, 4), chunk_len=8192, n_streams=2)),
+    (16, dict(nchans=302, ndms=100, nsamp=21000, chunk_len=8192, foff=-0.5, dm_step=0.25, norm_block=1024)),  # both planes on the shared-pattern kernel
+    (16, dict(nchans=1024, ndms=40, nsamp=30000, chunk_len=8192, foff=-0.2, dm_step=0.25, norm_block=4096, widths=(1, 2, 4, 64))),  # 128-bit statistics, 64-bit boxcars
+])
+def test_other_input_bit_depths(B, nbits, case):
+    """DESIGN.md reading A19: 4-bit (nibbles unpacked on the device) and 16-bit (two 8-bit planes, D = D(low) + 256 D(high))
+    input against the oracle, dense plane bit for bit."""
+    w = I.scaled(_tiny(**case), nbits=nbits)
+    cands, ref, res = _check_against_oracle(B, w)
+    assert res["only_gpu"] == 0 and res["only_oracle"] == 0 and res["width_ties"] == 0
+    assert len(ref) > 0
+
+
+def test_saturated_16_bit_input(B):
+    w = I.scaled(_tiny(nchans=1024, ndms=70, nsamp=9000, chunk_len=4096, f_top=1500.0, foff=-0.2, dm_step=0.25, norm_block=1024), nbits=16)
+    buf = B.pinned_empty(w.nbytes)
+    buf.numpy()[:] = 255                                 # every sample 65535
+    with B.Plan(w, taps=list(range(w.ndms_total))) as plan:
+        cands, tap = plan.run(buf)
+        assert len(cands) == 0
+        assert np.all(tap[:, :plan.nout[0]] == 65535 * w.nchans)
 
 
 def test_saturated_binned_input(B):

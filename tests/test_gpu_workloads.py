@@ -45,7 +45,7 @@ def B():
 
 def _pinned_fill(B, w):
     buf = B.pinned_empty(w.nbytes)
-    x = buf.numpy().reshape(w.nsamp, w.nchans)
+    x = buf.numpy().reshape(w.nsamp, w.row_bytes)
     I.fill(w, x)
     return buf, x
 
