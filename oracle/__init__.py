@@ -53,6 +53,10 @@ def _load():
         lib.aaor_block_stats.argtypes = [vp, u64, vp, vp, vp]
         lib.aaor_sps_row.restype = i64
         lib.aaor_sps_row.argtypes = [vp, u64, u64, u64, u64, vp, i32, dbl, u64, u64, vp, vp, vp, i64]
+        lib.aaor_sps_row2.restype = i64
+        lib.aaor_sps_row2.argtypes = [vp, u64, u64, u64, u64, vp, i32, dbl, u64, u64, i32, i32, vp, vp, vp, i64]
+        lib.aaor_series_stats.restype = None
+        lib.aaor_series_stats.argtypes = [vp, u64, vp, vp, vp]
         lib.aaor_num_threads.restype = i32
         _lib = lib
     return _lib
@@ -143,11 +147,21 @@ def block_stats(d: np.ndarray) -> Tuple[float, float, int]:
     return mu.value, sg.value, ns.value
 
 
+def series_stats(v: np.ndarray) -> Tuple[float, float, int]:
+    """Estimator A8 on a series of 64-bit values (the boxcar series of one width, reading A18)."""
+    v = np.ascontiguousarray(v, dtype=np.uint64)
+    mu, sg, ns = ctypes.c_double(), ctypes.c_double(), ctypes.c_uint64()
+    _load().aaor_series_stats(v.ctypes.data, v.size, ctypes.byref(mu), ctypes.byref(sg), ctypes.byref(ns))
+    return mu.value, sg.value, ns.value
+
+
 # ---- steps 7-8 -----------------------------------------------------------------
 def sps_row(d: np.ndarray, w, r: int, *, d_first: int = 0, tau_a: int = 0,
             tau_b: Optional[int] = None, nout: Optional[int] = None,
             geo: Optional[Dict] = None) -> Tuple[np.ndarray, np.ndarray, np.ndarray]:
-    """Candidates (tau, width, S/N double; binned units) of one dedispersed row."""
+    """Candidates (tau, width, S/N double; binned units) of one dedispersed row.  The workload's optional attributes
+    `wdec` (reading A20: widths above it on a coarser time grid) and `sigma_mode` (reading A18: 1 = statistics of each
+    width's own boxcar series) select the variants; both default to the search BASELINE.json states."""
     lib = _load()
     rg = w.ranges[r]
     if nout is None:
@@ -160,9 +174,10 @@ def sps_row(d: np.ndarray, w, r: int, *, d_first: int = 0, tau_a: int = 0,
     cap = max(1024, min(int(tau_b - tau_a), 1 << 22))
     while True:
         tau = np.empty(cap, dtype=np.uint64); ww = np.empty(cap, dtype=np.int32); sn = np.empty(cap, dtype=np.float64)
-        n = lib.aaor_sps_row(d.ctypes.data, d_first, d.size, nout, L, widths.ctypes.data, widths.size,
-                             float(w.snr_threshold), tau_a, tau_b, tau.ctypes.data, ww.ctypes.data,
-                             sn.ctypes.data, cap)
+        n = lib.aaor_sps_row2(d.ctypes.data, d_first, d.size, nout, L, widths.ctypes.data, widths.size,
+                              float(w.snr_threshold), tau_a, tau_b, int(getattr(w, "wdec", 0) or 0),
+                              int(getattr(w, "sigma_mode", 0) or 0), tau.ctypes.data, ww.ctypes.data,
+                              sn.ctypes.data, cap)
         if n < 0:
             raise ValueError("row segment does not cover the requested blocks")
         if n <= cap:

@@ -161,51 +161,126 @@ void aaor_block_stats(const uint32_t *d, uint64_t n, double *mu_out, double *sig
     *mu_out = mu; *sigma_out = sigma; *nsel_out = m;
 }
 
+/* ---- step 6 on a series of 64-bit values (the boxcar series of one width, reading A18) -----------------
+ * Same estimator as aaor_block_stats: a plain pass and three 3-sigma-clip passes, population sigma, from exact
+ * integer sums (128-bit sum of squares, 128-bit numerator rounded once). */
+void aaor_series_stats(const uint64_t *v, uint64_t n, double *mu_out, double *sigma_out, uint64_t *nsel_out)
+{
+    uint64_t m = 0, S1 = 0;
+    unsigned __int128 S2 = 0;
+    double mu = 0.0, sigma = 0.0;
+    for (uint64_t k = 0; k < n; ++k) { m++; S1 += v[k]; S2 += (unsigned __int128)v[k] * v[k]; }
+    if (m) moments(m, S1, S2, &mu, &sigma);
+    for (int pass = 0; pass < 3 && m; ++pass) {
+        double lim = 3.0 * sigma;
+        m = 0; S1 = 0; S2 = 0;
+        for (uint64_t k = 0; k < n; ++k)
+            if (fabs((double)v[k] - mu) <= lim) { m++; S1 += v[k]; S2 += (unsigned __int128)v[k] * v[k]; }
+        if (m) moments(m, S1, S2, &mu, &sigma);
+    }
+    *mu_out = mu; *sigma_out = sigma; *nsel_out = m;
+}
+
+/* Reading A20 (decimated long boxcars): widths above wdec are looked at on a coarser time grid, as in a search that
+ * halves the time resolution while it doubles the width: dec(w) = the smallest power of two with w / dec(w) <= wdec
+ * (1 if wdec <= 0 or w <= wdec); the boxcar of width w is evaluated only at tau with tau mod dec(w) == 0 (tau = the
+ * absolute binned sample index).  The sums themselves stay exact. */
+static uint64_t width_dec(uint64_t w, int wdec)
+{
+    uint64_t dec = 1;
+    if (wdec > 0)
+        while (w > (uint64_t)wdec * dec) dec *= 2;
+    return dec;
+}
+
 /* ---- steps 6-8 for one dedispersed row --------------------------------------
  * d[0..d_count) holds D[row][d_first .. d_first+d_count).  nout = number of valid
  * output samples of the row's range, L = norm-block length in binned samples.
  * Emits one candidate per tau in [tau_a, tau_b) (tau_a on a block boundary):
- *   for every width w with tau + w <= nout:  B_w = sum_{i<w} D[tau+i],
- *   S_w = (B_w - w*mu_k) / (sigma_k*sqrt(w)),  k = block containing tau   (A9, A10)
+ *   for every width w with tau + w <= nout (and tau on the width's grid, A20):  B_w = sum_{i<w} D[tau+i],
+ *   sigma_mode 0 (A10): S_w = (B_w - w*mu_k) / (sigma_k*sqrt(w)),  k = block containing tau   (A9)
+ *   sigma_mode 1 (A18): S_w = (B_w - mu_{k,w}) / sigma_{k,w}, (mu, sigma)_{k,w} = the robust statistics (A8) of the
+ *                boxcar series of width w itself over the block: B_w[t] for the t of block k on the width's grid with
+ *                t + w <= nout; a width with sigma_{k,w} = 0 or fewer than 32 such t is skipped
  *   w* = argmax_w S_w (ties -> smallest w);  emit iff S_{w*} >= thr, sigma_k > 0
  *   and the block has n_k >= 32 samples                                    (A11, A13)
  * Returns the number found (may exceed max_out; only max_out are stored) or -1
  * if d does not cover what is needed. */
+int64_t aaor_sps_row2(const uint32_t *d, uint64_t d_first, uint64_t d_count,
+                      uint64_t nout, uint64_t L,
+                      const int32_t *widths, int nwidths, double thr,
+                      uint64_t tau_a, uint64_t tau_b, int wdec, int sigma_mode,
+                      uint64_t *out_tau, int32_t *out_w, double *out_snr, int64_t max_out)
+{
+    int64_t found = 0;
+    if (tau_b > nout) tau_b = nout;
+    if (tau_a % L != 0) return -1;
+    double *wmu = (double *)malloc(sizeof(double) * (size_t)(nwidths > 0 ? nwidths : 1));
+    double *wsg = (double *)malloc(sizeof(double) * (size_t)(nwidths > 0 ? nwidths : 1));
+    uint64_t *series = sigma_mode ? (uint64_t *)malloc(sizeof(uint64_t) * (size_t)L) : NULL;
+    for (uint64_t b0 = tau_a; b0 < tau_b; b0 += L) {
+        uint64_t b1 = b0 + L < nout ? b0 + L : nout;       /* block [b0, b1) */
+        uint64_t n_k = b1 - b0, nsel;
+        double mu, sigma;
+        if (b0 < d_first || b1 > d_first + d_count) { found = -1; break; }
+        aaor_block_stats(d + (b0 - d_first), n_k, &mu, &sigma, &nsel);
+        if (!(sigma > 0.0) || n_k < 32) continue;
+        if (sigma_mode) {
+            int bad = 0;
+            for (int j = 0; j < nwidths; ++j) {
+                uint64_t w = (uint64_t)widths[j], dec = width_dec(w, wdec), ns = 0, dummy;
+                for (uint64_t t = b0; t < b1; ++t) {
+                    if (t % dec != 0 || t + w > nout) continue;
+                    if (t + w > d_first + d_count) { bad = 1; break; }
+                    uint64_t B = 0;
+                    for (uint64_t i = 0; i < w; ++i) B += d[t + i - d_first];
+                    series[ns++] = B;
+                }
+                if (bad) break;
+                wmu[j] = 0.0; wsg[j] = 0.0;
+                if (ns >= 32) aaor_series_stats(series, ns, &wmu[j], &wsg[j], &dummy);
+            }
+            if (bad) { found = -1; break; }
+        }
+        uint64_t e = b1 < tau_b ? b1 : tau_b;
+        int fail = 0;
+        for (uint64_t tau = b0; tau < e && !fail; ++tau) {
+            double best = 0.0; int32_t best_w = 0;
+            for (int j = 0; j < nwidths; ++j) {
+                uint64_t w = (uint64_t)widths[j];
+                if (tau + w > nout) continue;
+                if (tau % width_dec(w, wdec) != 0) continue;
+                if (tau + w > d_first + d_count) { fail = 1; break; }
+                int64_t B = 0;
+                for (uint64_t i = 0; i < w; ++i) B += d[tau + i - d_first];
+                double S;
+                if (sigma_mode) {
+                    if (!(wsg[j] > 0.0)) continue;
+                    S = ((double)B - wmu[j]) / wsg[j];
+                } else {
+                    S = ((double)B - (double)w * mu) / (sigma * sqrt((double)w));
+                }
+                if (best_w == 0 || S > best) { best = S; best_w = (int32_t)w; }
+            }
+            if (!fail && best_w != 0 && best >= thr) {
+                if (found < max_out) { out_tau[found] = tau; out_w[found] = best_w; out_snr[found] = best; }
+                found++;
+            }
+        }
+        if (fail) { found = -1; break; }
+    }
+    free(wmu); free(wsg); free(series);
+    return found;
+}
+
+/* The search of steps 6-8 as BASELINE.json states it: every width at every tau, white-noise scaling. */
 int64_t aaor_sps_row(const uint32_t *d, uint64_t d_first, uint64_t d_count,
                      uint64_t nout, uint64_t L,
                      const int32_t *widths, int nwidths, double thr,
                      uint64_t tau_a, uint64_t tau_b,
                      uint64_t *out_tau, int32_t *out_w, double *out_snr, int64_t max_out)
 {
-    int64_t found = 0;
-    if (tau_b > nout) tau_b = nout;
-    if (tau_a % L != 0) return -1;
-    for (uint64_t b0 = tau_a; b0 < tau_b; b0 += L) {
-        uint64_t b1 = b0 + L < nout ? b0 + L : nout;       /* block [b0, b1) */
-        uint64_t n_k = b1 - b0, nsel;
-        double mu, sigma;
-        if (b0 < d_first || b1 > d_first + d_count) return -1;
-        aaor_block_stats(d + (b0 - d_first), n_k, &mu, &sigma, &nsel);
-        if (!(sigma > 0.0) || n_k < 32) continue;
-        uint64_t e = b1 < tau_b ? b1 : tau_b;
-        for (uint64_t tau = b0; tau < e; ++tau) {
-            double best = 0.0; int32_t best_w = 0;
-            for (int j = 0; j < nwidths; ++j) {
-                uint64_t w = (uint64_t)widths[j];
-                if (tau + w > nout) continue;
-                if (tau + w > d_first + d_count) return -1;
-                int64_t B = 0;
-                for (uint64_t i = 0; i < w; ++i) B += d[tau + i - d_first];
-                double S = ((double)B - (double)w * mu) / (sigma * sqrt((double)w));
-                if (best_w == 0 || S > best) { best = S; best_w = (int32_t)w; }
-            }
-            if (best_w != 0 && best >= thr) {
-                if (found < max_out) { out_tau[found] = tau; out_w[found] = best_w; out_snr[found] = best; }
-                found++;
-            }
-        }
-    }
-    return found;
+    return aaor_sps_row2(d, d_first, d_count, nout, L, widths, nwidths, thr, tau_a, tau_b, 0, 0, out_tau, out_w, out_snr, max_out);
 }
 
 int aaor_num_threads(void)

@@ -79,6 +79,8 @@ class Workload:
     pulses: Tuple[Pulse, ...]
     norm_block: int = 65536
     nbits: int = 8          # bits per input sample: 8 (BASELINE.json configs), 4 or 16 (reading A19)
+    wdec: int = 0           # > 0: widths above it are searched on a coarser time grid (reading A20)
+    sigma_mode: int = 0     # 1: S/N from the statistics of each width's own boxcar series (reading A18)
 
     @property
     def ndms_total(self) -> int:

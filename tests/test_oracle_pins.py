@@ -329,6 +329,118 @@ def test_candidate_rule_brute_force(seed):
         assert all(t < 256 for t in tau)       # the 14-sample last block emits nothing (A13)
 
 
+# ---- readings A20 (long boxcars on a coarser time grid) and A18 (statistics of each width's own series) ----------
+def _dec(wd, wdec):
+    dec = 1
+    while wdec > 0 and wd > wdec * dec:
+        dec *= 2
+    return dec
+
+
+def _py_candidates_variants(d, widths, thr, L, nout, wdec, sigma_mode):
+    """The definition in python loops: exact integer boxcars, statistics through the exact-fraction restatement."""
+    out = []
+    for b0 in range(0, nout, L):
+        b1 = min(b0 + L, nout)
+        mu, sg, _ = _py_stats(d[b0:b1])
+        if not sg > 0 or b1 - b0 < 32:
+            continue
+        ws = {}
+        if sigma_mode:
+            for wd in widths:
+                series = [sum(int(v) for v in d[t:t + wd]) for t in range(b0, b1) if t % _dec(wd, wdec) == 0 and t + wd <= nout]
+                ws[wd] = _py_stats(np.array(series, dtype=np.int64))[:2] if len(series) >= 32 else (0.0, 0.0)
+        for tau in range(b0, b1):
+            best = None
+            for wd in widths:
+                if tau + wd > nout or tau % _dec(wd, wdec) != 0:
+                    continue
+                B = float(sum(int(v) for v in d[tau:tau + wd]))
+                if sigma_mode:
+                    if not ws[wd][1] > 0:
+                        continue
+                    S = (B - ws[wd][0]) / ws[wd][1]
+                else:
+                    S = (B - wd * mu) / (sg * math.sqrt(wd))
+                if best is None or S > best[1]:
+                    best = (wd, S)
+            if best is not None and best[1] >= thr:
+                out.append((tau, best[0], best[1]))
+    return out
+
+
+class _WV(_W):
+    def __init__(self, widths, thr, norm_block, wdec=0, sigma_mode=0):
+        super().__init__(widths, thr, norm_block)
+        self.wdec = wdec; self.sigma_mode = sigma_mode
+
+
+@pytest.mark.parametrize("wdec,sigma_mode", [(2, 0), (4, 0), (0, 1), (2, 1), (3, 1)])
+def test_search_variants_brute_force(wdec, sigma_mode):
+    rng = np.random.default_rng(10 * wdec + sigma_mode)
+    nout, L = 900, 256                     # last block has 132 samples: on a grid of 8 that is 17 < 32 boxcars
+    d = np.rint(rng.normal(5000, 50, size=nout)).astype(np.uint32)
+    d[71:79] += 90; d[200] += 400; d[250:266] += 60; d[600:605] += 110; d[nout - 3:] += 300
+    widths = (1, 2, 5, 8, 16)
+    tau, ww, sn = oracle.sps_row(d, _WV(widths, 3.0, L, wdec, sigma_mode), 0, nout=nout)
+    ref = _py_candidates_variants(d, widths, 3.0, L, nout, wdec, sigma_mode)
+    assert len(ref) > 10 and len({r[1] for r in ref}) >= 3
+    assert [int(t) for t in tau] == [r[0] for r in ref]
+    assert [int(a) for a in ww] == [r[1] for r in ref]
+    assert np.allclose(sn, [r[2] for r in ref], rtol=1e-12, atol=0)
+
+
+def test_decimated_widths_are_the_full_search_on_a_coarser_grid():
+    rng = np.random.default_rng(3)
+    d = np.rint(rng.normal(9000, 70, size=2048)).astype(np.uint32)
+    d[1001:1017] += 150                                             # 16-sample pulse starting at an odd sample
+    widths = (1, 2, 4, 8, 16, 32)
+    full = oracle.sps_row(d, _WV(widths, 5.0, 1024), 0, nout=d.size)
+    assert np.array_equal(oracle.sps_row(d, _WV(widths, 5.0, 1024, wdec=32), 0, nout=d.size)[0], full[0])   # wdec >= wmax: nothing changes
+    tau, ww, sn = oracle.sps_row(d, _WV(widths, 5.0, 1024, wdec=4), 0, nout=d.size)        # dec = 1 1 1 2 4 8
+    for t, a in zip(tau, ww):
+        assert t % _dec(int(a), 4) == 0
+    best_full = int(full[0][np.argmax(full[2])]), int(full[1][np.argmax(full[2])])
+    assert best_full == (1001, 16)                                   # the full search finds the pulse where it is
+    k = np.argmax(sn)
+    assert int(ww[k]) == 16 and int(tau[k]) in (1000, 1004) and sn[k] < full[2].max()    # the grid of width 16 is 4 samples
+    # a candidate of the decimated search at a tau on every grid has exactly the S/N of the full search there
+    both = {int(t): float(s) for t, a, s in zip(full[0], full[1], full[2])}
+    for t, a, s in zip(tau, ww, sn):
+        if t % 8 == 0 and int(t) in both:
+            assert s == both[int(t)]
+
+
+def test_series_statistics():
+    rng = np.random.default_rng(8)
+    d = rng.integers(1000, 2000, size=5000).astype(np.uint32)
+    assert oracle.series_stats(d.astype(np.uint64)) == oracle.block_stats(d)      # width 1: the block statistics themselves
+    v = (rng.integers(0, 1 << 22, size=3000) + (1 << 35)).astype(np.int64)        # boxcar sums of 16-bit data: past 2^32
+    v[rng.integers(0, v.size, 25)] += 1 << 30
+    mu, sg, n = oracle.series_stats(v.astype(np.uint64))
+    pm, ps, pn = _py_stats(v)
+    assert n == pn and mu == pm and abs(sg - ps) <= 1e-12 * ps
+
+
+def test_measured_sigma_of_white_noise_follows_sqrt_w():
+    """Reading A18 on Gaussian noise: the boxcar series of width w has sigma_w = 0.98487 sigma sqrt(w) (three 3-sigma
+    clips) and mean w mu, so the two S/N scalings agree to a few per cent; they differ when the noise is not white."""
+    rng = np.random.default_rng(12)
+    d = np.rint(rng.normal(50000, 300, size=1 << 16)).astype(np.uint32)
+    d[30000:30008] += 1500
+    widths = (1, 4, 16)
+    a = oracle.sps_row(d, _WV(widths, 8.0, 1 << 16), 0, nout=d.size)
+    b = oracle.sps_row(d, _WV(widths, 8.0, 1 << 16, sigma_mode=1), 0, nout=d.size)
+    ta, tb = int(a[0][np.argmax(a[2])]), int(b[0][np.argmax(b[2])])
+    assert abs(ta - 30000) <= 4 and abs(tb - 30000) <= 4
+    assert abs(a[2].max() / b[2].max() - 1) < 0.05
+    for w_ in widths:
+        series = np.convolve(d.astype(np.int64), np.ones(w_, dtype=np.int64), "valid")
+        mu, sg, _ = oracle.series_stats(series.astype(np.uint64))
+        # overlapping boxcars are correlated samples of the same Gaussian: the clip factor is still 0.98487
+        assert abs(mu / (w_ * 50000.0) - 1) < 1e-3 and abs(sg / (0.98487 * 300 * math.sqrt(w_)) - 1) < 0.03
+
+
 def test_boxcar_may_run_into_the_next_block_but_not_past_the_end():
     d = np.tile(np.array([99, 101], dtype=np.uint32), 64)     # two blocks of 64
     d[62:66] = 140
