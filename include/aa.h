@@ -111,6 +111,18 @@ typedef struct {
      * [nsamp][2 nchans] bytes.  4-bit samples are unpacked on the device; 16-bit samples are split into a low-byte and
      * a high-byte plane, both dedispersed by the 8-bit kernels and joined as D = D(low) + 256 D(high) (exact). */
     int32_t  nbits;
+    /* Reading A20 (decimated long boxcars): 0 = every width at every sample (BASELINE.json).  wdec > 0:
+     * a width w > wdec is searched on a coarser time grid, as in a search that halves the time resolution each time it
+     * doubles the width: only at tau (absolute binned sample) with tau mod dec(w) == 0, dec(w) = the smallest power
+     * of two with w / dec(w) <= wdec.  The boxcar sums themselves stay exact. */
+    int32_t  width_decimation;
+    /* Reading A18 (per-width measured sigma): 0 = S_w = (B_w - w mu) / (sigma sqrt w), white-noise
+     * scaling of the block's statistics (BASELINE.json).  1 = S_w = (B_w - mu_w) / sigma_w with (mu_w, sigma_w) the same
+     * robust estimator applied to the boxcar series of width w itself over the normalisation block (on the width's grid);
+     * a width with sigma_w = 0 or fewer than 32 boxcars in the block is skipped.  Needs normalisation blocks the
+     * cluster kernel takes (block / bin a multiple of 4, at most 131072 binned samples, 32-bit boxcar sums):
+     * AA_ERR_INVALID otherwise. */
+    int32_t  sigma_mode;
 } aa_plan_desc;
 
 typedef struct {

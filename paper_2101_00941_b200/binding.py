@@ -45,7 +45,8 @@ class PlanDescC(ctypes.Structure):
                 ("streams", ctypes.POINTER(ctypes.c_void_p)),
                 ("ntap", ctypes.c_int32), ("tap_dm_indices", ctypes.POINTER(ctypes.c_uint32)),
                 ("max_cands_per_subchunk", ctypes.c_uint64), ("stage_input", ctypes.c_int32),
-                ("dedisp_variant", ctypes.c_int32), ("nbits", ctypes.c_int32)]
+                ("dedisp_variant", ctypes.c_int32), ("nbits", ctypes.c_int32),
+                ("width_decimation", ctypes.c_int32), ("sigma_mode", ctypes.c_int32)]
 
 
 class PlanInfoC(ctypes.Structure):
@@ -198,6 +199,8 @@ def _desc_for(w, n_streams=None, chunk_len=None):
     d.chunk_len = int(chunk_len if chunk_len is not None else w.chunk_len)
     d.norm_block = int(getattr(w, "norm_block", 65536))
     d.nbits = int(getattr(w, "nbits", 8))
+    d.width_decimation = int(getattr(w, "wdec", 0))
+    d.sigma_mode = int(getattr(w, "sigma_mode", 0))
     d._keep = (ranges, widths)
     return d
 
@@ -255,6 +258,8 @@ class Plan:
         d.stage_input = 1 if stage_input else 0
         d.dedisp_variant = DEDISP_CHOICE[dedisp_variant] if isinstance(dedisp_variant, str) else int(dedisp_variant)
         d.nbits = int(getattr(w, "nbits", 8))
+        d.width_decimation = int(getattr(w, "wdec", 0))
+        d.sigma_mode = int(getattr(w, "sigma_mode", 0))
         self._arena = None
         self._streams = None
         if torch_resources:

@@ -201,10 +201,16 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
     p.row_bytes = (uint64_t)d->nchans * (uint64_t)p.nbits / 8;
     const uint64_t maxsample = (1ull << p.nbits) - 1;
 
+    if (d->width_decimation < 0 || d->sigma_mode < 0 || d->sigma_mode > 1) return AA_ERR_INVALID;
     for (int j = 0; j < d->nwidths; ++j) {
         if (p.widths[j] < 1 || (j && p.widths[j] <= p.widths[j - 1])) return AA_ERR_INVALID;
         p.wt.w[j] = p.widths[j];
+        int dec = 1;                                  // reading A20: the time grid of a width above wdec
+        if (d->width_decimation > 0)
+            while ((int64_t)p.widths[j] > (int64_t)d->width_decimation * dec) dec *= 2;
+        p.wt.dec[j] = dec;
     }
+    for (int j = d->nwidths; j < kMaxWidths; ++j) p.wt.dec[j] = 1;
     p.wmax = p.widths.back();
     if (p.wmax > 4096) return AA_ERR_INVALID;
 
@@ -302,6 +308,17 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         if (R.flush_ch < 2) return AA_ERR_INVALID;
         R.wide = (long double)maxsample * d->nchans * R.r.bin * p.wmax >= 4294967296.0L;
         R.small31 = (long double)maxsample * d->nchans * R.r.bin * p.wmax < 2147483648.0L;
+        if (d->sigma_mode) {
+            // per-width statistics live in the cluster kernel: block of 4 C segments of at most 16384 samples, C <= 8
+            const uint64_t bl = p.norm_block / (uint64_t)R.r.bin;
+            bool fits = !R.wide && !p.big && bl % 4 == 0;
+            if (fits) {
+                fits = false;
+                for (uint64_t C = 1; C <= 8 && bl % (4 * C) == 0; C *= 2)
+                    if (bl / C <= 16384) { fits = true; break; }
+            }
+            if (!fits) return AA_ERR_INVALID;
+        }
         if (R.in16) {
             auto it = std::find(p.bins.begin(), p.bins.end(), R.r.bin);
             if (it == p.bins.end()) { p.bins.push_back(R.r.bin); R.bin_slot = (int)p.bins.size() - 1; }
@@ -705,6 +722,7 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
                 sa.cands = S.d_cands;
                 sa.count = S.d_count;
                 sa.cap = (uint32_t)p->cap;
+                sa.sigma_mode = p->desc.sigma_mode;
                 AA_W(launch_sps(sa, p->wt, Rg.wide, Rg.small31, p->big, st));
                 S.sps_launches++;
                 AA_W(cudaEventRecord(e2, st));

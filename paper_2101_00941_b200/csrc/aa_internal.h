@@ -169,10 +169,11 @@ struct SpsArgs {
     aa_candidate *cands;
     uint32_t *count;
     uint32_t cap;
+    int32_t sigma_mode;    // 1: S/N from the statistics of each width's own boxcar series (reading A18; cluster kernel only)
 };
 
 constexpr int kMaxWidths = 32;
-struct WidthTable { int32_t w[kMaxWidths]; };
+struct WidthTable { int32_t w[kMaxWidths]; int32_t dec[kMaxWidths]; };   // widths and the time grid of each (A20)
 
 // ---- kernel launchers (each returns cudaGetLastError()) -------------------------------------
 // nbits 8: uint8 rows; 4: two samples per byte (even channel low), unpacked into the ring; 16: little-endian words,

@@ -48,6 +48,7 @@ struct Shared {
     double den[kMaxWidths];
     unsigned long long warp_tot[NT / 32];
     int w[kMaxWidths];        // widths (a dynamically indexed kernel parameter would go through the ADU pipe)
+    int dec[kMaxWidths];      // time grid of each width (reading A20): 1, or a power of two for widths above wdec
 };
 
 // BIG: the block's sum of squares may pass 2^64 (16-bit input on thousands of channels): every thread keeps its part
@@ -61,7 +62,7 @@ __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const __grid_c
 
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int d = blockIdx.y;
-    if (tid < kMaxWidths) sh.w[tid] = wt.w[tid];
+    if (tid < kMaxWidths) { sh.w[tid] = wt.w[tid]; sh.dec[tid] = wt.dec[tid]; }
     const int64_t b0 = (int64_t)blockIdx.x * a.block_len;
     int64_t b1 = b0 + a.block_len;
     if (b1 > a.nout_left) b1 = a.nout_left;
@@ -173,9 +174,10 @@ __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const __grid_c
             if (tau < e) {
                 const ACC p0 = P[tl];
                 bool any = false;
+                const uint32_t tabs = a.tau0 + (uint32_t)tau;          // absolute binned sample: the grids of A20 live on it
                 for (int j = 0; j < a.nwidths; ++j) {
                     const int w = sh.w[j];
-                    if (tau + w <= a.nout_left) {
+                    if (tau + w <= a.nout_left && (tabs & (uint32_t)(sh.dec[j] - 1)) == 0) {
                         const long long B = (long long)(ACC)(P[tl + w] - p0);
                         any |= (B >= sh.bthr[j]);
                     }
@@ -183,7 +185,7 @@ __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const __grid_c
                 if (any) {
                     for (int j = 0; j < a.nwidths; ++j) {
                         const int w = sh.w[j];
-                        if (tau + w > a.nout_left) continue;
+                        if (tau + w > a.nout_left || (tabs & (uint32_t)(sh.dec[j] - 1)) != 0) continue;
                         const long long B = (long long)(ACC)(P[tl + w] - p0);
                         const double num = __dsub_rn((double)B, __dmul_rn((double)w, mu));
                         const double S = __ddiv_rn(num, sh.den[j]);
@@ -234,19 +236,21 @@ constexpr int kSegMax = 16384;
 constexpr int kMaxCluster = 8;
 
 struct SharedC {
-    uint64_t red[3][NT2 / 32];
-    uint64_t part[4][kMaxCluster][3];   // [pass][rank] partial sums, written by the CTA of that rank
+    uint64_t red[5][NT2 / 32];
+    uint64_t part[2][kMaxCluster][4];   // [parity of the reduction][rank] partial sums, written by the CTA of that rank
     uint64_t bar;                       // mbarrier of the bulk load
     double mu, sigma;
     uint64_t m;
     uint32_t lo, hi;
     int empty;
     uint32_t thr_u[kMaxWidths];
-    double den[kMaxWidths];
+    double den[kMaxWidths];             // sigma sqrt(w) (A10) or the width's own sigma (A18)
+    double wmu[kMaxWidths];             // A18: the width's own mean
     int w[kMaxWidths];
+    int dec[kMaxWidths];
     uint32_t warp_tot[NT2 / 32];
-    uint2 wl[kMaxWidths];               // (width, pre-filter threshold): multiples of 4 first, then the others
-    int na, nu;
+    uint4 wl[kMaxWidths];               // (width, pre-filter threshold, grid, -): multiples of 4 first, then the others, then coarse grids
+    int na, nu, nd;
 };
 
 __device__ __forceinline__ bool clip_pred(double x, double mu, double lim)
@@ -290,7 +294,64 @@ __device__ __forceinline__ void st_cluster_u64(const void *local, uint32_t rank,
     asm volatile("st.shared::cluster.u64 [%0], %1;" ::"r"(r), "l"(v) : "memory");
 }
 
-// SMALL: every boxcar sum is below 2^31 (255 nchans bin wmax < 2^31), so the pre-filter B >= th is the sign of
+// Exact moments over the whole cluster.  Every thread brings its part (count, sum, sum of squares as low 64 bits plus
+// carries); the CTA's totals go to every CTA's shared memory (DSMEM), are added in rank order after a cluster barrier,
+// and mu = S1 / m, sigma = sqrt((m S2 - S1^2) / m^2) are formed from the 128-bit integers with one rounding each, so
+// all CTAs hold bit-identical values, equal to the oracle's.  `turn` alternates the DSMEM slot: the barrier of one
+// reduction separates the reads of the previous one from the writes of the next.  Returns the count.
+__device__ __forceinline__ uint64_t cluster_moments(SharedC &sh, int C, uint32_t rank, int &turn, uint64_t m, uint64_t S1, uint64_t S2,
+                                                    uint64_t carry, double &mu, double &sigma)
+{
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    m = warp_sum(m); S1 = warp_sum(S1);
+    const uint64_t lo = warp_sum(S2 & 0xFFFFFFFFull), hi = warp_sum(S2 >> 32);
+    carry = warp_sum(carry);
+    if (lane == 0) { sh.red[0][warp] = m; sh.red[1][warp] = S1; sh.red[2][warp] = lo; sh.red[3][warp] = hi; sh.red[4][warp] = carry; }
+    __syncthreads();
+    const int slot = turn & 1;
+    ++turn;
+    if (tid == 0) {
+        m = S1 = 0;
+        unsigned __int128 S2w = 0;
+        for (int w = 0; w < NT2 / 32; ++w) {
+            m += sh.red[0][w]; S1 += sh.red[1][w];
+            S2w += (unsigned __int128)sh.red[2][w] + ((unsigned __int128)sh.red[3][w] << 32) + ((unsigned __int128)sh.red[4][w] << 64);
+        }
+        if (C > 1) {
+            for (int r = 0; r < C; ++r) {
+                st_cluster_u64(&sh.part[slot][rank][0], (uint32_t)r, m);
+                st_cluster_u64(&sh.part[slot][rank][1], (uint32_t)r, S1);
+                st_cluster_u64(&sh.part[slot][rank][2], (uint32_t)r, (uint64_t)S2w);
+                st_cluster_u64(&sh.part[slot][rank][3], (uint32_t)r, (uint64_t)(S2w >> 64));
+            }
+        } else {
+            sh.part[slot][0][0] = m; sh.part[slot][0][1] = S1; sh.part[slot][0][2] = (uint64_t)S2w; sh.part[slot][0][3] = (uint64_t)(S2w >> 64);
+        }
+    }
+    if (C > 1) cluster_sync_all(); else __syncthreads();
+    if (tid == 0) {
+        m = S1 = 0;
+        unsigned __int128 S2w = 0;
+        for (int r = 0; r < C; ++r) {
+            m += sh.part[slot][r][0]; S1 += sh.part[slot][r][1];
+            S2w += (unsigned __int128)sh.part[slot][r][2] + ((unsigned __int128)sh.part[slot][r][3] << 64);
+        }
+        sh.m = m;
+        if (m) {
+            const unsigned __int128 N = (unsigned __int128)m * S2w - (unsigned __int128)S1 * S1;
+            const double dm = __ull2double_rn(m);
+            sh.mu = __ddiv_rn(__ull2double_rn(S1), dm);
+            sh.sigma = __dsqrt_rn(__ddiv_rn(u128_to_double(N), __dmul_rn(dm, dm)));
+        }
+    }
+    __syncthreads();
+    const uint64_t msel = sh.m;
+    if (msel) { mu = sh.mu; sigma = sh.sigma; }
+    __syncthreads();
+    return msel;
+}
+
+// SMALL: every boxcar sum is below 2^31 (maxsample nchans bin wmax < 2^31), so the pre-filter B >= th is the sign of
 // (th - 1) - B and costs one 3-input add and one OR per (tau, width).
 template <bool SMALL>
 __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const __grid_constant__ WidthTable wt, const int C, const int seg)
@@ -303,7 +364,7 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
     const int d = blockIdx.y;
     const uint32_t rank = C > 1 ? cluster_rank() : 0u;
     const int64_t blk = blockIdx.x / C;
-    if (tid < kMaxWidths) sh.w[tid] = wt.w[tid];
+    if (tid < kMaxWidths) { sh.w[tid] = wt.w[tid]; sh.dec[tid] = wt.dec[tid]; }
     const int64_t b0 = blk * a.block_len;
     int64_t b1 = b0 + a.block_len;
     if (b1 > a.nout_left) b1 = a.nout_left;
@@ -319,6 +380,7 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
     int64_t n_own = b1 - s0;                             // columns of the block inside the segment
     if (n_own > seg) n_own = seg;
     if (n_own < 0) n_own = 0;
+    const bool measured = a.sigma_mode != 0;             // reading A18
 
     // ---- load -------------------------------------------------------------------------------
     const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&sh.bar);
@@ -349,8 +411,9 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
                 : "memory");
     }
 
-    // ---- 1. statistics --------------------------------------------------------------------------
+    // ---- 1. statistics of the block (A8) -------------------------------------------------------
     double mu = 0.0, sigma = 0.0;
+    int turn = 0;
     const int n4 = (int)(n_own / 4);
     for (int pass = 0; pass < 4; ++pass) {
         uint32_t lo = 0u, span = 0xFFFFFFFFu;
@@ -411,70 +474,12 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
             }
             m = mc;
         }
-        m = warp_sum(m); S1 = warp_sum(S1); S2 = warp_sum(S2);
-        if (lane == 0) { sh.red[0][warp] = m; sh.red[1][warp] = S1; sh.red[2][warp] = S2; }
-        __syncthreads();
-        if (tid == 0) {
-            m = S1 = S2 = 0;
-            for (int w = 0; w < NT2 / 32; ++w) { m += sh.red[0][w]; S1 += sh.red[1][w]; S2 += sh.red[2][w]; }
-            if (C > 1) {
-                for (int r = 0; r < C; ++r) {
-                    st_cluster_u64(&sh.part[pass][rank][0], (uint32_t)r, m);
-                    st_cluster_u64(&sh.part[pass][rank][1], (uint32_t)r, S1);
-                    st_cluster_u64(&sh.part[pass][rank][2], (uint32_t)r, S2);
-                }
-            } else {
-                sh.part[pass][0][0] = m; sh.part[pass][0][1] = S1; sh.part[pass][0][2] = S2;
-            }
-        }
-        if (C > 1) cluster_sync_all(); else __syncthreads();
-        if (tid == 0) {
-            m = S1 = S2 = 0;
-            for (int r = 0; r < C; ++r) { m += sh.part[pass][r][0]; S1 += sh.part[pass][r][1]; S2 += sh.part[pass][r][2]; }
-            sh.m = m;
-            if (m) {
-                const unsigned __int128 N = (unsigned __int128)m * S2 - (unsigned __int128)S1 * S1;
-                const double dm = __ull2double_rn(m);
-                sh.mu = __ddiv_rn(__ull2double_rn(S1), dm);
-                sh.sigma = __dsqrt_rn(__ddiv_rn(u128_to_double(N), __dmul_rn(dm, dm)));
-            }
-        }
-        __syncthreads();
-        const uint64_t msel = sh.m;
-        if (msel) { mu = sh.mu; sigma = sh.sigma; }
-        __syncthreads();
-        if (!msel) break;
+        // (the launcher sends blocks whose sum of squares could pass 2^64 to the generic kernel: no carries here)
+        if (!cluster_moments(sh, C, rank, turn, m, S1, S2, 0, mu, sigma)) break;
     }
     if (!(sigma > 0.0) || n_k < 32) return;
 
-    // ---- 2. per-width constants ---------------------------------------------------------------
-    if (tid < a.nwidths) {
-        const double w = (double)sh.w[tid];
-        const double den = __dmul_rn(sigma, __dsqrt_rn(w));
-        sh.den[tid] = den;
-        // B >= floor(w mu + thr sigma sqrt w) - 1 is necessary for S >= thr; clamped to the 32-bit sums
-        const long long bt = __double2ll_rd(w * mu + a.thr * den) - 1;
-        sh.thr_u[tid] = bt <= 0 ? 0u : (bt >= 0xFFFFFFFFll ? 0xFFFFFFFFu : (uint32_t)bt);
-    }
-    __syncthreads();
-    if (tid == 0) {
-        // SMALL: th - 1 as a signed number, B >= th  <=>  (th - 1) - B < 0; th above every possible B -> never
-        auto enc = [&](uint32_t th) { return SMALL ? (th == 0u ? 0xFFFFFFFFu : (th > 0x7FFFFFFFu ? 0x7FFFFFFFu : th - 1u)) : th; };
-        int n = 0;
-        for (int j = 0; j < a.nwidths; ++j)
-            if ((sh.w[j] & 3) == 0) sh.wl[n++] = make_uint2((uint32_t)sh.w[j], enc(sh.thr_u[j]));
-        sh.na = n;
-        for (int j = 0; j < a.nwidths; ++j)
-            if ((sh.w[j] & 3) != 0) sh.wl[n++] = make_uint2((uint32_t)sh.w[j], enc(sh.thr_u[j]));
-        sh.nu = n - sh.na;
-    }
-
-    int64_t e = b1 < a.nemit ? b1 : (int64_t)a.nemit;     // taus [b0, e) of the block may emit
-    int64_t n_emit = e - s0;                              // ... [0, n_emit) of this segment
-    if (n_emit > seg) n_emit = seg;
-    if (n_emit <= 0) return;                              // nothing after this point is cluster-wide
-
-    // ---- 3. exclusive prefix sums in place: X[i] <- sum_{j<i} X[j], i <= n_in; constant beyond ------
+    // ---- 2. exclusive prefix sums in place: X[i] <- sum_{j<i} X[j], i <= n_in; constant beyond ------
     {
         const int total = seg + halo + 8;                 // slots the boxcar loop may read
         int chunk = (int)((n_in + 1 + NT2 - 1) / NT2);    // slots 0 .. n_in
@@ -526,10 +531,95 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
         __syncthreads();
     }
 
+    // ---- 3. per-width constants ---------------------------------------------------------------
+    const uint32_t tabs0 = a.tau0 + (uint32_t)s0;          // absolute binned sample of X[0]: a multiple of 4
+    if (measured) {
+        // reading A18: the robust statistics (A8) of each width's own boxcar series over the block, on the width's
+        // grid (A20), from the prefix sums: B = X[t + w] - X[t] (exact modulo 2^32: every sum is below 2^32)
+        for (int j = 0; j < a.nwidths; ++j) {
+            const int w = sh.w[j];
+            const uint32_t gm = (uint32_t)(sh.dec[j] - 1);
+            int64_t nv = a.nout_left - s0 - w + 1;        // columns t of this segment with t + w <= nout
+            if (nv > n_own) nv = n_own;
+            double wm = 0.0, ws = 0.0;
+            uint64_t cnt0 = 0;
+            for (int pass = 0; pass < 4; ++pass) {
+                uint32_t lo = 0u, span = 0xFFFFFFFFu;
+                bool run = true;
+                if (pass > 0) {
+                    if (tid == 0) {
+                        uint32_t l = 0, h = 0;
+                        sh.empty = clip_interval(wm, __dmul_rn(3.0, ws), l, h) ? 0 : 1;
+                        sh.lo = l;
+                        sh.hi = h;
+                    }
+                    __syncthreads();
+                    run = !sh.empty;
+                    lo = sh.lo;
+                    span = sh.hi - lo;
+                }
+                uint64_t m = 0, S1 = 0, S2 = 0, carry = 0;
+                if (run) {
+                    for (int64_t t = tid; t < nv; t += NT2) {
+                        if ((tabs0 + (uint32_t)t) & gm) continue;
+                        const uint32_t B = X[t + w] - X[t];
+                        if ((B - lo) <= span) {
+                            m += 1;
+                            S1 += B;
+                            const uint64_t sq = (uint64_t)B * B;
+                            S2 += sq;
+                            carry += S2 < sq;
+                        }
+                    }
+                }
+                const uint64_t got = cluster_moments(sh, C, rank, turn, m, S1, S2, carry, wm, ws);
+                if (pass == 0) cnt0 = got;
+                if (!got || cnt0 < 32) break;              // uniform over the cluster
+            }
+            if (tid == 0) {
+                const bool ok = cnt0 >= 32 && ws > 0.0;
+                sh.wmu[j] = wm;
+                sh.den[j] = ok ? ws : 0.0;
+                // B >= floor(mu_w + thr sigma_w) - 1 is necessary for S >= thr; a width without statistics never hits
+                const long long bt = ok ? __double2ll_rd(wm + a.thr * ws) - 1 : 0x7FFFFFFFFFFFll;
+                sh.thr_u[j] = bt <= 0 ? 0u : (bt >= 0xFFFFFFFFll ? 0xFFFFFFFFu : (uint32_t)bt);
+            }
+        }
+        __syncthreads();
+    } else {
+        if (tid < a.nwidths) {
+            const double w = (double)sh.w[tid];
+            const double den = __dmul_rn(sigma, __dsqrt_rn(w));
+            sh.den[tid] = den;
+            // B >= floor(w mu + thr sigma sqrt w) - 1 is necessary for S >= thr; clamped to the 32-bit sums
+            const long long bt = __double2ll_rd(w * mu + a.thr * den) - 1;
+            sh.thr_u[tid] = bt <= 0 ? 0u : (bt >= 0xFFFFFFFFll ? 0xFFFFFFFFu : (uint32_t)bt);
+        }
+        __syncthreads();
+    }
+    if (tid == 0) {
+        // SMALL: th - 1 as a signed number, B >= th  <=>  (th - 1) - B < 0; th above every possible B -> never
+        auto enc = [&](uint32_t th) { return SMALL ? (th == 0u ? 0xFFFFFFFFu : (th > 0x7FFFFFFFu ? 0x7FFFFFFFu : th - 1u)) : th; };
+        int n = 0;
+        for (int j = 0; j < a.nwidths; ++j)
+            if (sh.dec[j] == 1 && (sh.w[j] & 3) == 0) sh.wl[n++] = make_uint4((uint32_t)sh.w[j], enc(sh.thr_u[j]), 1u, 0u);
+        sh.na = n;
+        for (int j = 0; j < a.nwidths; ++j)
+            if (sh.dec[j] == 1 && (sh.w[j] & 3) != 0) sh.wl[n++] = make_uint4((uint32_t)sh.w[j], enc(sh.thr_u[j]), 1u, 0u);
+        sh.nu = n - sh.na;
+        for (int j = 0; j < a.nwidths; ++j)
+            if (sh.dec[j] > 1) sh.wl[n++] = make_uint4((uint32_t)sh.w[j], enc(sh.thr_u[j]), (uint32_t)sh.dec[j], 0u);
+        sh.nd = n - sh.na - sh.nu;
+    }
+    __syncthreads();
+
+    const int64_t n_emit = n_own;                         // taus [0, n_emit) of this segment may emit (blocks tile the sub-chunk)
+    if (n_emit <= 0) return;                              // nothing after this point is cluster-wide
+
     // ---- 4. boxcars, eight taus per thread -----------------------------------------------------------
     // (two groups of four, NT2 groups apart, so that every 16-byte access of a warp is contiguous)
     const int ngroups = (int)((n_emit + 3) / 4);
-    const int nw = a.nwidths, na = sh.na, nu = sh.nu;
+    const int nw = a.nwidths, na = sh.na, nu = sh.nu, nd = sh.nd;
     constexpr int GB = 4 * NT2;                          // distance of the second group in samples
     for (int g0 = 0; g0 < ngroups; g0 += 2 * NT2) {
         const int g = g0 + tid;
@@ -543,7 +633,7 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
             // widths that are multiples of 4: aligned 16-byte loads
 #pragma unroll 2
             for (int j = 0; j < na; ++j) {
-                const uint2 wt2 = sh.wl[j];
+                const uint4 wt2 = sh.wl[j];
                 const uint32_t th = wt2.y;
                 const uint4 qa = *reinterpret_cast<const uint4 *>(xg + wt2.x);
                 const uint4 qb = *reinterpret_cast<const uint4 *>(xg + wt2.x + gb);
@@ -559,7 +649,7 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
             // the others: the aligned pieces around tau + w, shifted by w mod 4 (uniform)
 #pragma unroll 1
             for (int j = na; j < na + nu; ++j) {
-                const uint2 wt2 = sh.wl[j];
+                const uint4 wt2 = sh.wl[j];
                 const uint32_t th = wt2.y;
                 const int r = (int)(wt2.x & 3u);
                 const uint32_t *xq = xg + (wt2.x - (uint32_t)r);
@@ -578,6 +668,29 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
                        ((v3 - pa.w) >= th ? 8u : 0u) | ((v4 - pb.x) >= th ? 16u : 0u) | ((v5 - pb.y) >= th ? 32u : 0u) |
                        ((v6 - pb.z) >= th ? 64u : 0u) | ((v7 - pb.w) >= th ? 128u : 0u);
             }
+            // widths on a coarser grid (A20): grid 2 looks at taus 0 and 2 of a group, grid 4 and beyond at tau 0, and
+            // only in the groups that start on the grid (tabs0 and GB are multiples of 4 and of every grid up to 1024)
+#pragma unroll 1
+            for (int j = na + nu; j < na + nu + nd; ++j) {
+                const uint4 wt2 = sh.wl[j];
+                const uint32_t th = wt2.y, grid = wt2.z;
+                const uint32_t ga = tabs0 + 4u * (uint32_t)g;
+                const bool ok_a = grid <= 4u || !(ga & (grid - 1u)), ok_b = grid <= 4u || !((ga + (uint32_t)gb) & (grid - 1u));
+                if (!ok_a && !ok_b) continue;
+                const uint32_t *xq = xg + wt2.x;
+                const uint32_t a0 = xq[0], b0 = xq[gb];
+                if (SMALL) {
+                    if (ok_a) f0 |= th + pa.x - a0;
+                    if (ok_b) f4 |= th + pb.x - b0;
+                } else {
+                    any |= (ok_a && (a0 - pa.x) >= th ? 1u : 0u) | (ok_b && (b0 - pb.x) >= th ? 16u : 0u);
+                }
+                if (grid == 2u) {
+                    const uint32_t a2 = xq[2], b2 = xq[gb + 2];
+                    if (SMALL) { f2 |= th + pa.z - a2; f6 |= th + pb.z - b2; }
+                    else any |= ((a2 - pa.z) >= th ? 4u : 0u) | ((b2 - pb.z) >= th ? 64u : 0u);
+                }
+            }
         }
         if (SMALL)
             any = (f0 >> 31) | (f1 >> 31) << 1 | (f2 >> 31) << 2 | (f3 >> 31) << 3 | (f4 >> 31) << 4 | (f5 >> 31) << 5 |
@@ -594,12 +707,19 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
             double best = 0.0;
             if (((any >> k) & 1u) && tl < n_emit) {
                 const uint32_t p0 = X[tl];
+                const uint32_t tabs = tabs0 + (uint32_t)tl;
                 for (int j = 0; j < nw; ++j) {
                     const int w = sh.w[j];
-                    if (tau + w > a.nout_left) continue;
+                    if (tau + w > a.nout_left || (tabs & (uint32_t)(sh.dec[j] - 1))) continue;
                     const long long B = (long long)(uint32_t)(X[tl + w] - p0);
-                    const double num = __dsub_rn((double)B, __dmul_rn((double)w, mu));
-                    const double S = __ddiv_rn(num, sh.den[j]);
+                    double S;
+                    if (measured) {
+                        const double sg = sh.den[j];
+                        if (!(sg > 0.0)) continue;
+                        S = __ddiv_rn(__dsub_rn((double)B, sh.wmu[j]), sg);
+                    } else {
+                        S = __ddiv_rn(__dsub_rn((double)B, __dmul_rn((double)w, mu)), sh.den[j]);
+                    }
                     if (best_w == 0 || S > best) { best = S; best_w = w; }
                 }
                 has = (best_w != 0) && (best >= a.thr);

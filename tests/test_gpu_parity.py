@@ -186,6 +186,36 @@ def test_other_input_bit_depths(B, nbits, case):
     assert len(ref) > 0
 
 
+@pytest.mark.parametrize("case", [
+    dict(wdec=2),                                                                        # plain shapes, generic SPS kernel (block 1024 = 4 * 256: cluster of 1)
+    dict(wdec=1, widths=(1, 2, 3, 8, 32), thr=4.0),
+    dict(wdec=4, widths=(1, 2, 4, 8, 16, 32, 64), norm_block=65536, chunk_len=65536, nsamp=200001, ndms=5),     # cluster of 4, grids up to 16
+    dict(wdec=2, widths=(2, 6, 7, 12, 20, 33), thr=4.5, norm_block=4096, chunk_len=8192),  # unaligned widths on coarse grids
+    dict(wdec=1, widths=(1, 2, 4, 4096), bins=(4,), nchans=20, nsamp=120000, chunk_len=32768, norm_block=32768, ndms=6, thr=4.0),  # grid 4096 > the group distance
+    dict(wdec=8, bins=(8,), norm_block=1040, chunk_len=8 * 1040, nsamp=50000, ndms=12, widths=(1, 4, 16, 32)),   # generic kernel (block of 130)
+    dict(sigma_mode=1),
+    dict(sigma_mode=1, wdec=2, widths=(1, 2, 4, 8, 16, 32), norm_block=4096, chunk_len=8192),
+    dict(sigma_mode=1, norm_block=65536, chunk_len=65536, nsamp=200001, ndms=5, widths=(1, 2, 4, 8, 16, 32, 64, 128)),   # cluster of 4, ragged last block
+    dict(sigma_mode=1, wdec=4, norm_block=131072, chunk_len=131072, nsamp=300000, ndms=4, widths=(1, 3, 8, 64)),        # cluster of 8
+    dict(sigma_mode=1, bins=(1, 2, 4), nsamp=40000, chunk_len=8192, n_streams=2),
+    dict(sigma_mode=1, nchans=302, ndms=100, nsamp=21000, chunk_len=8192, foff=-0.5, dm_step=0.25, norm_block=1024, n_streams=2),
+])
+def test_search_variants_a18_a20(B, case):
+    """Readings A20 (long boxcars on a coarser time grid) and A18 (S/N from each width's own statistics) against the
+    oracle: dense plane bit for bit, candidates under the north_star tolerances."""
+    case = dict(case)
+    wdec, sm = case.pop("wdec", 0), case.pop("sigma_mode", 0)
+    w = I.scaled(_tiny(**case), wdec=wdec, sigma_mode=sm)
+    cands, ref, res = _check_against_oracle(B, w)
+    assert res["only_gpu"] == 0 and res["only_oracle"] == 0 and res["width_ties"] == 0
+    assert len(ref) > 0
+
+
+def test_measured_sigma_needs_cluster_sized_blocks(B):
+    with pytest.raises(B.AAError):
+        B.Plan(I.scaled(_tiny(bins=(8,), norm_block=1040, chunk_len=8 * 1040, nsamp=50000), sigma_mode=1))   # block of 130 samples
+
+
 def test_saturated_16_bit_input(B):
     w = I.scaled(_tiny(nchans=1024, ndms=70, nsamp=9000, chunk_len=4096, f_top=1500.0, foff=-0.2, dm_step=0.25, norm_block=1024), nbits=16)
     buf = B.pinned_empty(w.nbytes)
