@@ -271,6 +271,13 @@ def run_config(B, k, steps, warmup, link_gbs, max_cands=1 << 24):
         step_s, st = leg(plan, step, steps)
         units = plan.info["dm_trial_samples"]
         variants = [plan.dedisp_variant(r) for r in range(len(w.ranges))]
+    # the same run with the lists thinned on the device (output_mode 1, reading A17): only peaks cross the link
+    with B.Plan(w, peaks=True) as plan:
+        def step_pk():
+            last["p"], _ = plan.run(host, max_cands=max_cands, want_taps=False)
+        pk_s, st_pk = leg(plan, step_pk, max(1, steps - 1))
+    out["peaks_mode"] = {"ms_per_step": 1e3 * pk_s, "peaks": int(len(last["p"])), "d2h_bytes_per_step": st_pk["d2h_bytes"],
+                         "sort_ms": st_pk["sort_ms"], "candidates_mode": {"d2h_bytes_per_step": st["d2h_bytes"], "sort_ms": st["sort_ms"]}}
     # the two things the end-to-end run overlaps, each alone: the copy of the observation, and the kernels on resident data
     dev_in = torch.empty(w.nbytes, dtype=torch.uint8, device="cuda")
     torch.cuda.synchronize()

@@ -123,6 +123,12 @@ typedef struct {
      * cluster kernel takes (block / bin a multiple of 4, at most 131072 binned samples, 32-bit boxcar sums):
      * AA_ERR_INVALID otherwise. */
     int32_t  sigma_mode;
+    /* 0 = aa_run returns every candidate (one per (DM, time), reading A11; BASELINE.json).  1 = it returns the PEAKS of
+     * that list (reading A17, the rule of aa_find_peaks): each sub-chunk's list is thinned on the device before it
+     * crosses the host link (kernels_peaks.cu), candidates whose neighbourhood reaches into an adjacent sub-chunk are
+     * settled by the host on the merged list; the result is exactly aa_find_peaks of the full list.  *n_cands and
+     * aa_stats.n_peaks then count peaks, aa_stats.n_candidates still counts the candidates found on the device. */
+    int32_t  output_mode;
 } aa_plan_desc;
 
 typedef struct {
@@ -154,6 +160,7 @@ typedef struct {
     int32_t  n_streams;
     uint64_t h2h_bytes;         /* aa_run_staged: bytes copied host -> pinned staging by the stream threads */
     double   h2h_ms;            /* ... and the time those copies took, summed over threads */
+    uint64_t n_peaks;           /* output_mode 1: peaks returned (0 otherwise) */
 } aa_stats;
 
 /* Device timeline of one sub-chunk of the last run, in milliseconds after the start of the run (CUDA events

@@ -57,6 +57,8 @@ def _load():
         lib.aaor_sps_row2.argtypes = [vp, u64, u64, u64, u64, vp, i32, dbl, u64, u64, i32, i32, vp, vp, vp, i64]
         lib.aaor_series_stats.restype = None
         lib.aaor_series_stats.argtypes = [vp, u64, vp, vp, vp]
+        lib.aaor_find_peaks.restype = None
+        lib.aaor_find_peaks.argtypes = [vp, i64, vp]
         lib.aaor_num_threads.restype = i32
         _lib = lib
     return _lib
@@ -218,6 +220,17 @@ def find_peaks(cands: np.ndarray) -> np.ndarray:
         if np.any(nb & beats):
             keep[i] = False
     return cands[keep]
+
+
+def find_peaks_fast(cands: np.ndarray) -> np.ndarray:
+    """find_peaks for long lists (sorted by (dm_index, t_start)): the same rule with the pairs that cannot be
+    neighbours left out (aaor_find_peaks).  Pinned to the all-pairs `find_peaks` on random lists."""
+    cands = np.ascontiguousarray(cands, dtype=CAND_DTYPE)
+    key = (cands["dm_index"].astype(np.uint64) << np.uint64(32)) | cands["t_start"].astype(np.uint64)
+    assert np.all(np.diff(key.astype(np.int64)) >= 0), "list must be sorted by (dm_index, t_start)"
+    keep = np.empty(len(cands), dtype=np.uint8)
+    _load().aaor_find_peaks(cands.ctypes.data, len(cands), keep.ctypes.data)
+    return cands[keep.astype(bool)]
 
 
 def run(x: np.ndarray, w, *, keep_dense: bool = False, row_subset: Optional[Dict[int, Sequence[int]]] = None,

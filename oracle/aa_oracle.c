@@ -283,6 +283,43 @@ int64_t aaor_sps_row(const uint32_t *d, uint64_t d_first, uint64_t d_count,
     return aaor_sps_row2(d, d_first, d_count, nout, L, widths, nwidths, thr, tau_a, tau_b, 0, 0, out_tau, out_w, out_snr, max_out);
 }
 
+/* ---- peak finding (reading A17) on a list sorted by (dm_index, t_start) ------------------------------------
+ * keep[i] = 1 iff no neighbour beats candidate i.  Neighbours: |dm' - dm| <= 1 and the boxcars overlap or touch in
+ * raw samples (t' <= t + w and t <= t' + w').  c' beats c iff snr' > snr, or snr' == snr and (dm', t') < (dm, t).
+ * The definition is the all-pairs loop of oracle.find_peaks (python); this is the same test with the pairs that cannot
+ * be neighbours left out: other rows than dm-1, dm, dm+1, and starts outside [t - wmax, t + w] (wmax = the largest
+ * width in the list).  Pinned against the all-pairs loop on random lists. */
+typedef struct { uint32_t dm_index, t_start, width; float snr; } aaor_cand;
+
+void aaor_find_peaks(const aaor_cand *c, int64_t n, uint8_t *keep)
+{
+    uint64_t wmax = 0;
+    for (int64_t i = 0; i < n; ++i) if (c[i].width > wmax) wmax = c[i].width;
+    #pragma omp parallel for schedule(dynamic, 1024)
+    for (int64_t i = 0; i < n; ++i) {
+        keep[i] = 1;
+        for (int dd = -1; dd <= 1 && keep[i]; ++dd) {
+            int64_t dm = (int64_t)c[i].dm_index + dd;
+            if (dm < 0) continue;
+            int64_t t_lo = (int64_t)c[i].t_start - (int64_t)wmax, t_hi = (int64_t)c[i].t_start + (int64_t)c[i].width;
+            /* first record with (dm_index, t_start) >= (dm, t_lo) */
+            int64_t a = 0, b = n;
+            while (a < b) {
+                int64_t m = (a + b) / 2;
+                if ((int64_t)c[m].dm_index < dm || ((int64_t)c[m].dm_index == dm && (int64_t)c[m].t_start < t_lo)) a = m + 1; else b = m;
+            }
+            for (int64_t j = a; j < n && (int64_t)c[j].dm_index == dm && (int64_t)c[j].t_start <= t_hi; ++j) {
+                if (j == i) continue;
+                if ((int64_t)c[i].t_start > (int64_t)c[j].t_start + (int64_t)c[j].width) continue;      /* not touching */
+                int beats = c[j].snr > c[i].snr ||
+                            (c[j].snr == c[i].snr && (c[j].dm_index < c[i].dm_index ||
+                                                      (c[j].dm_index == c[i].dm_index && c[j].t_start < c[i].t_start)));
+                if (beats) { keep[i] = 0; break; }
+            }
+        }
+    }
+}
+
 int aaor_num_threads(void)
 {
     int n = 1;

@@ -46,7 +46,7 @@ class PlanDescC(ctypes.Structure):
                 ("ntap", ctypes.c_int32), ("tap_dm_indices", ctypes.POINTER(ctypes.c_uint32)),
                 ("max_cands_per_subchunk", ctypes.c_uint64), ("stage_input", ctypes.c_int32),
                 ("dedisp_variant", ctypes.c_int32), ("nbits", ctypes.c_int32),
-                ("width_decimation", ctypes.c_int32), ("sigma_mode", ctypes.c_int32)]
+                ("width_decimation", ctypes.c_int32), ("sigma_mode", ctypes.c_int32), ("output_mode", ctypes.c_int32)]
 
 
 class PlanInfoC(ctypes.Structure):
@@ -72,7 +72,7 @@ class StatsC(ctypes.Structure):
                 ("dedisp_launches", ctypes.c_uint64), ("sps_launches", ctypes.c_uint64),
                 ("prep_launches", ctypes.c_uint64), ("n_candidates", ctypes.c_uint64), ("n_stored", ctypes.c_uint64),
                 ("overflow", ctypes.c_int32), ("n_streams", ctypes.c_int32),
-                ("h2h_bytes", ctypes.c_uint64), ("h2h_ms", ctypes.c_double)]
+                ("h2h_bytes", ctypes.c_uint64), ("h2h_ms", ctypes.c_double), ("n_peaks", ctypes.c_uint64)]
 
 
 class SubchunkTimesC(ctypes.Structure):
@@ -233,7 +233,7 @@ class Plan:
 
     def __init__(self, w, *, n_streams: Optional[int] = None, chunk_len: Optional[int] = None,
                  taps: Optional[Sequence[int]] = None, max_cands_per_subchunk: int = 0,
-                 torch_resources: bool = True, stage_input: bool = False, dedisp_variant="auto"):
+                 torch_resources: bool = True, stage_input: bool = False, dedisp_variant="auto", peaks: bool = False):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the path has no CPU fallback")
@@ -260,6 +260,7 @@ class Plan:
         d.nbits = int(getattr(w, "nbits", 8))
         d.width_decimation = int(getattr(w, "wdec", 0))
         d.sigma_mode = int(getattr(w, "sigma_mode", 0))
+        d.output_mode = 1 if peaks else 0
         self._arena = None
         self._streams = None
         if torch_resources:

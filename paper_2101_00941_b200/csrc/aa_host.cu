@@ -67,7 +67,7 @@ struct Range {
     std::vector<std::pair<int, int>> taps;   // (local dm, tap row)
 };
 
-constexpr int kEvFixed = 7;     // h2d0 h2d1 ct1 bin0 bin1 list0 list1
+constexpr int kEvFixed = 9;     // h2d0 h2d1 ct1 bin0 bin1 list0 list1 peaks0 peaks1
 
 struct Stream {
     cudaStream_t st = nullptr;
@@ -77,7 +77,10 @@ struct Stream {
     uint32_t *d_D = nullptr;
     uint32_t *d_D2 = nullptr;         // 16-bit input: dedispersed high-byte plane of the current range
     aa_candidate *d_cands = nullptr;
-    uint32_t *d_count = nullptr;
+    uint32_t *d_count = nullptr;      // [0] candidates found, [1] records of the thinned list (output_mode 1)
+    int32_t *d_head = nullptr;        // output_mode 1: bucket grid, chain and thinned list of the peak kernels
+    uint32_t *d_next = nullptr;
+    aa_candidate *d_peaks = nullptr;
     uint32_t *h_count = nullptr;      // pinned
     aa_candidate *h_cands = nullptr;  // pinned
     uint32_t *h_tap = nullptr;        // pinned
@@ -108,6 +111,10 @@ struct aa_plan {
     int nbits = 8, planes = 1;        // planes: 8-bit planes the input is processed as (2 for 16-bit samples)
     uint64_t row_bytes = 0;           // bytes of one input time sample (all channels)
     bool big = false;                 // a block's sum of squares may pass 2^63: 128-bit statistics
+    bool peaks = false;               // output_mode 1: lists are thinned on the device (reading A17)
+    int pk_shift = 5, pk_nbk = 1;     // bucket grid of the peak kernels: 2^shift raw samples per bucket, buckets per row
+    uint32_t wmax_raw = 1;            // longest boxcar in raw samples
+    std::atomic<uint64_t> total_raw{0};
     int n_streams = 1;
     uint64_t arena_bytes = 0, pinned_bytes = 0;
     void *arena = nullptr;
@@ -436,6 +443,15 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
     }
     p.cap = d->max_cands_per_subchunk ? d->max_cands_per_subchunk : (1ull << 21);
     if (p.cap > (1ull << 30)) return AA_ERR_INVALID;
+    if (d->output_mode < 0 || d->output_mode > 1) return AA_ERR_INVALID;
+    p.peaks = d->output_mode == 1;
+    p.wmax_raw = (uint32_t)p.wmax * (uint32_t)bin_max;
+    p.pk_shift = 5;
+    while (((p.L - 1) >> p.pk_shift) + 1 > 4096) ++p.pk_shift;
+    p.pk_nbk = (int)(((p.L - 1) >> p.pk_shift) + 1);
+    uint64_t ndms_all = 0;
+    for (auto &R : p.ranges) ndms_all += (uint64_t)R.r.ndms;
+    if (ndms_all >= (1ull << 30)) return AA_ERR_INVALID;       // the two top bits of dm_index carry the peak flags
 
     // arena layout (256-byte aligned bump allocation, computed identically in carve())
     uint64_t off = 0;
@@ -455,6 +471,11 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         if (p.planes == 2) take(p.d_rows * p.pitchD * 4);
         take(p.cap * sizeof(aa_candidate));
         take(256);
+        if (p.peaks) {
+            take(ndms_all * (uint64_t)p.pk_nbk * 4);
+            take(p.cap * 4);
+            take(p.cap * sizeof(aa_candidate));
+        }
     }
     p.arena_bytes = round_up(off, 256);
     p.pinned_bytes = (uint64_t)p.n_streams * (256 + p.cap * sizeof(aa_candidate) + p.tap_stage_elems * 4 +
@@ -485,6 +506,13 @@ void carve(aa_plan &p)
         if (p.planes == 2) S.d_D2 = reinterpret_cast<uint32_t *>(take(p.d_rows * p.pitchD * 4));
         S.d_cands = reinterpret_cast<aa_candidate *>(take(p.cap * sizeof(aa_candidate)));
         S.d_count = reinterpret_cast<uint32_t *>(take(256));
+        if (p.peaks) {
+            uint64_t ndms_all = 0;
+            for (auto &R : p.ranges) ndms_all += (uint64_t)R.r.ndms;
+            S.d_head = reinterpret_cast<int32_t *>(take(ndms_all * (uint64_t)p.pk_nbk * 4));
+            S.d_next = reinterpret_cast<uint32_t *>(take(p.cap * 4));
+            S.d_peaks = reinterpret_cast<aa_candidate *>(take(p.cap * sizeof(aa_candidate)));
+        }
     }
 }
 
@@ -524,6 +552,13 @@ void destroy_plan(aa_plan *p)
     if (p->ev_start) cudaEventDestroy(p->ev_start);
     if (p->own_arena && p->arena) cudaFree(p->arena);
     delete p;
+}
+
+// order of the returned list: (dm_index, t_start); the two top bits of dm_index may carry peak flags on the way
+inline bool cand_less(const aa_candidate &a, const aa_candidate &b)
+{
+    const uint32_t da = a.dm_index & kPeakDmMask, db = b.dm_index & kPeakDmMask;
+    return da != db ? da < db : a.t_start < b.t_start;
 }
 
 inline bool wait_flag(aa_plan *p, std::atomic<int> &f)
@@ -750,7 +785,22 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
                 }
             }
         }
-        AA_W(cudaMemcpyAsync(S.h_count, S.d_count, sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
+        AA_W(cudaEventRecord(S.ev[7], st));
+        if (p->peaks) {
+            // thin the sub-chunk's list on the device: only peaks and border records cross the link (reading A17)
+            PeakArgs pa{};
+            pa.cands = S.d_cands; pa.count = S.d_count; pa.cap = (uint32_t)p->cap;
+            pa.head = S.d_head; pa.next = S.d_next;
+            pa.nrows = (int32_t)p->ndms_total; pa.nbk = p->pk_nbk; pa.shift = p->pk_shift;
+            pa.t0 = (uint32_t)(j * L);
+            pa.t1 = (uint32_t)std::min<uint64_t>((j + 1) * L, p->t_valid);
+            pa.wmax_raw = p->wmax_raw;
+            pa.has_left = j > 0; pa.has_right = j + 1 < p->n_sub;
+            pa.out = S.d_peaks; pa.out_count = S.d_count + 1; pa.out_cap = (uint32_t)p->cap;
+            AA_W(launch_peaks(pa, st));
+        }
+        AA_W(cudaEventRecord(S.ev[8], st));
+        AA_W(cudaMemcpyAsync(S.h_count, S.d_count, 2 * sizeof(uint32_t), cudaMemcpyDeviceToHost, st));
         if (staged && j + (uint64_t)p->n_streams < p->n_sub) {
             // the staging buffer is free once this sub-chunk's H2D is done: fill it for the next one while
             // the stream computes
@@ -760,14 +810,16 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
         AA_W(cudaStreamSynchronize(st));           // stream-scoped wait, never device-wide
         p->done[j].store(1, std::memory_order_release);
 
-        const uint64_t found = *S.h_count;
+        const uint64_t found_raw = S.h_count[0];
+        if (found_raw > p->cap) p->overflow.store(1);
+        p->total_raw.fetch_add(found_raw);
+        const uint64_t found = p->peaks ? (uint64_t)S.h_count[1] : found_raw;   // records that cross the link
         const uint64_t n = std::min<uint64_t>(found, p->cap);
-        if (found > p->cap) p->overflow.store(1);
         AA_W(cudaEventRecord(S.ev[5], st));
-        if (n) AA_W(cudaMemcpyAsync(S.h_cands, S.d_cands, n * sizeof(aa_candidate), cudaMemcpyDeviceToHost, st));
+        if (n) AA_W(cudaMemcpyAsync(S.h_cands, p->peaks ? S.d_peaks : S.d_cands, n * sizeof(aa_candidate), cudaMemcpyDeviceToHost, st));
         AA_W(cudaEventRecord(S.ev[6], st));
         AA_W(cudaStreamSynchronize(st));
-        S.d2h_bytes += 4 + n * sizeof(aa_candidate);
+        S.d2h_bytes += 8 + n * sizeof(aa_candidate);
 
         // host-to-host output stage of this stream: the sub-chunk's list goes to the caller's buffer
         // and is put in (dm_index, t_start) order right here, while the GPU works on the next sub-chunks
@@ -778,9 +830,7 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
             m = std::min<uint64_t>(n, max_cands - pos);
             if (m) {
                 std::memcpy(out + pos, S.h_cands, m * sizeof(aa_candidate));
-                std::sort(out + pos, out + pos + m, [](const aa_candidate &a, const aa_candidate &b) {
-                    return a.dm_index != b.dm_index ? a.dm_index < b.dm_index : a.t_start < b.t_start;
-                });
+                std::sort(out + pos, out + pos + m, cand_less);
             }
         }
         {
@@ -790,7 +840,7 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
             uint32_t *cnt = &p->run_cnt[j * (uint64_t)(p->ndms_total + 1)];
             uint64_t i = 0;
             for (uint32_t d = 0; d <= p->ndms_total; ++d) {
-                while (i < m && out[pos + i].dm_index < d) ++i;
+                while (i < m && (out[pos + i].dm_index & kPeakDmMask) < d) ++i;
                 cnt[d] = (uint32_t)i;
             }
         }
@@ -838,6 +888,7 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
             cudaEventElapsedTime(&ms, S.ev[kEvFixed + 3 * ri + 1], S.ev[kEvFixed + 3 * ri + 2]); S.sps_ms += ms;
         }
         cudaEventElapsedTime(&ms, S.ev[5], S.ev[6]); S.d2h_ms += ms;
+        if (p->peaks) { cudaEventElapsedTime(&ms, S.ev[7], S.ev[8]); S.sps_ms += ms; }
 
         aa_subchunk_times &T = p->timeline[j];
         T = aa_subchunk_times{};
@@ -935,6 +986,52 @@ void helper_main(aa_plan *p)
     }
 }
 
+// output_mode 1: `out[0..n)` is the merged list of what the sub-chunks sent, sorted by (dm_index, t_start): decided
+// peaks, and border records (flagged; beaten on their own sub-chunk or not).  A border record that is not yet beaten
+// is a peak iff no border record of the rows dm-1 .. dm+1 beats it (its other neighbours were all seen on the device).
+// Beaten records still beat others, so flags are only added while the list is scanned, and dropped at the end.
+uint64_t settle_borders(aa_plan *p, aa_candidate *out, uint64_t n)
+{
+    // first record of every trial
+    uint64_t i = 0;
+    for (uint32_t d = 0; d <= p->ndms_total; ++d) {
+        while (i < n && (out[i].dm_index & kPeakDmMask) < d) ++i;
+        p->dm_dst[d] = i;
+    }
+    auto beats = [](const aa_candidate &x, const aa_candidate &c) {
+        if (x.snr != c.snr) return x.snr > c.snr;
+        const uint32_t dx = x.dm_index & kPeakDmMask, dc = c.dm_index & kPeakDmMask;
+        if (dx != dc) return dx < dc;
+        return x.t_start < c.t_start;
+    };
+    for (uint64_t k = 0; k < n; ++k) {
+        aa_candidate &c = out[k];
+        if (!(c.dm_index & kPeakBorder) || (c.dm_index & kPeakBeaten)) continue;
+        const uint32_t dm = c.dm_index & kPeakDmMask;
+        const uint64_t t = c.t_start, te = t + c.width, t_lo = t > p->wmax_raw ? t - p->wmax_raw : 0;
+        bool beaten = false;
+        for (int dd = -1; dd <= 1 && !beaten; ++dd) {
+            const int64_t row = (int64_t)dm + dd;
+            if (row < 0 || row >= (int64_t)p->ndms_total) continue;
+            const aa_candidate *b = out + p->dm_dst[row], *e = out + p->dm_dst[row + 1];
+            const aa_candidate *q = std::lower_bound(b, e, t_lo, [](const aa_candidate &x, uint64_t v) { return x.t_start < v; });
+            for (; q < e && (uint64_t)q->t_start <= te; ++q) {
+                if (q == &c || !(q->dm_index & kPeakBorder) || t > (uint64_t)q->t_start + q->width) continue;
+                if (beats(*q, c)) { beaten = true; break; }
+            }
+        }
+        if (beaten) c.dm_index |= kPeakBeaten;
+    }
+    uint64_t m = 0;
+    for (uint64_t k = 0; k < n; ++k)
+        if (!(out[k].dm_index & kPeakBeaten)) {
+            out[m] = out[k];
+            out[m].dm_index &= kPeakDmMask;
+            ++m;
+        }
+    return m;
+}
+
 int run_impl(aa_plan *p, const uint8_t *input, Input mode, aa_candidate *out, uint64_t max_cands,
              uint64_t *n_cands, uint32_t *tap_out)
 {
@@ -956,7 +1053,7 @@ int run_impl(aa_plan *p, const uint8_t *input, Input mode, aa_candidate *out, ui
     const auto t0 = std::chrono::steady_clock::now();
     for (uint64_t j = 0; j < p->n_sub; ++j) { p->loaded[j].store(0); p->done[j].store(0); p->dedisp_issued[j].store(0); }
     for (int j = 0; j < p->n_streams; ++j) p->copied[j].store(0);
-    p->error.store(0); p->out_pos.store(0); p->total.store(0); p->overflow.store(0);
+    p->error.store(0); p->out_pos.store(0); p->total.store(0); p->total_raw.store(0); p->overflow.store(0);
     for (auto &S : p->streams) {
         S.h2d_ms = S.d2h_ms = S.prep_ms = S.dedisp_ms = S.sps_ms = S.h2h_ms = 0;
         S.h2d_bytes = S.d2h_bytes = S.dedisp_launches = S.sps_launches = S.prep_launches = S.h2h_bytes = 0;
@@ -990,13 +1087,15 @@ int run_impl(aa_plan *p, const uint8_t *input, Input mode, aa_candidate *out, ui
             command(p, aa_plan::Cmd::scatter);
             command(p, aa_plan::Cmd::copyback);
         } else {
-            std::sort(out, out + stored, [](const aa_candidate &a, const aa_candidate &b) {
-                return a.dm_index != b.dm_index ? a.dm_index < b.dm_index : a.t_start < b.t_start;
-            });
+            std::sort(out, out + stored, cand_less);
         }
     }
+    uint64_t n_peaks = 0;
+    if (p->peaks) {
+        n_peaks = settle_borders(p, out, stored);
+    }
     const auto t2 = std::chrono::steady_clock::now();
-    *n_cands = total;
+    *n_cands = p->peaks ? n_peaks : total;
 
     aa_stats &st = p->stats;
     st = aa_stats{};
@@ -1010,8 +1109,9 @@ int run_impl(aa_plan *p, const uint8_t *input, Input mode, aa_candidate *out, ui
         st.prep_launches += S.prep_launches;
         st.h2h_bytes += S.h2h_bytes; st.h2h_ms += S.h2h_ms;
     }
-    st.n_candidates = total;
-    st.n_stored = stored;
+    st.n_candidates = p->total_raw.load();
+    st.n_stored = p->peaks ? n_peaks : stored;
+    st.n_peaks = n_peaks;
     st.overflow = (p->overflow.load() || total > max_cands) ? 1 : 0;
     st.n_streams = p->n_streams;
     return st.overflow ? AA_ERR_OVERFLOW : AA_OK;

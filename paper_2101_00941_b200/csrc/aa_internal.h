@@ -172,6 +172,24 @@ struct SpsArgs {
     int32_t sigma_mode;    // 1: S/N from the statistics of each width's own boxcar series (reading A18; cluster kernel only)
 };
 
+// ---- peak finding on the device (kernels_peaks.cu, reading A17) ---------------------------------------------------
+struct PeakArgs {
+    const aa_candidate *cands;     // the sub-chunk's raw list
+    const uint32_t *count;         // records found (may exceed cap)
+    uint32_t cap;
+    int32_t *head;                 // [nrows][nbk] first record of each bucket, -1 = empty
+    uint32_t *next;                // [cap] chain
+    int32_t nrows, nbk, shift;     // DM trials of the plan, buckets per row, log2 of the bucket length in raw samples
+    uint32_t t0, t1;               // raw samples [t0, t1) in which this sub-chunk's candidates start
+    uint32_t wmax_raw;             // longest boxcar in raw samples
+    int32_t has_left, has_right;   // a previous / next sub-chunk exists
+    aa_candidate *out;             // peaks and border records; dm_index bit 31 = beaten, bit 30 = border
+    uint32_t *out_count;
+    uint32_t out_cap;
+};
+cudaError_t launch_peaks(const PeakArgs &a, cudaStream_t st);
+constexpr uint32_t kPeakBeaten = 0x80000000u, kPeakBorder = 0x40000000u, kPeakDmMask = 0x3FFFFFFFu;
+
 constexpr int kMaxWidths = 32;
 struct WidthTable { int32_t w[kMaxWidths]; int32_t dec[kMaxWidths]; };   // widths and the time grid of each (A20)
 

@@ -216,6 +216,34 @@ def test_measured_sigma_needs_cluster_sized_blocks(B):
         B.Plan(I.scaled(_tiny(bins=(8,), norm_block=1040, chunk_len=8 * 1040, nsamp=50000), sigma_mode=1))   # block of 130 samples
 
 
+@pytest.mark.parametrize("case", [
+    dict(thr=3.0),                                                              # 4 sub-chunks, dense noise candidates: many border records
+    dict(thr=3.2, n_streams=3, chunk_len=3 * 2048, nsamp=30000, widths=(1, 2, 4, 8, 64)),
+    dict(thr=3.5, bins=(1, 2, 4), nsamp=40000, chunk_len=8192, n_streams=2),   # ranges with different bins: neighbours across a range edge
+    dict(thr=3.0, bins=(8,), nsamp=60000, chunk_len=16384, ndms=20, widths=(1, 2, 4, 8, 32)),   # boxcars of 256 raw samples
+    dict(thr=4.0, nchans=302, ndms=100, nsamp=21000, chunk_len=4096, foff=-0.5, dm_step=0.25, norm_block=1024, n_streams=2),
+    dict(thr=3.0, chunk_len=1024, norm_block=1024, nsamp=9000, widths=(1, 2, 4, 8, 16, 128)),   # boxcars longer than a tenth of a sub-chunk
+])
+def test_peaks_on_the_device_equal_the_rule_on_the_full_list(B, case):
+    """output_mode 1 (reading A17): every sub-chunk's list is thinned on the device, borders are settled on the host;
+    the result must be exactly the peak rule applied to the oracle's full candidate list."""
+    w = _tiny(**case)
+    buf, x = _pinned_fill(B, w)
+    with B.Plan(w, peaks=True) as plan:
+        got, _ = plan.run(buf, want_taps=False)
+        st = plan.stats()
+        assert not plan.overflow and plan.info["n_subchunks"] >= 3
+    ref, _ = oracle.run(x, w)
+    want = oracle.find_peaks_fast(ref)
+    assert st["n_candidates"] == len(ref) and st["n_peaks"] == len(got)
+    assert 0 < len(want) < len(ref)
+    assert got.tobytes() == want.tobytes()
+    assert B.find_peaks(ref).tobytes() == want.tobytes()        # the host post-step agrees as well
+    with B.Plan(w) as plan:                                      # and fewer bytes crossed the link than in candidate mode
+        plan.run(buf, want_taps=False)
+        assert st["d2h_bytes"] < plan.stats()["d2h_bytes"]
+
+
 def test_saturated_16_bit_input(B):
     w = I.scaled(_tiny(nchans=1024, ndms=70, nsamp=9000, chunk_len=4096, f_top=1500.0, foff=-0.2, dm_step=0.25, norm_block=1024), nbits=16)
     buf = B.pinned_empty(w.nbytes)

@@ -175,6 +175,23 @@ def test_cfg2_full_streamed_equals_single_stream_and_oracle(B):
         assert top["snr"] >= 0.6 * expect and 0.5 * p.width <= top["width"] <= 2 * max(p.width, 1), (p, top)
 
 
+def test_cfg1_cfg2_peaks_on_the_device(B):
+    """cfg1 and cfg2 in output_mode 1 return exactly the peaks of the oracle's candidate list."""
+    for k in (1, 2):
+        w = I.workload(k)
+        buf, x = _pinned_fill(B, w)
+        with B.Plan(w, peaks=True) as plan:
+            got, _ = plan.run(buf, want_taps=False)
+            st = plan.stats()
+        ref, _ = oracle.run(x, w)
+        want = oracle.find_peaks_fast(ref)
+        assert st["n_candidates"] == len(ref) and len(want) < len(ref) / 10
+        assert got.tobytes() == want.tobytes(), k
+        # the strongest peak sits on the strongest injected pulse
+        top = got[np.argmax(got["snr"])]
+        assert any(abs(int(top["dm_index"]) - p.dm) <= 2 and abs(int(top["t_start"]) - p.t0) <= 2 * p.width + 2 for p in w.pulses)
+
+
 def _run_sampled(B, w, cells_extra, max_pulses=4, **plan_kw):
     buf, x = _pinned_fill(B, w)
     geo = oracle.geometry(w)

@@ -510,6 +510,25 @@ def test_peaks_hand_made_cases():
     assert len(oracle.find_peaks(_cl([]))) == 0
 
 
+def test_fast_peak_finding_is_the_all_pairs_rule():
+    """aaor_find_peaks (rows dm-1..dm+1, starts in [t - wmax, t + w]) against the all-pairs definition on random lists
+    with clumps, exact S/N ties, touching boxcars and gaps of one sample."""
+    rng = np.random.default_rng(17)
+    for trial in range(6):
+        n = 400
+        a = np.zeros(n, dtype=oracle.CAND_DTYPE)
+        a["dm_index"] = rng.integers(0, 12, n)
+        a["t_start"] = rng.integers(0, 300, n) * (1 if trial % 2 else 4)
+        a["width"] = rng.choice([1, 2, 4, 8, 32], n)
+        a["snr"] = rng.integers(6, 12, n).astype(np.float32) + (rng.random(n) < 0.5) * rng.random(n).astype(np.float32)
+        key = (a["dm_index"].astype(np.uint64) << np.uint64(32)) | a["t_start"].astype(np.uint64)
+        _, first = np.unique(key, return_index=True)                 # one candidate per (dm, t), sorted
+        a = a[np.sort(first)]
+        a = a[np.lexsort((a["t_start"], a["dm_index"]))]
+        slow, fast = oracle.find_peaks(a), oracle.find_peaks_fast(a)
+        assert 0 < len(slow) < len(a) and slow.tobytes() == fast.tobytes()
+
+
 def test_peaks_invariants_on_a_real_candidate_list():
     """peaks are a subset; no two peaks are neighbours; every dropped candidate has a neighbour that beats it;
     the injected cfg1 pulse gives one peak at exactly (DM 50, t 20000, w 8)."""
