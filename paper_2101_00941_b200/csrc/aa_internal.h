@@ -81,7 +81,8 @@ struct WsRecord {
     uint32_t esh[kSpG][2];          // byte k of the pair: 8 * e_{k,i} (16-bit input: e_{k,i} <= 2)
     uint32_t pofs;                  // byte offset of this stage's pattern rows inside the shared-memory ring
     int32_t dep;                    // the rows may be written once the consumers are done with stage dep (-1: at once)
-    uint32_t pad2[2];
+    uint32_t group;                 // channel group this stage sums: channels group * kSpG .. (stages are not in channel order)
+    uint32_t pad2;
     uint32_t poff[kSpDB];           // byte offset, inside the ring, of trial d's word (tau 0, tau 1)
 };
 static_assert(sizeof(WsRecord) % 16 == 0, "records are fetched with 16-byte bulk copies");

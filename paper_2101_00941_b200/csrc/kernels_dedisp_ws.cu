@@ -254,8 +254,8 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
             if (q < nstages && lane < REC / 16) cp_async16(myrec + j * REC + lane * 16, recs + (size_t)q * REC + lane * 16);
             asm volatile("cp.async.commit_group;" ::: "memory");
         };
-        // leader lane: the four channel windows of stage q, described by record copy R, into window slot w
-        auto issue = [&](int q, const WsRecord *R, int w) {
+        // leader lane: the four channel windows of the stage described by record copy R (channels 4 R->group ..), into window slot w
+        auto issue = [&](const WsRecord *R, int w) {
             uint32_t bytes = 0;
 #pragma unroll
             for (int i = 0; i < G; ++i) bytes += R->rbytes[i];
@@ -264,7 +264,7 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
             const uint32_t dst = sm_raw + w * raw_bytes;
 #pragma unroll
             for (int i = 0; i < G; ++i)
-                bulk_g2s(dst + i * ROWS, in + ((size_t)(q * G + i) * a.pitch_in + R->rbase[i]) * ES, R->rbytes[i], bar);
+                bulk_g2s(dst + i * ROWS, in + ((size_t)(R->group * G + i) * a.pitch_in + R->rbase[i]) * ES, R->rbytes[i], bar);
         };
 
         // turn it of this team is stage s = team + it * NTEAM; record copy slot it % 3, window slot 2 * team + (it & 1)
@@ -272,7 +272,7 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
         prefetch_record(team + NTEAM, 1);
         asm volatile("cp.async.wait_group 1;" ::: "memory");
         __syncwarp();
-        if (member == 0 && lane == 0 && team < nstages) issue(team, reinterpret_cast<const WsRecord *>(myrecp), 2 * team);
+        if (member == 0 && lane == 0 && team < nstages) issue(reinterpret_cast<const WsRecord *>(myrecp), 2 * team);
         __syncwarp();
 
         int rj = 0;                              // it % NRECBUF
@@ -288,7 +288,7 @@ __global__ void __launch_bounds__(NT, 1) dedisp_ws_kernel(const DedispArgs a)
                 // next turn's windows go to the slot read one turn ago: the whole team must be done with it
                 const int f = s - NTEAM;
                 if (f >= 0) mbar_wait_lane(full + 8 * (f % NSLOT), (uint32_t)((f / NSLOT) & 1));
-                issue(s + NTEAM, reinterpret_cast<const WsRecord *>(myrecp + rj1 * REC), 2 * team + ((it + 1) & 1));
+                issue(reinterpret_cast<const WsRecord *>(myrecp + rj1 * REC), 2 * team + ((it + 1) & 1));
             }
             __syncwarp();
             const uint32_t nchunk = R->nchunk, nbatch = R->nbatch, npat = R->npat;

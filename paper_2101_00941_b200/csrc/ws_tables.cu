@@ -110,6 +110,35 @@ bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_
                                    ? ((uint32_t)i * (uint32_t)rows + (m & ~7u)) | (8u * (m & 3u)) << 16 | ((m >> 2) & 1u) << 21
                                    : ((uint32_t)i * (uint32_t)rows + 2u * (m & ~3u)) | (m & 3u) << 16;
         }
+    // Stage order.  The producers' work per stage grows with the pattern count and the row length (3 patterns x 1100
+    // samples at the top of a 300 MHz band, 7 x 1950 at the bottom) while the consumers' work is the same for every
+    // stage, so in channel order the producers idle through the first half of a CTA and the consumers wait for them
+    // through the second half.  The sum over channel groups may be taken in any order (exact integers): stages
+    // alternate between the cheapest and the dearest groups left, and the ring of pattern rows evens out the pairs.
+    // The kernel's producer teams take every fourth stage (8 producer warps in teams of kWsTeam = 2), so the alternation runs
+    // cheap-dear-cheap-dear / dear-cheap-dear-cheap: every team gets both kinds.
+    // One order for all DM blocks, so that the CTAs of a time tile still walk the channels together (L2).
+    std::vector<double> cost((size_t)ngrp, 0.0);
+    for (int b = 0; b < nblk; ++b)
+        for (int g = 0; g < ngrp; ++g) {
+            const WsRecord &R = out[(size_t)b * ngrp + g];
+            cost[(size_t)g] += (double)R.nchunk * (40.0 + 34.0 * R.npat);
+        }
+    std::vector<int> rank((size_t)ngrp), order((size_t)ngrp);
+    for (int g = 0; g < ngrp; ++g) rank[(size_t)g] = g;
+    std::stable_sort(rank.begin(), rank.end(), [&](int x, int y) { return cost[(size_t)x] < cost[(size_t)y]; });
+    for (int s = 0, lo = 0, hi = ngrp - 1; s < ngrp; ++s)
+        order[(size_t)s] = ((s & 1) ^ ((s >> 2) & 1)) ? rank[(size_t)hi--] : rank[(size_t)lo++];
+    {
+        std::vector<WsRecord> staged(out.size());
+        for (int b = 0; b < nblk; ++b)
+            for (int s = 0; s < ngrp; ++s) {
+                WsRecord &R = staged[(size_t)b * ngrp + s];
+                R = out[(size_t)b * ngrp + order[(size_t)s]];
+                R.group = (uint32_t)order[(size_t)s];
+            }
+        out.swap(staged);
+    }
     // The pattern rows of successive stages go round a ring in shared memory.  Offsets are fixed here, per DM
     // block; dep = the latest earlier stage whose rows overlap the new ones (the producers wait until the
     // consumers are done with it), never older than s - kWsWindow (barrier slots are reused modulo kWsSlots).
@@ -123,8 +152,8 @@ bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_
         size_t oldest = 0;
         int64_t head = 0;
         int dep_run = -1;     // stages dropped from `live` are covered by an earlier wait only if dep never decreases
-        for (int g = 0; g < ngrp; ++g) {
-            WsRecord &R = out[(size_t)b * ngrp + g];
+        for (int s = 0; s < ngrp; ++s) {
+            WsRecord &R = out[(size_t)b * ngrp + s];
             const int64_t size = ((int64_t)R.npat * 2 * R.nchunk * 16 + 127) / 128 * 128;
             if (head + size > C) head = 0;
             const int64_t lo = head, hi = head + size;
@@ -133,10 +162,10 @@ bool ws_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, int32_
             // stages are consumed in order: everything up to the newest overlapping one must be gone
             for (size_t j = oldest; j < live.size(); ++j)
                 if (live[j].lo < hi && lo < live[j].hi) dep = live[j].s;
-            dep = std::max(dep, std::max(dep_run, g - kWsWindow));
+            dep = std::max(dep, std::max(dep_run, s - kWsWindow));
             dep_run = dep;
             while (oldest < live.size() && live[oldest].s <= dep) ++oldest;
-            live.push_back({g, lo, hi});
+            live.push_back({s, lo, hi});
             R.pofs = (uint32_t)lo;
             R.dep = dep;
             for (int dl = 0; dl < DB; ++dl) R.poff[dl] += (uint32_t)lo;
