@@ -129,6 +129,11 @@ typedef struct {
      * settled by the host on the merged list; the result is exactly aa_find_peaks of the full list.  *n_cands and
      * aa_stats.n_peaks then count peaks, aa_stats.n_candidates still counts the candidates found on the device. */
     int32_t  output_mode;
+    /* Debug / A-B timing knob for the single-pulse-search kernel: 0 = the plan's choice; 1 = keep the first cluster
+     * kernel (sps_cluster_kernel: four passes over the segment for the statistics) where the second
+     * (sps_cluster2_kernel: one pass + the listed outliers) would serve.  Same results.  Other values: AA_ERR_INVALID. */
+    int32_t  sps_variant;
+    int32_t  reserved0;        /* keeps the size a multiple of 8; must be 0 */
 } aa_plan_desc;
 
 typedef struct {

@@ -46,7 +46,8 @@ class PlanDescC(ctypes.Structure):
                 ("ntap", ctypes.c_int32), ("tap_dm_indices", ctypes.POINTER(ctypes.c_uint32)),
                 ("max_cands_per_subchunk", ctypes.c_uint64), ("stage_input", ctypes.c_int32),
                 ("dedisp_variant", ctypes.c_int32), ("nbits", ctypes.c_int32),
-                ("width_decimation", ctypes.c_int32), ("sigma_mode", ctypes.c_int32), ("output_mode", ctypes.c_int32)]
+                ("width_decimation", ctypes.c_int32), ("sigma_mode", ctypes.c_int32), ("output_mode", ctypes.c_int32),
+                ("sps_variant", ctypes.c_int32), ("reserved0", ctypes.c_int32)]
 
 
 class PlanInfoC(ctypes.Structure):
@@ -233,7 +234,8 @@ class Plan:
 
     def __init__(self, w, *, n_streams: Optional[int] = None, chunk_len: Optional[int] = None,
                  taps: Optional[Sequence[int]] = None, max_cands_per_subchunk: int = 0,
-                 torch_resources: bool = True, stage_input: bool = False, dedisp_variant="auto", peaks: bool = False):
+                 torch_resources: bool = True, stage_input: bool = False, dedisp_variant="auto", peaks: bool = False,
+                 sps_variant: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: the path has no CPU fallback")
@@ -261,6 +263,7 @@ class Plan:
         d.width_decimation = int(getattr(w, "wdec", 0))
         d.sigma_mode = int(getattr(w, "sigma_mode", 0))
         d.output_mode = 1 if peaks else 0
+        d.sps_variant = int(sps_variant)
         self._arena = None
         self._streams = None
         if torch_resources:

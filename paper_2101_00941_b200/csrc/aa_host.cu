@@ -444,6 +444,7 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
     p.cap = d->max_cands_per_subchunk ? d->max_cands_per_subchunk : (1ull << 21);
     if (p.cap > (1ull << 30)) return AA_ERR_INVALID;
     if (d->output_mode < 0 || d->output_mode > 1) return AA_ERR_INVALID;
+    if (d->sps_variant < 0 || d->sps_variant > 1 || d->reserved0 != 0) return AA_ERR_INVALID;
     p.peaks = d->output_mode == 1;
     p.wmax_raw = (uint32_t)p.wmax * (uint32_t)bin_max;
     p.pk_shift = 5;
@@ -758,7 +759,8 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
                 sa.count = S.d_count;
                 sa.cap = (uint32_t)p->cap;
                 sa.sigma_mode = p->desc.sigma_mode;
-                AA_W(launch_sps(sa, p->wt, Rg.wide, Rg.small31, p->big, st));
+                sa.maxval = (uint32_t)(((1ull << p->nbits) - 1) * (uint64_t)nchans * b);
+                AA_W(launch_sps(sa, p->wt, Rg.wide, Rg.small31, p->big, p->desc.sps_variant == 1, st));
                 S.sps_launches++;
                 AA_W(cudaEventRecord(e2, st));
                 // tapped rows: runs of consecutive trials leave in one strided copy (all rows tapped = the dense

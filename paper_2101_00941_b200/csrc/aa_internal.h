@@ -171,6 +171,7 @@ struct SpsArgs {
     uint32_t *count;
     uint32_t cap;
     int32_t sigma_mode;    // 1: S/N from the statistics of each width's own boxcar series (reading A18; cluster kernel only)
+    uint32_t maxval;       // largest value a dedispersed sample can take (maxsample * nchans * bin)
 };
 
 // ---- peak finding on the device (kernels_peaks.cu, reading A17) ---------------------------------------------------
@@ -221,7 +222,8 @@ int dedisp_stage_channels(bool in16);
 cudaError_t dedisp_configure();   // opt in to large dynamic shared memory (once per process)
 // wide: boxcar sums need 64 bits (maxsample nchans bin wmax >= 2^32); small31: they stay below 2^31;
 // big: a block's sum of squares may pass 2^63 (16-bit input on many channels): 128-bit sums in the generic kernel
-cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, bool small31, bool big, cudaStream_t st);
+// force_v1: keep sps_cluster_kernel where sps_cluster2_kernel would serve (A/B timing and tests)
+cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, bool small31, bool big, bool force_v1, cudaStream_t st);
 cudaError_t sps_configure();
 
 }  // namespace aa

@@ -249,7 +249,7 @@ struct SharedC {
     int w[kMaxWidths];
     int dec[kMaxWidths];
     uint32_t warp_tot[NT2 / 32];
-    uint4 wl[kMaxWidths];               // (width, pre-filter threshold, grid, -): multiples of 4 first, then the others, then coarse grids
+    uint4 wl[kMaxWidths + 1];           // (width, pre-filter threshold, grid, -): multiples of 4 first, then the others, then coarse grids
     int na, nu, nd;
 };
 
@@ -746,6 +746,556 @@ __global__ void __launch_bounds__(NT2) sps_cluster_kernel(const SpsArgs a, const
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Cluster kernel, second version (white-noise scaling A10, every width at every sample, boxcar sums below 2^31).
+// Same layout as sps_cluster_kernel (segment + boxcar tail of one normalisation block per CTA, cluster of C CTAs
+// per block, series read from HBM once), a third of the instructions and ONE cluster-wide wait instead of five:
+//   pass A   thread t walks its own chunk of the segment once: exact sum and sum of squares (the block's pass 0,
+//            A8) and the chunk total for the prefix sums;
+//   pass B   walks it again: writes the exclusive prefix sums in place and marks (one bit per sample) the samples
+//            outside the CTA's "core" interval mu' +- 2.75 sigma' (mu', sigma' = plain moments of the segment
+//            alone: a guess that needs no other CTA);
+//   list     the marked samples (0.6 % of white noise) are appended to a small list that every CTA of the
+//            cluster receives (DSMEM stores), with the CTA's exact sums and its core interval; one cluster barrier;
+//   stats    warp 0 of every CTA then holds everything the three clip passes need: a 3-sigma interval I that
+//            contains every core selects all samples but the listed ones outside I, so
+//            (m, S1, S2)(I) = totals - sums over {listed x not in I}: exact integers, the oracle's mu and sigma
+//            bit for bit.  If an interval does not contain a core (strong interference: sigma collapses after the
+//            first clip), a list is full, or a core is empty, the pass and those after it walk the whole segment
+//            as sps_cluster_kernel does;
+//   boxcars  that chain (three dependent rounds of interval, sums, 128-bit moments, double division and root) is
+//            serial and takes one warp several microseconds, so warps 1-7 do not wait for it: they run the integer
+//            pre-filter th_w + P[tau] - P[tau + w] < 0 with thresholds GUESSED from the unclipped moments
+//            (mu0 - sigma0 / 20, 0.9 sigma0) and keep one bit per tau.  When the chain is done the guess is checked
+//            against the true thresholds (guess <= truth for every width: the bits are then a superset of the hits;
+//            otherwise the pre-filter is repeated with the truth), and the marked taus get the double-precision S/N
+//            of every width, the arg-max and the threshold test with the final mu and sigma.
+//            Pre-filter: two widths per 3-input OR, widths below 4 from the next 16-byte piece, eight taus per thread.
+constexpr int kListTotal = 1536;      // list entries per CTA (all ranks' outliers): 6 KB
+
+struct SharedC2 {
+    SharedC c;                           // the fields the slow path and the candidate stage share with version 1
+    uint64_t redA[2][NT2 / 32];          // pass A: sum, sum of squares per warp
+    uint64_t part2[kMaxCluster][6];      // per rank: n_own, S1, S2, (lc | hc << 32), listed entries, flags
+    uint64_t lbar[NT2 / 32];             // mbarriers of the warps' bulk loads
+    uint32_t nlist;                      // entries this CTA found (may exceed its room)
+    int slow_from;                       // 0: statistics done by warp 0; k: passes k..3 take the slow path
+    uint32_t ths[4];                     // pre-filter thresholds of widths 1, 2, 3 (index w; "never" if the width is not searched)
+    int slot[kMaxWidths];                // where width j's threshold lives: wl index, or -w for the widths below 4
+    int dup;                             // wl index that repeats the last aligned width (-1: none)
+    uint32_t thg[kMaxWidths];            // guessed thresholds (plain), for the check against thr_u
+    int nsm, guess_ok;
+};
+
+constexpr int NTP = NT2 - 32;            // threads of the pre-filter (warps 1-7)
+constexpr uint32_t kNever = 0x7FFFFFFFu;
+// th - 1 as a signed number: B >= th  <=>  (th - 1) - B < 0; th above every possible B (< 2^31) -> never
+__device__ __forceinline__ uint32_t enc_thr(uint32_t th) { return th == 0u ? 0xFFFFFFFFu : (th > 0x7FFFFFFFu ? kNever : th - 1u); }
+
+// Integer pre-filter over the taus [0, 4 ngroups) of the segment by the NTP threads gid = 0 .. NTP - 1: thread gid takes
+// the groups of four taus g = it * 2 NTP + gid and g + NTP of round it; bit 8 it + k of the result marks tau k of the pair.
+__device__ __forceinline__ void prefilter(const uint32_t *X, const SharedC2 &s2, int gid, int ngroups, uint64_t &flo, uint32_t &fhi)
+{
+    const SharedC &sh = s2.c;
+    const int na2 = (sh.na + 1) & ~1, nu = sh.nu, nsm = s2.nsm;
+    constexpr int GB = 4 * NTP;
+    flo = 0ull;
+    fhi = 0u;
+    const uint32_t th1 = s2.ths[1], th2 = s2.ths[2], th3 = s2.ths[3];
+    int it = 0;
+    for (int g0 = 0; g0 < ngroups; g0 += 2 * NTP, ++it) {
+        const int g = g0 + gid;
+        if (g >= ngroups) break;
+        const bool two = g + NTP < ngroups;               // else the second group repeats the first
+        const uint32_t *xg = X + 4 * g;
+        const int gb = two ? GB : 0;
+        const uint4 pa = *reinterpret_cast<const uint4 *>(xg), pb = *reinterpret_cast<const uint4 *>(xg + gb);
+        uint32_t f0 = 0, f1 = 0, f2 = 0, f3 = 0, f4 = 0, f5 = 0, f6 = 0, f7 = 0;   // sign bits collect the hits
+        if (nsm) {
+            // widths 1, 2, 3: P[tau + w] comes from the group itself and the next 16-byte piece
+            const uint4 na4 = *reinterpret_cast<const uint4 *>(xg + 4), nb4 = *reinterpret_cast<const uint4 *>(xg + gb + 4);
+            f0 |= (th1 + pa.x - pa.y) | (th2 + pa.x - pa.z); f0 |= th3 + pa.x - pa.w;
+            f1 |= (th1 + pa.y - pa.z) | (th2 + pa.y - pa.w); f1 |= th3 + pa.y - na4.x;
+            f2 |= (th1 + pa.z - pa.w) | (th2 + pa.z - na4.x); f2 |= th3 + pa.z - na4.y;
+            f3 |= (th1 + pa.w - na4.x) | (th2 + pa.w - na4.y); f3 |= th3 + pa.w - na4.z;
+            f4 |= (th1 + pb.x - pb.y) | (th2 + pb.x - pb.z); f4 |= th3 + pb.x - pb.w;
+            f5 |= (th1 + pb.y - pb.z) | (th2 + pb.y - pb.w); f5 |= th3 + pb.y - nb4.x;
+            f6 |= (th1 + pb.z - pb.w) | (th2 + pb.z - nb4.x); f6 |= th3 + pb.z - nb4.y;
+            f7 |= (th1 + pb.w - nb4.x) | (th2 + pb.w - nb4.y); f7 |= th3 + pb.w - nb4.z;
+        }
+        // widths that are multiples of 4: aligned 16-byte loads, two widths per round (one 3-input OR takes both)
+#pragma unroll 2
+        for (int j = 0; j < na2; j += 2) {
+            const uint4 w0 = sh.wl[j], w1 = sh.wl[j + 1];
+            const uint4 qa = *reinterpret_cast<const uint4 *>(xg + w0.x), qb = *reinterpret_cast<const uint4 *>(xg + w0.x + gb);
+            const uint4 ra = *reinterpret_cast<const uint4 *>(xg + w1.x), rb = *reinterpret_cast<const uint4 *>(xg + w1.x + gb);
+            const uint32_t t0 = w0.y, t1 = w1.y;
+            f0 |= (t0 + pa.x - qa.x) | (t1 + pa.x - ra.x); f1 |= (t0 + pa.y - qa.y) | (t1 + pa.y - ra.y);
+            f2 |= (t0 + pa.z - qa.z) | (t1 + pa.z - ra.z); f3 |= (t0 + pa.w - qa.w) | (t1 + pa.w - ra.w);
+            f4 |= (t0 + pb.x - qb.x) | (t1 + pb.x - rb.x); f5 |= (t0 + pb.y - qb.y) | (t1 + pb.y - rb.y);
+            f6 |= (t0 + pb.z - qb.z) | (t1 + pb.z - rb.z); f7 |= (t0 + pb.w - qb.w) | (t1 + pb.w - rb.w);
+        }
+        // the others: the aligned pieces around tau + w, shifted by w mod 4 (uniform)
+#pragma unroll 1
+        for (int j = na2; j < na2 + nu; ++j) {
+            const uint4 wt2 = sh.wl[j];
+            const uint32_t th = wt2.y;
+            const int r = (int)(wt2.x & 3u);
+            const uint32_t *xq = xg + (wt2.x - (uint32_t)r);
+            const uint4 q0 = *reinterpret_cast<const uint4 *>(xq), q1 = *reinterpret_cast<const uint4 *>(xq + 4),
+                        q2 = *reinterpret_cast<const uint4 *>(xq + gb), q3 = *reinterpret_cast<const uint4 *>(xq + gb + 4);
+            uint32_t v0, v1, v2, v3, v4, v5, v6, v7;
+            if (r == 1) { v0 = q0.y; v1 = q0.z; v2 = q0.w; v3 = q1.x; v4 = q2.y; v5 = q2.z; v6 = q2.w; v7 = q3.x; }
+            else if (r == 2) { v0 = q0.z; v1 = q0.w; v2 = q1.x; v3 = q1.y; v4 = q2.z; v5 = q2.w; v6 = q3.x; v7 = q3.y; }
+            else { v0 = q0.w; v1 = q1.x; v2 = q1.y; v3 = q1.z; v4 = q2.w; v5 = q3.x; v6 = q3.y; v7 = q3.z; }
+            f0 |= th + pa.x - v0; f1 |= th + pa.y - v1; f2 |= th + pa.z - v2; f3 |= th + pa.w - v3;
+            f4 |= th + pb.x - v4; f5 |= th + pb.y - v5; f6 |= th + pb.z - v6; f7 |= th + pb.w - v7;
+        }
+        if ((int)((f0 | f1 | f2 | f3) | (f4 | f5 | f6 | f7)) < 0) {
+            uint32_t any = (f0 >> 31) | (f1 >> 31) << 1 | (f2 >> 31) << 2 | (f3 >> 31) << 3 | (f4 >> 31) << 4 | (f5 >> 31) << 5 |
+                           (f6 >> 31) << 6 | (f7 >> 31) << 7;
+            if (!two) any &= 15u;                         // the repeated group is not evaluated twice
+            if (it < 8) flo |= (uint64_t)any << (8 * it);
+            else fhi |= any << (8 * (it - 8));
+        }
+    }
+}
+// thresholds of the pre-filter into their slots (plain threshold th of width j)
+__device__ __forceinline__ void put_threshold(SharedC2 &s2, int j, uint32_t th)
+{
+    const int sl = s2.slot[j];
+    const uint32_t e = enc_thr(th);
+    if (sl < 0) {
+        s2.ths[-sl] = e;
+    } else {
+        s2.c.wl[sl].y = e;
+        if (s2.dup >= 0 && sl == s2.dup - 1) s2.c.wl[s2.dup].y = e;
+    }
+}
+
+
+__device__ __forceinline__ void st_cluster_u32(const void *local, uint32_t rank, uint32_t v)
+{
+    uint32_t a = (uint32_t)__cvta_generic_to_shared(local), r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(a), "r"(rank));
+    asm volatile("st.shared::cluster.u32 [%0], %1;" ::"r"(r), "r"(v) : "memory");
+}
+__device__ __forceinline__ uint64_t warp_sum_all(uint64_t v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ void moments_from_sums(uint64_t m, uint64_t S1, unsigned __int128 S2, double &mu, double &sigma)
+{
+    const unsigned __int128 N = (unsigned __int128)m * S2 - (unsigned __int128)S1 * S1;
+    const double dm = __ull2double_rn(m);
+    mu = __ddiv_rn(__ull2double_rn(S1), dm);
+    sigma = __dsqrt_rn(__ddiv_rn(u128_to_double(N), __dmul_rn(dm, dm)));
+}
+
+__global__ void __launch_bounds__(NT2) sps_cluster2_kernel(const SpsArgs a, const __grid_constant__ WidthTable wt, const int C, const int seg)
+{
+    extern __shared__ __align__(16) uint8_t dyn[];
+    uint32_t *X = reinterpret_cast<uint32_t *>(dyn);     // segment + tail; later its exclusive prefix sums
+    const int total = seg + a.wmax - 1 + 8;              // slots the boxcar loop may read
+    uint32_t *LST = X + total;                           // [C][lreg] listed samples of every rank
+    const int lreg = kListTotal / C;
+    __shared__ SharedC2 s2;
+    SharedC &sh = s2.c;
+
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int d = blockIdx.y;
+    const uint32_t rank = C > 1 ? cluster_rank() : 0u;
+    const int64_t blk = blockIdx.x / C;
+    if (tid < kMaxWidths) { sh.w[tid] = wt.w[tid]; sh.dec[tid] = 1; }
+    const int64_t b0 = blk * a.block_len;
+    int64_t b1 = b0 + a.block_len;
+    if (b1 > a.nout_left) b1 = a.nout_left;
+    if (b0 >= b1 || b0 >= a.nemit) return;               // uniform over the cluster
+    const int64_t n_k = b1 - b0;
+    const uint32_t *row = a.D + (size_t)d * a.pitch;
+    const int64_t s0 = b0 + (int64_t)rank * seg;         // first column of this CTA's segment
+    const int64_t navail = a.ncols < a.nout_left ? (int64_t)a.ncols : a.nout_left;
+    const int halo = a.wmax - 1;
+    int n_in = (int)((navail - s0 > seg + halo) ? seg + halo : (navail - s0 < 0 ? 0 : navail - s0));   // columns held
+    int n_own = (int)((b1 - s0 > seg) ? seg : (b1 - s0 < 0 ? 0 : b1 - s0));                             // ... of the block
+    if (n_own > n_in) n_own = n_in;
+
+    // ---- load: one bulk copy per warp (the part its threads walk), each onto its own mbarrier, so that a warp starts
+    //      as soon as its own part has landed -------------------------------------------------------------------------
+    int chunk = (n_in + 1 + NT2 - 1) / NT2;               // slots 0 .. n_in over the threads
+    chunk |= 1;                                           // odd stride: conflict-free
+    const int i0 = tid * chunk;
+    const int c_in = min(max(n_in - i0, 0), chunk);       // elements of the thread's chunk that hold data
+    const int c_own = min(max(n_own - i0, 0), chunk);     // ... that belong to the block (the rest is the boxcar tail)
+    if (tid == 0) {
+#pragma unroll
+        for (int w = 0; w < NT2 / 32; ++w)
+            asm volatile("mbarrier.init.shared::cta.b64 [%0], 1;" ::"r"((uint32_t)__cvta_generic_to_shared(&s2.lbar[w])));
+        asm volatile("fence.mbarrier_init.release.cluster;" ::: "memory");
+        s2.nlist = 0;
+        s2.slow_from = 0;
+    }
+    if (tid == 32) {
+        // width classes of the pre-filter: below 4 (from the neighbouring piece), multiples of 4 (aligned loads, taken two
+        // at a time: an odd count repeats the last one), the rest
+        int n = 0, nsm = 0;
+        s2.ths[0] = s2.ths[1] = s2.ths[2] = s2.ths[3] = kNever;
+        for (int j = 0; j < a.nwidths; ++j)
+            if (wt.w[j] < 4) { s2.slot[j] = -wt.w[j]; ++nsm; }
+        s2.nsm = nsm;
+        for (int j = 0; j < a.nwidths; ++j)
+            if ((wt.w[j] & 3) == 0) { s2.slot[j] = n; sh.wl[n++] = make_uint4((uint32_t)wt.w[j], kNever, 1u, 0u); }
+        sh.na = n;
+        s2.dup = -1;
+        if (n & 1) { s2.dup = n; sh.wl[n] = sh.wl[n - 1]; }
+        int q = (n + 1) & ~1;
+        for (int j = 0; j < a.nwidths; ++j)
+            if (wt.w[j] > 4 && (wt.w[j] & 3) != 0) { s2.slot[j] = q; sh.wl[q++] = make_uint4((uint32_t)wt.w[j], kNever, 1u, 0u); }
+        sh.nu = q - ((n + 1) & ~1);
+    }
+    __syncthreads();
+    // every CTA of the cluster must be running before its shared memory is written: arrive now, wait before the first remote store
+    if (C > 1) asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    {
+        const int n4 = (n_in + 3) / 4 * 4;                // whole 16-byte pieces; the row pitch leaves room
+        const int e0 = warp * 32 * chunk, e1 = min(e0 + 32 * chunk, n4);
+        if (e1 > e0) {
+            const uint32_t bar = (uint32_t)__cvta_generic_to_shared(&s2.lbar[warp]);
+            if (lane == 0) {
+                const uint32_t bytes = (uint32_t)(e1 - e0) * 4u;
+                asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(bar), "r"(bytes) : "memory");
+                asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];" ::"r"(
+                                 (uint32_t)__cvta_generic_to_shared(X + e0)),
+                             "l"(row + s0 + e0), "r"(bytes), "r"(bar)
+                             : "memory");
+            }
+            uint32_t ok = 0;
+            while (!ok)
+                asm volatile(
+                    "{\n\t.reg .pred p;\n\t"
+                    "mbarrier.try_wait.parity.shared::cta.b64 p, [%1], 0;\n\t"
+                    "selp.u32 %0, 1, 0, p;\n\t}"
+                    : "=r"(ok)
+                    : "r"(bar)
+                    : "memory");
+        }
+    }
+
+    // ---- pass A: the thread's chunk [i0, i0 + chunk): exact sums over the block's part, total over all of it ----
+    uint32_t *xp = X + i0;
+    uint32_t run = 0;
+    uint64_t S1 = 0, S2 = 0;
+    {
+        const bool fast32 = (uint64_t)a.maxval * (uint64_t)chunk < 0x100000000ull;   // the chunk's sum fits 32 bits
+        if (fast32) {
+#pragma unroll 8
+            for (int k = 0; k < c_own; ++k) {
+                const uint32_t x = xp[k];
+                run += x;
+                S2 += (uint64_t)x * x;
+            }
+            S1 = run;
+        } else {
+#pragma unroll 4
+            for (int k = 0; k < c_own; ++k) {
+                const uint32_t x = xp[k];
+                S1 += x;
+                S2 += (uint64_t)x * x;
+            }
+            run = (uint32_t)S1;
+        }
+#pragma unroll 4
+        for (int k = c_own; k < c_in; ++k) run += xp[k];
+    }
+    uint32_t incl = run;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+        const uint32_t v = __shfl_up_sync(0xffffffffu, incl, o);
+        if (lane >= o) incl += v;
+    }
+    S1 = warp_sum_all(S1);
+    S2 = warp_sum_all(S2);
+    if (lane == 31) sh.warp_tot[warp] = incl;
+    if (lane == 0) { s2.redA[0][warp] = S1; s2.redA[1][warp] = S2; }
+    __syncthreads();
+    // every thread: the segment's sums, its own exclusive prefix, and the core interval from the segment's plain moments
+    uint32_t pre = incl - run;
+    S1 = 0; S2 = 0;
+#pragma unroll
+    for (int w = 0; w < NT2 / 32; ++w) {
+        if (w < warp) pre += sh.warp_tot[w];
+        S1 += s2.redA[0][w];
+        S2 += s2.redA[1][w];
+    }
+    uint32_t lc = 1u, hc = 0u;                            // empty core: everything is listed (-> slow path)
+    if (n_own > 0) {
+        const double kcore = 2.75;                        // 0.6 % of white noise outside: about 100 listed samples per segment
+        const double nn = (double)n_own, mean = (double)S1 / nn;
+        double var = (double)S2 / nn - mean * mean;       // a guess: need not be exact
+        if (!(var > 0.0)) var = 0.0;
+        const double sd = sqrt(var);
+        double l = ceil(mean - kcore * sd), h = floor(mean + kcore * sd);
+        if (l < 0.0) l = 0.0;
+        if (h > 4294967295.0) h = 4294967295.0;
+        if (l <= h) { lc = (uint32_t)l; hc = (uint32_t)h; }
+    }
+    const uint32_t cspan = hc - lc;                       // empty core: 0xFFFFFFFF, no sample passes (x - lc) <= ... see below
+    const bool core_empty = lc > hc;
+
+    // ---- pass B: exclusive prefix sums in place; one bit per sample of the block outside the core ---------------
+    uint32_t mk[3] = {0u, 0u, 0u};
+#pragma unroll
+    for (int wd = 0; wd < 3; ++wd) {
+        const int k0 = 32 * wd;
+        const int kend = min(c_own - k0, 32);
+        uint32_t m = 0, bit = 1u;
+#pragma unroll 8
+        for (int k = 0; k < kend; ++k) {
+            const uint32_t x = xp[k0 + k];
+            xp[k0 + k] = pre;
+            pre += x;
+            if ((x - lc) > cspan) m |= bit;
+            bit += bit;
+        }
+        mk[wd] = m;
+    }
+    if (core_empty) {                                     // (x - 1) > 0xFFFFFFFF never holds: mark everything instead
+#pragma unroll
+        for (int wd = 0; wd < 3; ++wd) {
+            const int kend = min(c_own - 32 * wd, 32);
+            mk[wd] = kend <= 0 ? 0u : (kend >= 32 ? 0xFFFFFFFFu : ((1u << kend) - 1u));
+        }
+    }
+    for (int k = c_own; k < c_in; ++k) {                  // the boxcar tail
+        const uint32_t x = xp[k];
+        xp[k] = pre;
+        pre += x;
+    }
+    if (c_in > 0 && i0 + c_in == n_in) xp[c_in] = pre;    // slot n_in: the total
+    if (n_in == 0 && tid == 0) X[0] = 0u;
+    if (C > 1) asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");   // all CTAs run: remote stores may begin
+    __syncthreads();
+    {
+        const uint32_t last = X[n_in];
+        for (int i = n_in + 1 + tid; i < total; i += NT2) X[i] = last;
+    }
+    // the marked samples (x = P[i + 1] - P[i]) go to every CTA's copy of this rank's list
+#pragma unroll
+    for (int wd = 0; wd < 3; ++wd) {
+        uint32_t m = mk[wd];
+        while (m) {
+            const int k = __ffs(m) - 1;
+            m &= m - 1u;
+            const int i = i0 + 32 * wd + k;
+            const uint32_t x = X[i + 1] - X[i];
+            const uint32_t pos = atomicAdd(&s2.nlist, 1u);
+            if (pos < (uint32_t)lreg) {
+                uint32_t *slot = LST + rank * lreg + pos;
+                if (C > 1) {
+                    for (int r = 0; r < C; ++r) st_cluster_u32(slot, (uint32_t)r, x);
+                } else {
+                    *slot = x;
+                }
+            }
+        }
+    }
+    __syncthreads();
+    if (tid == 0) {
+        const uint32_t found = s2.nlist;
+        const uint64_t flags = (found > (uint32_t)lreg || (core_empty && n_own > 0)) ? 1ull : 0ull;
+        const uint64_t v[6] = {(uint64_t)n_own, S1, S2, (uint64_t)lc | ((uint64_t)hc << 32),
+                               (uint64_t)(found > (uint32_t)lreg ? (uint32_t)lreg : found), flags};
+        for (int r = 0; r < C; ++r)
+#pragma unroll
+            for (int q = 0; q < 6; ++q) {
+                if (C > 1) st_cluster_u64(&s2.part2[rank][q], (uint32_t)r, v[q]);
+                else s2.part2[0][q] = v[q];
+            }
+    }
+    if (C > 1) cluster_sync_all(); else __syncthreads();
+
+    // ---- warp 0: statistics (A8) from the totals and the lists, the same integers in every CTA;
+    //      warps 1-7 meanwhile: pre-filter with guessed thresholds ------------------------------------------------------
+    const int n_emit = n_own;                             // taus [0, n_emit) of this segment may emit (blocks tile the sub-chunk)
+    const int ngroups = (n_emit + 3) / 4;
+    uint64_t flo = 0ull;
+    uint32_t fhi = 0u;
+    if (warp == 0) {
+        uint64_t n = 0, T1 = 0;
+        unsigned __int128 T2 = 0;
+        bool listed_ok = true;
+        for (int r = 0; r < C; ++r) {
+            n += s2.part2[r][0]; T1 += s2.part2[r][1]; T2 += s2.part2[r][2];
+            if (s2.part2[r][5]) listed_ok = false;
+        }
+        double mu = 0.0, sigma = 0.0;
+        int slow = 0;
+        if (n) {
+            moments_from_sums(n, T1, T2, mu, sigma);      // pass 0: every sample
+            for (int pass = 1; pass < 4; ++pass) {
+                uint32_t lo = 0, hi = 0;
+                if (!clip_interval(mu, __dmul_rn(3.0, sigma), lo, hi)) break;   // nothing selected: keep the last values
+                bool covered = listed_ok;
+                for (int r = 0; r < C; ++r) {
+                    const uint64_t ch = s2.part2[r][3];
+                    if (s2.part2[r][0] && !(lo <= (uint32_t)ch && hi >= (uint32_t)(ch >> 32))) covered = false;
+                }
+                if (!covered) { slow = pass; break; }
+                const uint32_t span = hi - lo;
+                uint64_t mr = 0, R1 = 0, R2 = 0, carry = 0;   // the listed samples the interval rejects
+                for (int r = 0; r < C; ++r) {
+                    const int cnt = (int)s2.part2[r][4];
+                    const uint32_t *L = LST + r * lreg;
+#pragma unroll 4
+                    for (int e = lane; e < cnt; e += 32) {
+                        const uint32_t x = L[e];
+                        const bool rej = (x - lo) > span;
+                        const uint32_t xr = rej ? x : 0u;
+                        mr += rej ? 1u : 0u;
+                        R1 += xr;
+                        const uint64_t sq = (uint64_t)xr * xr;
+                        R2 += sq;
+                        carry += R2 < sq;
+                    }
+                }
+                mr = warp_sum_all(mr); R1 = warp_sum_all(R1);
+                const uint64_t r2lo = warp_sum_all(R2 & 0xFFFFFFFFull), r2hi = warp_sum_all(R2 >> 32);
+                carry = warp_sum_all(carry);
+                const unsigned __int128 R2w = (unsigned __int128)r2lo + ((unsigned __int128)r2hi << 32) + ((unsigned __int128)carry << 64);
+                const uint64_t m = n - mr;
+                if (!m) break;
+                moments_from_sums(m, T1 - R1, T2 - R2w, mu, sigma);
+            }
+        }
+        if (lane == 0) { sh.mu = mu; sh.sigma = sigma; sh.m = n; s2.slow_from = slow; }
+    } else {
+        const int gid = tid - 32;
+        if (gid < a.nwidths) {
+            // the unclipped moments, roughly (nothing exact depends on them)
+            uint64_t n = 0, T1 = 0, T2 = 0;
+            for (int r = 0; r < C; ++r) { n += s2.part2[r][0]; T1 += s2.part2[r][1]; T2 += s2.part2[r][2]; }
+            const double nn = (double)n, mean = (double)T1 / nn;
+            double var = (double)T2 / nn - mean * mean;
+            if (!(var > 0.0)) var = 0.0;
+            const double sd = sqrt(var), w = (double)sh.w[gid];
+            const double bt = floor(w * (mean - 0.05 * sd) + a.thr * (0.9 * sd) * sqrt(w)) - 1.0;
+            const uint32_t th = bt <= 0.0 ? 0u : (bt >= 4294967295.0 ? 0xFFFFFFFFu : (uint32_t)bt);
+            s2.thg[gid] = th;
+            put_threshold(s2, gid, th);
+        }
+        asm volatile("bar.sync 1, %0;" ::"n"(NTP) : "memory");
+        if (n_emit > 0) prefilter(X, s2, gid, ngroups, flo, fhi);
+    }
+    __syncthreads();
+    double mu = sh.mu, sigma = sh.sigma;
+    const int slow_from = s2.slow_from;
+    __syncthreads();
+    if (slow_from) {
+        // rare: the remaining passes over the whole segment, x = P[i + 1] - P[i], as version 1 does them
+        int turn = 0;
+        for (int pass = slow_from; pass < 4; ++pass) {
+            uint32_t lo = 0u, span = 0u;
+            bool run2 = true;
+            if (tid == 0) {
+                uint32_t l = 0, h = 0;
+                sh.empty = clip_interval(mu, __dmul_rn(3.0, sigma), l, h) ? 0 : 1;
+                sh.lo = l;
+                sh.hi = h;
+            }
+            __syncthreads();
+            run2 = !sh.empty;
+            lo = sh.lo;
+            span = sh.hi - lo;
+            uint64_t m = 0, Q1 = 0, Q2 = 0, carry = 0;
+            if (run2) {
+                for (int i = tid; i < n_own; i += NT2) {
+                    const uint32_t x = X[i + 1] - X[i];
+                    if ((x - lo) <= span) {
+                        m += 1;
+                        Q1 += x;
+                        const uint64_t sq = (uint64_t)x * x;
+                        Q2 += sq;
+                        carry += Q2 < sq;
+                    }
+                }
+            }
+            if (!cluster_moments(sh, C, rank, turn, m, Q1, Q2, carry, mu, sigma)) break;
+        }
+    }
+    if (!(sigma > 0.0) || n_k < 32) return;
+
+    // ---- per-width constants with the final mu, sigma; was the guess below the truth for every width? ---------------
+    if (tid < a.nwidths) {
+        const double w = (double)sh.w[tid];
+        const double den = __dmul_rn(sigma, __dsqrt_rn(w));
+        sh.den[tid] = den;
+        // B >= floor(w mu + thr sigma sqrt w) - 1 is necessary for S >= thr; clamped to the 32-bit sums
+        const long long bt = __double2ll_rd(w * mu + a.thr * den) - 1;
+        sh.thr_u[tid] = bt <= 0 ? 0u : (bt >= 0xFFFFFFFFll ? 0xFFFFFFFFu : (uint32_t)bt);
+    }
+    __syncthreads();
+    if (tid == 0) {
+        int ok = 1;
+        for (int j = 0; j < a.nwidths; ++j) ok &= s2.thg[j] <= sh.thr_u[j];
+        s2.guess_ok = ok;
+        if (!ok)
+            for (int j = 0; j < a.nwidths; ++j) put_threshold(s2, j, sh.thr_u[j]);
+    }
+    __syncthreads();
+    if (n_emit <= 0) return;
+    if (!s2.guess_ok && warp > 0) prefilter(X, s2, tid - 32, ngroups, flo, fhi);   // rare: sigma fell by more than a tenth
+
+    // ---- the marked taus: S/N of every width in double, arg-max, threshold, warp-aggregated append ---------------------
+    const int nw = a.nwidths, gid = tid - 32;
+    const int niter = (ngroups + 2 * NTP - 1) / (2 * NTP);
+    if (warp == 0) return;                                // holds no marks
+    for (int it = 0; it < niter; ++it) {
+        const uint32_t any = it < 8 ? (uint32_t)(flo >> (8 * it)) & 0xFFu : (fhi >> (8 * (it - 8))) & 0xFFu;
+        if (!__any_sync(0xffffffffu, any != 0)) continue;
+        const int g = it * 2 * NTP + gid;
+#pragma unroll 1
+        for (int k = 0; k < 8; ++k) {
+            if (!__any_sync(0xffffffffu, (any >> k) & 1u)) continue;
+            const int tl = 4 * (g + (k >> 2) * NTP) + (k & 3);
+            const int64_t tau = s0 + tl;                  // column inside the sub-chunk
+            bool has = false;
+            int best_w = 0;
+            double best = 0.0;
+            if (((any >> k) & 1u) && tl < n_emit) {
+                const uint32_t p0 = X[tl];
+                for (int j = 0; j < nw; ++j) {
+                    const int w = sh.w[j];
+                    if (tau + w > a.nout_left) continue;
+                    const long long B = (long long)(uint32_t)(X[tl + w] - p0);
+                    const double S = __ddiv_rn(__dsub_rn((double)B, __dmul_rn((double)w, mu)), sh.den[j]);
+                    if (best_w == 0 || S > best) { best = S; best_w = w; }
+                }
+                has = (best_w != 0) && (best >= a.thr);
+            }
+            const unsigned mask = __ballot_sync(0xffffffffu, has);
+            if (mask) {
+                uint32_t base = 0;
+                const int leader = __ffs(mask) - 1;
+                if (lane == leader) base = atomicAdd(a.count, (uint32_t)__popc(mask));
+                base = __shfl_sync(0xffffffffu, base, leader);
+                if (has) {
+                    const uint32_t slot = base + __popc(mask & ((1u << lane) - 1));
+                    if (slot < a.cap) {
+                        aa_candidate c;
+                        c.dm_index = a.dm_base + (uint32_t)d;
+                        c.t_start = (a.tau0 + (uint32_t)tau) * a.bin;
+                        c.width = (uint32_t)best_w * a.bin;
+                        c.snr = (float)best;
+                        a.cands[slot] = c;
+                    }
+                }
+            }
+        }
+    }
+}
+
 // cluster size and segment length of the cluster variant; false: use the generic kernel
 bool sps_cluster_shape(const SpsArgs &a, bool wide, int &C, int &seg)
 {
@@ -762,6 +1312,11 @@ bool sps_cluster_shape(const SpsArgs &a, bool wide, int &C, int &seg)
 size_t sps_cluster_smem(const SpsArgs &a, int seg)
 {
     return (size_t)(seg + a.wmax - 1 + 8) * 4;
+}
+
+size_t sps_cluster2_smem(const SpsArgs &a, int seg)
+{
+    return sps_cluster_smem(a, seg) + (size_t)kListTotal * 4;
 }
 
 size_t sps_smem(const SpsArgs &a, bool wide)
@@ -782,12 +1337,14 @@ cudaError_t sps_configure()
     if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(sps_kernel<uint32_t, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024);
     if (e != cudaSuccess) return e;
+    e = cudaFuncSetAttribute(sps_cluster2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
+    if (e != cudaSuccess) return e;
     e = cudaFuncSetAttribute(sps_cluster_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
     if (e != cudaSuccess) return e;
     return cudaFuncSetAttribute(sps_cluster_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 100 * 1024);
 }
 
-cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, bool small31, bool big, cudaStream_t st)
+cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, bool small31, bool big, bool force_v1, cudaStream_t st)
 {
     if (a.nemit <= 0 || a.ndms <= 0) return cudaSuccess;
     const unsigned nblk = (unsigned)((a.nemit + a.block_len - 1) / a.block_len);
@@ -805,6 +1362,13 @@ cudaError_t launch_sps(const SpsArgs &a, const WidthTable &wt, bool wide, bool s
         at[0].val.clusterDim.z = 1;
         cfg.attrs = at;
         cfg.numAttrs = 1;
+        // version 2 serves the search BASELINE.json states: white-noise scaling, every width at every sample
+        bool plain = small31 && a.sigma_mode == 0 && !force_v1;
+        for (int j = 0; j < a.nwidths; ++j) plain = plain && wt.dec[j] == 1;
+        if (plain) {
+            cfg.dynamicSmemBytes = sps_cluster2_smem(a, seg);
+            return cudaLaunchKernelEx(&cfg, sps_cluster2_kernel, a, wt, C, seg);
+        }
         return small31 ? cudaLaunchKernelEx(&cfg, sps_cluster_kernel<true>, a, wt, C, seg)
                        : cudaLaunchKernelEx(&cfg, sps_cluster_kernel<false>, a, wt, C, seg);
     }

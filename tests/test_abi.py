@@ -33,7 +33,7 @@ def test_struct_layouts_match_header():
     # aa_plan_desc: int32 nchans (+pad), u64, 3 doubles, ... natural alignment on LP64
     assert B.PlanDescC.nsamp.offset == 8 and B.PlanDescC.ranges.offset == 48
     assert B.PlanDescC.snr_threshold.offset == 72 and B.PlanDescC.chunk_len.offset == 88
-    assert B.PlanDescC.stage_input.offset == 152 and B.PlanDescC.dedisp_variant.offset == 156 and B.PlanDescC.nbits.offset == 160 and B.PlanDescC.sigma_mode.offset == 168 and B.PlanDescC.output_mode.offset == 172 and ctypes.sizeof(B.PlanDescC) == 176
+    assert B.PlanDescC.stage_input.offset == 152 and B.PlanDescC.dedisp_variant.offset == 156 and B.PlanDescC.nbits.offset == 160 and B.PlanDescC.sigma_mode.offset == 168 and B.PlanDescC.output_mode.offset == 172 and B.PlanDescC.sps_variant.offset == 176 and ctypes.sizeof(B.PlanDescC) == 184
     assert ctypes.sizeof(B.DedispModelC) == 96 and B.DedispModelC.ring_bytes.offset == 80
     assert ctypes.sizeof(B.StatsC) == 144 and B.StatsC.h2h_bytes.offset == 120 and B.StatsC.n_peaks.offset == 136
 

@@ -31,8 +31,10 @@ def _run_gpu(B, w, buf, *, taps="all", **kw):
         return cands, tap, plan.info, plan.nout, plan.stats()
 
 
-def _check_against_oracle(B, w, **kw):
+def _check_against_oracle(B, w, mutate=None, **kw):
     buf, x = _pinned_fill(B, w)
+    if mutate is not None:
+        mutate(x)
     cands, tap, info, nout, _ = _run_gpu(B, w, buf, **kw)
     ref, dense, geo = oracle.run(x, w, keep_dense=True)
     assert info["maxshift"] == geo["maxshift"] and nout == geo["nout"]
@@ -106,6 +108,59 @@ def test_sps_and_corner_turn_variants(B, case):
     """Shapes that select each SPS kernel (cluster sizes 1-8, generic fallback) and each corner-turn kernel."""
     w = _tiny(**case)
     cands, ref, res = _check_against_oracle(B, w)
+    assert res["only_gpu"] == 0 and res["only_oracle"] == 0 and res["width_ties"] == 0
+    assert len(ref) > 0
+
+
+def _interference(kind):
+    """Input rows that defeat the fast statistics path of sps_cluster2_kernel (listed outliers + totals): the kernel
+    must then walk the whole segment for the remaining clip passes and still return the oracle's numbers."""
+    def mutate(x):
+        nsamp = x.shape[0]
+        if kind == "burst":            # 12 % of one stretch far above the noise: the outlier lists overflow
+            a = nsamp // 3
+            x[a:a + nsamp // 8, :] = 250
+        elif kind == "spikes":         # a few enormous samples: sigma collapses after the first clip, the 3-sigma interval
+            x[nsamp // 5::997, :] = 255    # of the next pass falls inside the core of the first guess
+            x[nsamp // 7::1013, :] = 0
+        elif kind == "constant":       # sigma = 0 over whole blocks: nothing may be emitted there
+            x[: nsamp // 2, :] = 77
+        elif kind == "steps":          # two levels: the plain moments put the core between them
+            x[::2, :] = 10
+            x[1::2, :] = 240
+        elif kind == "dense_spikes":   # 5 % of the samples four sigma out: more listed samples than a cluster's lists hold
+            x[3::20, :] = 255
+        elif kind == "almost_constant":  # sigma far below one count: no integer lies within 2.75 sigma of the mean
+            x[:, :] = 77
+            x[nsamp // 3, 0] = 78
+            x[nsamp // 3 + 40000, 1] = 79
+    return mutate
+
+
+@pytest.mark.parametrize("sps_variant", [0, 1])
+@pytest.mark.parametrize("kind", ["burst", "spikes", "constant", "steps", "dense_spikes", "almost_constant"])
+@pytest.mark.parametrize("case", [
+    dict(norm_block=16384, chunk_len=16384, nsamp=70000, ndms=6),             # one CTA per block
+    dict(norm_block=65536, chunk_len=65536, nsamp=200001, ndms=4),            # cluster of 4, ragged last block
+    dict(norm_block=131072, chunk_len=131072, nsamp=300000, ndms=3),          # cluster of 8
+])
+def test_sps_statistics_under_interference(B, case, kind, sps_variant):
+    """Both cluster kernels (sps_variant 1 keeps the first one) on rows whose statistics take the slow path."""
+    w = _tiny(**case)
+    cands, ref, res = _check_against_oracle(B, w, mutate=_interference(kind), sps_variant=sps_variant)
+    assert res["only_gpu"] == 0 and res["only_oracle"] == 0 and res["width_ties"] == 0
+
+
+@pytest.mark.parametrize("case", [
+    dict(norm_block=32768, chunk_len=32768, nsamp=150000, ndms=6),
+    dict(norm_block=65536, chunk_len=65536, nsamp=200001, ndms=5),
+    dict(widths=(2, 6, 7, 12, 20, 33), thr=4.5, norm_block=4096, chunk_len=8192),
+    dict(widths=(1, 2, 3, 4, 8, 9), thr=4.5, norm_block=8192, chunk_len=8192, nsamp=40000),
+])
+def test_first_cluster_kernel_still_matches(B, case):
+    """aa_plan_desc.sps_variant = 1: sps_cluster_kernel where sps_cluster2_kernel would run."""
+    w = _tiny(**case)
+    cands, ref, res = _check_against_oracle(B, w, sps_variant=1)
     assert res["only_gpu"] == 0 and res["only_oracle"] == 0 and res["width_ties"] == 0
     assert len(ref) > 0
 
