@@ -322,7 +322,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--per-config", default="auto",
                     help="comma-separated other configs to run end to end after the main workload (3 steps each) and "
-                         "report under per_config; 'auto' = 2,4,5 for the default single-GPU run of workload 3, 'none' = skip")
+                         "report under per_config; 'auto' = 1,2,4,5 for the default single-GPU run of workload 3, 'none' = skip")
     ap.add_argument("--shard-observation", action="store_true",
                     help="strong scaling: ONE observation split by time over the ranks (whole normalisation blocks + halo "
                          "per rank, candidate lists gathered on rank 0); default: one observation per rank (weak)")
@@ -343,12 +343,12 @@ def main():
     from paper_2101_00941_b200 import binding as B
 
     rank, world, local = dist_env()
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
-    torch.cuda.set_device(local)
     from paper_2101_00941_b200 import dist_util
     placement = dist_util.place_rank(local, world)          # NUMA node of the GPU: host threads and first touch
     print(f"[bench] rank {rank}/{world} gpu {local}: {placement}", file=sys.stderr)
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback)")
+    torch.cuda.set_device(local)
     dist_util.init("nccl", device=torch.device("cuda", local))
     B.load_library()
 
@@ -534,7 +534,7 @@ def main():
     # ---- the other configs of BASELINE.json, end to end (north_star: "the 4096-channel configs") ----
     pcs = args.per_config
     if pcs == "auto":
-        pcs = "2,4,5" if (world == 1 and args.workload == 3 and not args.nsamp and not args.shard_observation
+        pcs = "1,2,4,5" if (world == 1 and args.workload == 3 and not args.nsamp and not args.shard_observation
                           and args.nbits == 8) else "none"
     if rank == 0 and pcs != "none":
         line["per_config"] = {}

@@ -82,7 +82,9 @@ def place_rank(local: int, world: int) -> dict:
         if world > 1 or node_cpus:
             os.sched_setaffinity(0, cpus)
         info.update({"numa_node": node, "cpus": len(cpus)})
-        if "OMP_NUM_THREADS" not in os.environ:
+        # torchrun exports OMP_NUM_THREADS=1 to every rank unless the user set it: that would fill 34 GB per rank with one
+        # thread; a value of 1 under torchrun is therefore read as "not chosen" and replaced by the rank's share of cores
+        if "OMP_NUM_THREADS" not in os.environ or (world > 1 and os.environ["OMP_NUM_THREADS"] == "1"):
             os.environ["OMP_NUM_THREADS"] = str(max(1, len(cpus)))
         info["omp_threads"] = int(os.environ["OMP_NUM_THREADS"])
     except Exception as e:                                  # placement is an optimisation, never a failure
