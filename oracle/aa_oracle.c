@@ -24,8 +24,12 @@
  * vs its closed form; candidate rule vs python loops.
  * Parity unpinned against the paper (the paper fixes none of them): the choice
  * of estimator (A8), the norm-block length (A9), the candidate definition
- * (A11).  They are conventions of this build, pinned only to their own written
- * definition by brute force.
+ * (A11), the peak rule (A17, aaor_find_peaks), the per-width statistics (A18,
+ * aaor_series_stats / aaor_sps_row2), the packing of other bit depths (A19,
+ * aaor_bin_u16 and the unpackers of __init__.py) and the grid of long widths
+ * (A20, aaor_sps_row2).  They are conventions of this build, pinned only to
+ * their own written definition: python-loop brute force, exact fractions,
+ * closed forms, hand-made cases (tests/test_oracle_pins.py).
  *
  * Floating point: double everywhere, no FMA contraction (compile with
  * -ffp-contract=off), statistics from exact integer sums so that the only
