@@ -1126,10 +1126,20 @@ __global__ void __launch_bounds__(NT2) sps_cluster2_kernel(const SpsArgs a, cons
         uint64_t n = 0, T1 = 0;
         unsigned __int128 T2 = 0;
         bool listed_ok = true;
+        uint32_t lcmin = 0xFFFFFFFFu, hcmax = 0u;         // an interval contains every core iff it contains [lcmin, hcmax]
         for (int r = 0; r < C; ++r) {
             n += s2.part2[r][0]; T1 += s2.part2[r][1]; T2 += s2.part2[r][2];
             if (s2.part2[r][5]) listed_ok = false;
+            if (s2.part2[r][0]) {
+                const uint64_t ch = s2.part2[r][3];
+                lcmin = min(lcmin, (uint32_t)ch);
+                hcmax = max(hcmax, (uint32_t)(ch >> 32));
+            }
         }
+        // the lists: 32 / C lanes walk the list of each rank
+        const int lpr = 32 / C, lr = lane / lpr, l0 = lane % lpr;
+        const int cnt = (int)s2.part2[lr][4];
+        const uint32_t *L = LST + lr * lreg;
         double mu = 0.0, sigma = 0.0;
         int slow = 0;
         if (n) {
@@ -1137,32 +1147,26 @@ __global__ void __launch_bounds__(NT2) sps_cluster2_kernel(const SpsArgs a, cons
             for (int pass = 1; pass < 4; ++pass) {
                 uint32_t lo = 0, hi = 0;
                 if (!clip_interval(mu, __dmul_rn(3.0, sigma), lo, hi)) break;   // nothing selected: keep the last values
-                bool covered = listed_ok;
-                for (int r = 0; r < C; ++r) {
-                    const uint64_t ch = s2.part2[r][3];
-                    if (s2.part2[r][0] && !(lo <= (uint32_t)ch && hi >= (uint32_t)(ch >> 32))) covered = false;
-                }
-                if (!covered) { slow = pass; break; }
+                if (!(listed_ok && lo <= lcmin && hi >= hcmax)) { slow = pass; break; }
                 const uint32_t span = hi - lo;
                 uint64_t mr = 0, R1 = 0, R2 = 0, carry = 0;   // the listed samples the interval rejects
-                for (int r = 0; r < C; ++r) {
-                    const int cnt = (int)s2.part2[r][4];
-                    const uint32_t *L = LST + r * lreg;
-#pragma unroll 4
-                    for (int e = lane; e < cnt; e += 32) {
-                        const uint32_t x = L[e];
-                        const bool rej = (x - lo) > span;
-                        const uint32_t xr = rej ? x : 0u;
-                        mr += rej ? 1u : 0u;
-                        R1 += xr;
-                        const uint64_t sq = (uint64_t)xr * xr;
-                        R2 += sq;
-                        carry += R2 < sq;
-                    }
+#pragma unroll 1
+                for (int e = l0; e < cnt; e += lpr) {
+                    const uint32_t x = L[e];
+                    const bool rej = (x - lo) > span;
+                    const uint32_t xr = rej ? x : 0u;
+                    mr += rej ? 1u : 0u;
+                    R1 += xr;
+                    const uint64_t sq = (uint64_t)xr * xr;
+                    R2 += sq;
+                    carry += R2 < sq;
                 }
-                mr = warp_sum_all(mr); R1 = warp_sum_all(R1);
+                // one butterfly for the small numbers (count and carries: below 2^16 each), one for each 64-bit sum
+                uint64_t mc = warp_sum_all(mr | (carry << 32));
+                R1 = warp_sum_all(R1);
                 const uint64_t r2lo = warp_sum_all(R2 & 0xFFFFFFFFull), r2hi = warp_sum_all(R2 >> 32);
-                carry = warp_sum_all(carry);
+                mr = mc & 0xFFFFFFFFull;
+                carry = mc >> 32;
                 const unsigned __int128 R2w = (unsigned __int128)r2lo + ((unsigned __int128)r2hi << 32) + ((unsigned __int128)carry << 64);
                 const uint64_t m = n - mr;
                 if (!m) break;
