@@ -782,7 +782,6 @@ struct SharedC2 {
     int slow_from;                       // 0: statistics done by warp 0; k: passes k..3 take the slow path
     uint32_t ths[4];                     // pre-filter thresholds of widths 1, 2, 3 (index w; "never" if the width is not searched)
     int slot[kMaxWidths];                // where width j's threshold lives: wl index, or -w for the widths below 4
-    int dup;                             // wl index that repeats the last aligned width (-1: none)
     uint32_t thg[kMaxWidths];            // guessed thresholds (plain), for the check against thr_u
     int nsm, guess_ok;
 };
@@ -797,7 +796,7 @@ __device__ __forceinline__ uint32_t enc_thr(uint32_t th) { return th == 0u ? 0xF
 __device__ __forceinline__ void prefilter(const uint32_t *X, const SharedC2 &s2, int gid, int ngroups, uint64_t &flo, uint32_t &fhi)
 {
     const SharedC &sh = s2.c;
-    const int na2 = (sh.na + 1) & ~1, nu = sh.nu, nsm = s2.nsm;
+    const int na = sh.na, nu = sh.nu, nsm = s2.nsm;
     constexpr int GB = 4 * NTP;
     flo = 0ull;
     fhi = 0u;
@@ -825,7 +824,7 @@ __device__ __forceinline__ void prefilter(const uint32_t *X, const SharedC2 &s2,
         }
         // widths that are multiples of 4: aligned 16-byte loads, two widths per round (one 3-input OR takes both)
 #pragma unroll 2
-        for (int j = 0; j < na2; j += 2) {
+        for (int j = 0; j + 1 < na; j += 2) {
             const uint4 w0 = sh.wl[j], w1 = sh.wl[j + 1];
             const uint4 qa = *reinterpret_cast<const uint4 *>(xg + w0.x), qb = *reinterpret_cast<const uint4 *>(xg + w0.x + gb);
             const uint4 ra = *reinterpret_cast<const uint4 *>(xg + w1.x), rb = *reinterpret_cast<const uint4 *>(xg + w1.x + gb);
@@ -835,9 +834,16 @@ __device__ __forceinline__ void prefilter(const uint32_t *X, const SharedC2 &s2,
             f4 |= (t0 + pb.x - qb.x) | (t1 + pb.x - rb.x); f5 |= (t0 + pb.y - qb.y) | (t1 + pb.y - rb.y);
             f6 |= (t0 + pb.z - qb.z) | (t1 + pb.z - rb.z); f7 |= (t0 + pb.w - qb.w) | (t1 + pb.w - rb.w);
         }
+        if (na & 1) {                                     // an odd count: the last one alone
+            const uint4 w0 = sh.wl[na - 1];
+            const uint4 qa = *reinterpret_cast<const uint4 *>(xg + w0.x), qb = *reinterpret_cast<const uint4 *>(xg + w0.x + gb);
+            const uint32_t t0 = w0.y;
+            f0 |= t0 + pa.x - qa.x; f1 |= t0 + pa.y - qa.y; f2 |= t0 + pa.z - qa.z; f3 |= t0 + pa.w - qa.w;
+            f4 |= t0 + pb.x - qb.x; f5 |= t0 + pb.y - qb.y; f6 |= t0 + pb.z - qb.z; f7 |= t0 + pb.w - qb.w;
+        }
         // the others: the aligned pieces around tau + w, shifted by w mod 4 (uniform)
 #pragma unroll 1
-        for (int j = na2; j < na2 + nu; ++j) {
+        for (int j = na; j < na + nu; ++j) {
             const uint4 wt2 = sh.wl[j];
             const uint32_t th = wt2.y;
             const int r = (int)(wt2.x & 3u);
@@ -869,7 +875,6 @@ __device__ __forceinline__ void put_threshold(SharedC2 &s2, int j, uint32_t th)
         s2.ths[-sl] = e;
     } else {
         s2.c.wl[sl].y = e;
-        if (s2.dup >= 0 && sl == s2.dup - 1) s2.c.wl[s2.dup].y = e;
     }
 }
 
@@ -939,7 +944,7 @@ __global__ void __launch_bounds__(NT2) sps_cluster2_kernel(const SpsArgs a, cons
     }
     if (tid == 32) {
         // width classes of the pre-filter: below 4 (from the neighbouring piece), multiples of 4 (aligned loads, taken two
-        // at a time: an odd count repeats the last one), the rest
+        // at a time), the rest
         int n = 0, nsm = 0;
         s2.ths[0] = s2.ths[1] = s2.ths[2] = s2.ths[3] = kNever;
         for (int j = 0; j < a.nwidths; ++j)
@@ -948,12 +953,10 @@ __global__ void __launch_bounds__(NT2) sps_cluster2_kernel(const SpsArgs a, cons
         for (int j = 0; j < a.nwidths; ++j)
             if ((wt.w[j] & 3) == 0) { s2.slot[j] = n; sh.wl[n++] = make_uint4((uint32_t)wt.w[j], kNever, 1u, 0u); }
         sh.na = n;
-        s2.dup = -1;
-        if (n & 1) { s2.dup = n; sh.wl[n] = sh.wl[n - 1]; }
-        int q = (n + 1) & ~1;
+        int q = n;
         for (int j = 0; j < a.nwidths; ++j)
             if (wt.w[j] > 4 && (wt.w[j] & 3) != 0) { s2.slot[j] = q; sh.wl[q++] = make_uint4((uint32_t)wt.w[j], kNever, 1u, 0u); }
-        sh.nu = q - ((n + 1) & ~1);
+        sh.nu = q - n;
     }
     __syncthreads();
     // every CTA of the cluster must be running before its shared memory is written: arrive now, wait before the first remote store
@@ -1032,10 +1035,10 @@ __global__ void __launch_bounds__(NT2) sps_cluster2_kernel(const SpsArgs a, cons
     uint32_t lc = 1u, hc = 0u;                            // empty core: everything is listed (-> slow path)
     if (n_own > 0) {
         const double kcore = 2.75;                        // 0.6 % of white noise outside: about 100 listed samples per segment
-        const double nn = (double)n_own, mean = (double)S1 / nn;
-        double var = (double)S2 / nn - mean * mean;       // a guess: need not be exact
+        const double inv = 1.0 / (double)n_own, mean = (double)S1 * inv;
+        double var = (double)S2 * inv - mean * mean;      // a guess: need not be exact
         if (!(var > 0.0)) var = 0.0;
-        const double sd = sqrt(var);
+        const double sd = (double)sqrtf((float)var);
         double l = ceil(mean - kcore * sd), h = floor(mean + kcore * sd);
         if (l < 0.0) l = 0.0;
         if (h > 4294967295.0) h = 4294967295.0;
