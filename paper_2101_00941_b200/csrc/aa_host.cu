@@ -88,6 +88,7 @@ struct Stream {
     std::vector<cudaEvent_t> ev;      // timing events
     struct TapCopy { int row; uint64_t tau0, n, off; };
     std::vector<TapCopy> tapcopies;   // capacity = ntap, reserved at plan creation; refilled per sub-chunk
+    std::vector<uint32_t> sort_cur;   // [ndms_total + 1] cursors of the per-sub-chunk counting sort (sized at plan creation)
     // per-run accumulators
     double h2d_ms = 0, d2h_ms = 0, prep_ms = 0, dedisp_ms = 0, sps_ms = 0, h2h_ms = 0;
     uint64_t h2d_bytes = 0, d2h_bytes = 0, dedisp_launches = 0, sps_launches = 0, prep_launches = 0, h2h_bytes = 0;
@@ -830,20 +831,51 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
         uint64_t m = 0;
         if (pos < max_cands) {
             m = std::min<uint64_t>(n, max_cands - pos);
-            if (m) {
-                std::memcpy(out + pos, S.h_cands, m * sizeof(aa_candidate));
-                std::sort(out + pos, out + pos + m, cand_less);
-            }
         }
         {
-            // where each trial starts inside this run
+            // The kernel appends in no particular order.  The key (trial, start inside the sub-chunk) has few bits, so the
+            // run is put in order by a least-significant-digit radix sort that ping-pongs between the pinned staging and the
+            // caller's buffer (11 bits per pass, no other memory), instead of one m log m comparison sort; the table of
+            // where each trial starts inside this run, which the final interleave needs, comes from one more histogram.
             p->runs[j].pos = pos < max_cands ? pos : max_cands;
             p->runs[j].n = m;
-            uint32_t *cnt = &p->run_cnt[j * (uint64_t)(p->ndms_total + 1)];
-            uint64_t i = 0;
-            for (uint32_t d = 0; d <= p->ndms_total; ++d) {
-                while (i < m && (out[pos + i].dm_index & kPeakDmMask) < d) ++i;
-                cnt[d] = (uint32_t)i;
+            const uint32_t nd = p->ndms_total;
+            uint32_t *cnt = &p->run_cnt[j * (uint64_t)(nd + 1)];
+            uint32_t *cur = S.sort_cur.data();
+            aa_candidate *dst = out + pos, *src = S.h_cands;
+            int tbits = 1, dbits = 1;
+            while ((1ull << tbits) < L) ++tbits;
+            while ((1u << dbits) < nd) ++dbits;
+            const uint64_t t_sub = j * L;
+            auto key = [&](const aa_candidate &c) {
+                return ((uint64_t)(c.dm_index & kPeakDmMask) << tbits) | (uint64_t)(c.t_start - (uint32_t)t_sub);
+            };
+            bool in_range = true;
+            std::fill(cur, cur + nd + 1, 0u);
+            for (uint64_t i = 0; i < m; ++i) {
+                const aa_candidate &c = src[i];
+                const uint32_t d = c.dm_index & kPeakDmMask;
+                in_range = in_range && d < nd && (uint64_t)(c.t_start - (uint32_t)t_sub) < (1ull << tbits);
+                cur[std::min<uint32_t>(d, nd - 1) + 1]++;
+            }
+            for (uint32_t d = 0; d < nd; ++d) cur[d + 1] += cur[d];      // cur[d] = first record of trial d
+            std::memcpy(cnt, cur, (size_t)(nd + 1) * sizeof(uint32_t));
+            if (m && !in_range) {                       // never expected: keep the plain sort for it
+                std::memcpy(dst, src, m * sizeof(aa_candidate));
+                std::sort(dst, dst + m, cand_less);
+            } else if (m) {
+                constexpr int kDigit = 11;
+                uint32_t hist[1 << kDigit];
+                aa_candidate *a = src, *b = dst;
+                for (int shift = 0; shift < tbits + dbits; shift += kDigit) {
+                    std::memset(hist, 0, sizeof(hist));
+                    for (uint64_t i = 0; i < m; ++i) hist[(key(a[i]) >> shift) & ((1u << kDigit) - 1)]++;
+                    uint32_t run = 0;
+                    for (uint32_t &h : hist) { const uint32_t c = h; h = run; run += c; }
+                    for (uint64_t i = 0; i < m; ++i) b[hist[(key(a[i]) >> shift) & ((1u << kDigit) - 1)]++] = a[i];
+                    std::swap(a, b);
+                }
+                if (a != dst) std::memcpy(dst, a, m * sizeof(aa_candidate));
             }
         }
         if (tap_out && !tapcopies.empty()) {
@@ -1209,7 +1241,10 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
     for (auto &R : p->ranges) p->ndms_total += (uint32_t)R.r.ndms;
     p->nactive = (int)std::min<uint64_t>((uint64_t)p->n_streams, p->n_sub);
     try {
-        for (auto &S : p->streams) S.tapcopies.reserve((size_t)std::max(1, d->ntap));
+        for (auto &S : p->streams) {
+            S.tapcopies.reserve((size_t)std::max(1, d->ntap));
+            S.sort_cur.assign((size_t)p->ndms_total + 1, 0u);
+        }
         p->runs.assign(p->n_sub, aa_plan::Run{});
         p->run_cnt.assign(p->n_sub * (uint64_t)(p->ndms_total + 1), 0u);
         p->dm_dst.assign((size_t)p->ndms_total + 1, 0);
