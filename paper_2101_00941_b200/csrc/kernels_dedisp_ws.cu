@@ -55,7 +55,7 @@ static_assert(NCW * REG_CONS + NPW * REG_PROD <= (NCW + NPW) * 80, "register bud
 // its first word).  q: this lane's first window byte of channel 0, chunk offset included; dst: shared
 // address of this lane's four words of pattern 0's even copy; st: this lane stores; rowbytes: bytes per copy.
 template <int NPAT, int K0>
-__device__ __forceinline__ void build_batch(const WsRecord *R, const uint8_t *q, uint32_t dst, uint32_t st, uint32_t rowbytes)
+__device__ __forceinline__ void build_batch(const uint32_t (&cds)[G], const WsRecord *Rr, const uint8_t *q, uint32_t dst, uint32_t st, uint32_t rowbytes)
 {
     uint32_t acc[NPAT][4];
 #pragma unroll
@@ -65,7 +65,7 @@ __device__ __forceinline__ void build_batch(const WsRecord *R, const uint8_t *q,
 
 #pragma unroll
     for (int i = 0; i < G; ++i) {
-        const uint32_t cd = R->chdesc[i];
+        const uint32_t cd = cds[i];
         const uint8_t *qi = q + (cd & 0xFFFFu);
         const uint2 v0 = *reinterpret_cast<const uint2 *>(qi);
         const uint2 v1 = *reinterpret_cast<const uint2 *>(qi + 8);
@@ -76,7 +76,7 @@ __device__ __forceinline__ void build_batch(const WsRecord *R, const uint8_t *q,
         const uint32_t xs0 = __funnelshift_r(t0, t1, sh), xs1 = __funnelshift_r(t1, t2, sh),
                        xs2 = __funnelshift_r(t2, t3, sh);
         uint2 es = make_uint2(0, 0);
-        if (i > 0) es = *reinterpret_cast<const uint2 *>(R->esh[i]);
+        if (i > 0) es = *reinterpret_cast<const uint2 *>(Rr->esh[i]);
 #pragma unroll
         for (int k = 0; k < NPAT; ++k) {
             uint32_t x0 = xs0, x1 = xs1;
@@ -113,7 +113,7 @@ __device__ __forceinline__ void build_batch(const WsRecord *R, const uint8_t *q,
 // them to the channel's smallest shift (word select + 16-bit funnel shift) and per pattern shifts by the
 // extra e_{k,i} <= 2 samples with one PRMT (selector 0x3210 + e * 0x2222: 0, 2 or 4 bytes into the word pair).
 template <int NPAT, int K0>
-__device__ __forceinline__ void build_batch16(const WsRecord *R, const uint8_t *q, uint32_t dst, uint32_t st, uint32_t rowbytes)
+__device__ __forceinline__ void build_batch16(const uint32_t (&cds)[G], const WsRecord *Rr, const uint8_t *q, uint32_t dst, uint32_t st, uint32_t rowbytes)
 {
     uint32_t acc[NPAT][4];
 #pragma unroll
@@ -123,7 +123,7 @@ __device__ __forceinline__ void build_batch16(const WsRecord *R, const uint8_t *
 
 #pragma unroll
     for (int i = 0; i < G; ++i) {
-        const uint32_t cd = R->chdesc[i];
+        const uint32_t cd = cds[i];
         const uint8_t *qi = q + (cd & 0xFFFFu);
         const uint2 v0 = *reinterpret_cast<const uint2 *>(qi);
         const uint2 v1 = *reinterpret_cast<const uint2 *>(qi + 8);
@@ -137,7 +137,7 @@ __device__ __forceinline__ void build_batch16(const WsRecord *R, const uint8_t *
         const uint32_t t0 = __funnelshift_r(a0, a1, f), t1 = __funnelshift_r(a1, a2, f), t2 = __funnelshift_r(a2, a3, f),
                        t3 = __funnelshift_r(a3, a4, f), t4 = __funnelshift_r(a4, a5, f);
         uint2 es = make_uint2(0, 0);
-        if (i > 0) es = *reinterpret_cast<const uint2 *>(R->esh[i]);
+        if (i > 0) es = *reinterpret_cast<const uint2 *>(Rr->esh[i]);
 #pragma unroll
         for (int k = 0; k < NPAT; ++k) {
             uint32_t x0 = t0, x1 = t1, x2 = t2, x3 = t3;
@@ -173,18 +173,30 @@ __device__ __forceinline__ void build_stage(const WsRecord *R, const uint8_t *ra
                                             uint32_t nbatch, int member, int lane)
 {
     const uint32_t rowbytes = 16u * nchunk;
+    // the stage's channel descriptors stay in registers over the batches (one uniform load and its latency less per
+    // channel and batch: 25.88 -> 25.36 ms per cfg3 launch); the extra shifts too would spill (measured: slower)
+    // (16-bit input keeps more values alive per lane and would spill: it reads them in every batch)
+    uint32_t cds[G];
+    if (!IN16) {
+#pragma unroll
+        for (int i = 0; i < G; ++i) cds[i] = R->chdesc[i];
+    }
     for (uint32_t b = (uint32_t)member; b < nbatch; b += TEAM) {
+        if (IN16) {
+#pragma unroll
+            for (int i = 0; i < G; ++i) cds[i] = R->chdesc[i];
+        }
         const uint32_t chunk = b * 31u + (uint32_t)lane;
         // chunk nchunk is read for its first sample only; nothing beyond it is read
         const uint8_t *q = rawslot + (IN16 ? 16u : 8u) * (chunk < nchunk ? chunk : nchunk);
         const uint32_t dst = P + 16u * chunk;
         const uint32_t st = lane < 31 && chunk < nchunk;
         if (IN16) {
-            build_batch16<NPAT_LO, 0>(R, q, dst, st, rowbytes);
-            if (NPAT_HI > 0) build_batch16<(NPAT_HI > 0 ? NPAT_HI : 1), NPAT_LO>(R, q, dst, st, rowbytes);
+            build_batch16<NPAT_LO, 0>(cds, R, q, dst, st, rowbytes);
+            if (NPAT_HI > 0) build_batch16<(NPAT_HI > 0 ? NPAT_HI : 1), NPAT_LO>(cds, R, q, dst, st, rowbytes);
         } else {
-            build_batch<NPAT_LO, 0>(R, q, dst, st, rowbytes);
-            if (NPAT_HI > 0) build_batch<(NPAT_HI > 0 ? NPAT_HI : 1), NPAT_LO>(R, q, dst, st, rowbytes);
+            build_batch<NPAT_LO, 0>(cds, R, q, dst, st, rowbytes);
+            if (NPAT_HI > 0) build_batch<(NPAT_HI > 0 ? NPAT_HI : 1), NPAT_LO>(cds, R, q, dst, st, rowbytes);
         }
     }
 }
