@@ -242,6 +242,19 @@ def test_cfg5_reduced_length_sampled_16_streams(B):
     assert n_cells >= 5
 
 
+@pytest.mark.parametrize("variant", [dict(nbits=4), dict(nbits=16), dict(sigma_mode=1), dict(wdec=16), dict(sigma_mode=1, wdec=16)],
+                         ids=["4bit", "16bit", "measured-sigma", "decimated-widths", "measured-sigma+decimated"])
+def test_cfg3_shape_search_variants_sampled(B, variant):
+    """The S:8(f) rows (readings A18-A20) on the headline workload's shape: 4096 channels, 2048 trials, 131072-sample
+    sub-chunks on 4 streams, the kernels bench.py times plus the ones these variants select (per-width statistics and
+    coarse grids in the first cluster kernel, 64-bit boxcar sums for 16-bit input); sampled rows x blocks against the oracle."""
+    w = I.scaled(I.workload(3), nsamp=1 << 19, chunk_len=1 << 19, n_streams=4, name="cfg3_short", **variant)
+    w = I.scaled(w, pulses=(I.Pulse(dm=300.0, t0=150000, width=16, amp=0.35), I.Pulse(dm=1500.0, t0=300000, width=128, amp=0.12)))
+    extra = [(0, [0, 1023, 2047], 0), (0, [7, 640], 3), (0, [0, 2047], 7)]      # block 7 is the ragged last one
+    cands, n_cells, n_ref, _ = _run_sampled(B, w, extra, max_pulses=2)
+    assert n_cells >= 10 and n_ref > 0
+
+
 @pytest.mark.skipif(not _full(60), reason="needs 34.4 GB pinned + headroom (AA_FULL=1 forces it)")
 def test_cfg4_full_size_sampled(B):
     w = I.workload(4)
