@@ -17,7 +17,7 @@ LIB = os.path.join(HERE, "libaa.so")
 
 NVCC_FLAGS = [
     "-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
-    "-Xcompiler", "-fPIC,-ffp-contract=off,-pthread", "--fmad=true", "-shared",
+    "-Xcompiler", "-fPIC,-ffp-contract=off,-pthread", "--fmad=true", "-shared", "-ldl",
 ]
 
 

@@ -20,6 +20,8 @@
 #include <thread>
 #include <vector>
 
+#include <nvtx3/nvToolsExt.h>
+
 #include "aa_internal.h"
 
 using namespace aa;
@@ -556,6 +558,15 @@ void destroy_plan(aa_plan *p)
     delete p;
 }
 
+// NVTX ranges: a profiler's timeline shows the call and, per stream thread, every sub-chunk; without a
+// profiler attached the calls return at once
+struct NvtxRange {
+    explicit NvtxRange(const char *name) { nvtxRangePushA(name); }
+    ~NvtxRange() { nvtxRangePop(); }
+    NvtxRange(const NvtxRange &) = delete;
+    NvtxRange &operator=(const NvtxRange &) = delete;
+};
+
 // order of the returned list: (dm_index, t_start); the two top bits of dm_index may carry peak flags on the way
 inline bool cand_less(const aa_candidate &a, const aa_candidate &b)
 {
@@ -616,6 +627,7 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
     if (staged && (uint64_t)s < p->n_sub) stage((uint64_t)s);
 
     for (uint64_t j = (uint64_t)s; j < p->n_sub; j += (uint64_t)p->n_streams) {
+        NvtxRange nvtx_sub("aa: sub-chunk (H2D, corner turn, dedispersion, SPS, D2H, host stage)");
         // the new rows overwrite ring columns last read by sub-chunks j-n_streams-1 and j-n_streams
         if (j >= (uint64_t)p->n_streams + 1 && !wait_flag(p, p->done[j - p->n_streams - 1])) return;
 
@@ -1073,6 +1085,7 @@ int run_impl(aa_plan *p, const uint8_t *input, Input mode, aa_candidate *out, ui
     if (!p || !input || !n_cands || (!out && max_cands)) return AA_ERR_INVALID;
     if (tap_out && p->taps_in.empty()) return AA_ERR_INVALID;
     g_last_cuda_error = 0;
+    NvtxRange nvtx_run(resident ? "aa_run_resident" : mode == Input::staged ? "aa_run_staged" : "aa_run");
     cudaPointerAttributes at{};
     cudaError_t pe = cudaPointerGetAttributes(&at, input);
     if (pe != cudaSuccess) { cudaGetLastError(); at.type = cudaMemoryTypeUnregistered; }
