@@ -1,0 +1,88 @@
+"""GPU parity on seeded random shapes: channels, trials, DM step, band, time bins, normalisation block, streams, width
+lists, thresholds, bit depth, the A18 / A20 search variants, both cluster SPS kernels and rows of interference, drawn
+from one seeded generator and compared with the oracle element by element (dense plane bit-exact, candidates by
+tests/_compare.py).  The fixed cases of test_gpu_parity.py name what they cover; these cover what nobody thought of."""
+import random
+
+import numpy as np
+import pytest
+
+import oracle
+from paper_2101_00941_b200 import inputs as I
+from _compare import compare_candidates
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def B():
+    from paper_2101_00941_b200 import binding
+    binding.load_library()
+    return binding
+
+
+def _draw(rng, it):
+    bins = rng.choice([(1,), (1,), (2,), (4,), (1, 2), (8,)])
+    nb = max(rng.choice([1024, 2048, 4096, 8192, 16384, 32768, 65536, 131072]), 128 * max(bins))
+    n_streams = rng.choice([1, 1, 2, 3])
+    nchans = rng.choice([8, 16, 30, 64, 100, 300, 512])
+    ndms = rng.choice([5, 17, 40, 64, 70, 130])
+    dm_step = rng.choice([0.25, 1.0, 3.0])
+    foff = rng.choice([-4.0, -0.5, -0.2])
+    widths = rng.choice([(1, 2, 4, 8), (1, 2, 4, 8, 16, 32, 64), (1, 3, 5, 32), (2, 6, 7, 12, 20, 33), (4, 8, 256), (1, 2, 3), (1,),
+                         (8, 16, 24), (1, 2, 4, 8, 16, 32, 64, 128, 256)])
+    thr = rng.choice([4.0, 5.0, 6.0])
+    chunk = nb * rng.choice([1, 1, 2]) * n_streams
+    nsamp = rng.randint(chunk + 3000, 3 * chunk + 20000)
+    kind = rng.choice([None, None, None, "spikes", "burst", "constant"])
+    sps_variant = rng.choice([0, 0, 1])
+    nbits = rng.choice([8, 8, 8, 4, 16])
+    wdec = rng.choice([0, 0, 0, 2, 8])
+    sigma_mode = rng.choice([0, 0, 0, 1])
+    if nbits == 4 and nchans % 2:
+        nchans += 1
+    if nbits != 8:
+        kind = None
+    ranges, lo = [], 0.0
+    for b in bins:
+        ranges.append(I.DMRange(lo, dm_step, ndms, b))
+        lo += dm_step * ndms
+    w = I.Workload(name=f"random{it}", nchans=nchans, nsamp=nsamp, tsamp=64e-6, f_top=1500.0, foff=foff, ranges=tuple(ranges),
+                   widths=widths, snr_threshold=thr, n_streams=n_streams, chunk_len=chunk, noise_seed=1000 + it,
+                   pulses=(I.Pulse(dm=dm_step * ndms * 0.4, t0=nsamp // 3, width=4, amp=4.0),), norm_block=nb)
+    return I.scaled(w, nbits=nbits, wdec=wdec, sigma_mode=sigma_mode), kind, sps_variant
+
+
+@pytest.mark.parametrize("seed", [2, 3, 4, 5])
+def test_random_shapes_match_the_oracle(B, seed):
+    rng = random.Random(seed)
+    ran = 0
+    for it in range(40):
+        w, kind, sps_variant = _draw(rng, it)
+        if w.f_top + (w.nchans - 1) * w.foff <= 100.0:
+            continue                                   # the band would reach zero frequency
+        buf = B.pinned_empty(w.nbytes)
+        x = buf.numpy().reshape(w.nsamp, w.row_bytes)
+        I.fill(w, x)
+        if kind == "spikes":
+            x[w.nsamp // 5::997, :] = 255
+        elif kind == "burst":
+            x[w.nsamp // 3: w.nsamp // 3 + w.nsamp // 8, :] = 250
+        elif kind == "constant":
+            x[: w.nsamp // 2, :] = 77
+        try:
+            plan = B.Plan(w, taps=list(range(w.ndms_total)), sps_variant=sps_variant, max_cands_per_subchunk=1 << 23)
+        except RuntimeError:
+            continue                                   # e.g. sub-chunk shorter than the DM sweep, A18 on a block no cluster takes
+        with plan:
+            cands, tap = plan.run(buf, max_cands=1 << 24)
+            assert not plan.overflow, (seed, it)
+        ref, dense, geo = oracle.run(x, w, keep_dense=True)
+        base = 0
+        for r, rg in enumerate(w.ranges):
+            assert np.array_equal(tap[base:base + rg.ndms, :geo["nout"][r]], dense[r]), (seed, it, r)
+            base += rg.ndms
+        res = compare_candidates(cands, ref, w.snr_threshold)
+        assert res["only_gpu"] == 0 and res["only_oracle"] == 0, (seed, it, res)
+        ran += 1
+    assert ran >= 25
