@@ -86,3 +86,70 @@ def test_random_shapes_match_the_oracle(B, seed):
         assert res["only_gpu"] == 0 and res["only_oracle"] == 0, (seed, it, res)
         ran += 1
     assert ran >= 25
+
+
+def _draw_fine(B, rng, it):
+    """Fine channels and fine DM steps: the delay tables the shared-pattern dedispersion kernels are built for."""
+    bins = rng.choice([(1,), (1,), (2,), (4,), (1, 2, 4), (16,), (32,), (8, 16)])
+    nchans = rng.choice([256, 302, 600, 1024, 1029, 2048, 4096])
+    f_top = rng.choice([1500.0, 1550.0, 800.0])
+    foff = -rng.choice([100.0, 300.0, 200.0]) / nchans
+    ndms = rng.choice([33, 64, 70, 128, 200])
+    dm_step = rng.choice([0.1, 0.25, 0.5, 1.0])
+    nb = max(rng.choice([1024, 4096, 16384]), 128 * max(bins))
+    n_streams = rng.choice([1, 2])
+    chunk = nb * rng.choice([1, 2, 4]) * n_streams
+    variant = rng.choice(["auto", "auto", "ws1024", "ws512", "sp1024", "plain"])
+    peaks = rng.choice([False, False, True])
+    ranges, lo = [], rng.choice([0.0, 50.0, 300.0])
+    for b in bins:
+        ranges.append(I.DMRange(lo, dm_step, ndms, b))
+        lo += dm_step * ndms
+    w = I.Workload(name=f"fine{it}", nchans=nchans, nsamp=10 * chunk + 10 ** 6, tsamp=64e-6, f_top=f_top, foff=foff,
+                   ranges=tuple(ranges), widths=(1, 2, 4, 8, 16), snr_threshold=5.0, n_streams=n_streams, chunk_len=chunk,
+                   noise_seed=3000 + it, pulses=(), norm_block=nb)
+    try:
+        g = B.plan_geometry(w)
+    except RuntimeError:
+        return None
+    if g["halo"] > chunk // n_streams:                 # sub-chunks must hold the DM sweep
+        chunk = -(-g["halo"] // (nb * n_streams)) * nb * n_streams
+    nsamp = chunk + g["maxshift"] + rng.randint(2000, max(chunk, 4000))
+    if nsamp * nchans > 3e8:                           # keep the oracle to seconds
+        nsamp = max(chunk // n_streams + g["maxshift"] + 1000, int(3e8 // nchans))
+    w = I.scaled(w, nsamp=nsamp, chunk_len=chunk, pulses=(I.Pulse(dm=lo * 0.5, t0=nsamp // 4, width=4, amp=2.0),))
+    return w, variant, peaks
+
+
+@pytest.mark.parametrize("seed", [11, 12])
+def test_random_fine_channel_shapes_match_the_oracle(B, seed):
+    rng = random.Random(seed)
+    ran = shared_pattern = 0
+    for it in range(30):
+        drawn = _draw_fine(B, rng, it)
+        if drawn is None:
+            continue
+        w, variant, peaks = drawn
+        buf = B.pinned_empty(w.nbytes)
+        x = buf.numpy().reshape(w.nsamp, w.row_bytes)
+        I.fill(w, x)
+        try:
+            plan = B.Plan(w, taps=list(range(w.ndms_total)), dedisp_variant=variant, peaks=peaks, max_cands_per_subchunk=1 << 22)
+        except RuntimeError:
+            continue
+        with plan:
+            shared_pattern += any(plan.dedisp_variant(r) in (1, 2, 3, 4, 5) for r in range(len(w.ranges)))
+            cands, tap = plan.run(buf, max_cands=1 << 24)
+            assert not plan.overflow, (seed, it)
+        ref, dense, geo = oracle.run(x, w, keep_dense=True)
+        base = 0
+        for r, rg in enumerate(w.ranges):
+            assert np.array_equal(tap[base:base + rg.ndms, :geo["nout"][r]], dense[r]), (seed, it, r, variant)
+            base += rg.ndms
+        if peaks:
+            assert cands.tobytes() == oracle.find_peaks_fast(ref).tobytes(), (seed, it)
+        else:
+            res = compare_candidates(cands, ref, w.snr_threshold)
+            assert res["only_gpu"] == 0 and res["only_oracle"] == 0, (seed, it, res)
+        ran += 1
+    assert ran >= 20 and shared_pattern >= 8
