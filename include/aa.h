@@ -35,8 +35,9 @@ typedef enum {
     AA_ERR_NOT_PINNED = -2,  /* aa_run input is pageable host memory (never staged silently) */
     AA_ERR_OOM = -3,         /* device or pinned allocation failed */
     AA_ERR_CUDA = -4,        /* a CUDA call failed; see aa_last_cuda_error() */
-    AA_ERR_OVERFLOW = -5     /* more candidates than the output / per-sub-chunk buffers hold;
+    AA_ERR_OVERFLOW = -5,    /* more candidates than the output / per-sub-chunk buffers hold;
                                 the run is otherwise valid and *n_cands is the true total */
+    AA_ERR_LIMIT = -6        /* request larger than the fixed capacity of aa_find_peaks_device_noalloc */
 } aa_status;
 
 typedef enum {
@@ -286,6 +287,41 @@ int aa_get_timeline(const aa_plan *p, aa_subchunk_times *out, uint64_t max, uint
  * Pure host code: needs no plan and no GPU. */
 int aa_find_peaks(const aa_candidate *cands, uint64_t n, aa_candidate *out, uint64_t max_out, uint64_t *n_out,
                   int32_t nthreads);
+
+/*
+ * Peak finding (the rule of aa_find_peaks, reading A17) on a candidate list that is already in DEVICE memory, for
+ * callers that may not allocate device memory while they run: a real-time ingest loop in its streamed phase (one
+ * cudaMalloc / cudaFree waits for the whole device and stalls every other stream's copies and kernels
+ * and :71 allocate everything beforehand for that reason), or a process whose device memory all belongs to one
+ * owner (a framework's caching pool, an arena carved at start-up) behind whose back a raw cudaMalloc would fail or
+ * fragment.  The call makes no cudaMalloc / cudaFree and calls no library routine that allocates: the bucket grid
+ * and chains the kernels need sit in a fixed array inside the library image.  That array costs 8 MiB of device
+ * memory on every GPU that loads libaa.so, from load until the process exits, whether or not this function is used.
+ *   cands   : device, n records in ANY order, at most one per (dm_index, t_start); records with dm_index >= ndms or
+ *             t_start >= t_end are ignored (neither peaks nor neighbours)
+ *   n       : <= AA_PEAKS_NOALLOC_MAX_CANDS, else AA_ERR_LIMIT
+ *   ndms    : number of DM rows, > 0; t_end: candidates start in [0, t_end) raw samples, > 0.  The grid has
+ *             ndms * ceil(t_end / 2^shift) cells, shift >= 5 chosen so that they fit AA_PEAKS_NOALLOC_MAX_CELLS;
+ *             AA_ERR_LIMIT if ndms alone exceeds it.  Coarser cells only cost time.
+ *   wmax    : no record's width exceeds it (raw samples); a longer boxcar may be missed as a neighbour
+ *   out     : device, room for max_out records; receives the peaks, UNORDERED (sort by (dm_index, t_start) to
+ *             compare with aa_find_peaks: the same set of records, bit for bit)
+ *   n_out   : device uint32; receives the number of peaks found, which may exceed max_out (only max_out are stored)
+ *   stream  : cudaStream_t of the current device (NULL = the default stream); everything is enqueued on it and the
+ *             call returns without waiting: read out / n_out after synchronising the stream
+ *   cuda_error : host, may be NULL; the cudaError_t when the call returns AA_ERR_CUDA, else 0
+ * First call on a device: it looks up the array's device address (cudaGetSymbolAddress, once per device, with
+ * the device that is current at the call) and remembers it; make that first call during set-up, before any stream
+ * capture is begun.  Sharing: every call on a device uses the same array, which keeps the previous call's contents;
+ * each call empties the cells it will use on `stream` before its kernels, so calls that follow one another on one
+ * stream are independent, but two calls that can be on the GPU at the same time (two streams with no event
+ * between them, two host threads) race on the array and give wrong peaks: order them.  Errors: AA_ERR_INVALID
+ * (NULL pointers, ndms or t_end 0), AA_ERR_LIMIT (sizes above), AA_ERR_CUDA.
+ */
+#define AA_PEAKS_NOALLOC_MAX_CANDS (1u << 20)   /* records per call */
+#define AA_PEAKS_NOALLOC_MAX_CELLS (1u << 20)   /* bucket cells per call */
+int aa_find_peaks_device_noalloc(const aa_candidate *cands, uint32_t n, uint32_t ndms, uint32_t t_end, uint32_t wmax,
+                                 aa_candidate *out, uint32_t max_out, uint32_t *n_out, void *stream, int *cuda_error);
 
 /* NULL-safe.  Frees everything the plan allocated (not a caller-owned arena or streams). */
 void aa_destroy(aa_plan *p);

@@ -16,6 +16,9 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "libaa.so")
 
 AA_OK, AA_ERR_INVALID, AA_ERR_NOT_PINNED, AA_ERR_OOM, AA_ERR_CUDA, AA_ERR_OVERFLOW = 0, -1, -2, -3, -4, -5
+AA_ERR_LIMIT = -6
+#: fixed capacity of aa_find_peaks_device_noalloc (aa.h)
+PEAKS_NOALLOC_MAX_CANDS, PEAKS_NOALLOC_MAX_CELLS = 1 << 20, 1 << 20
 #: aa_dedisp_choice (aa_plan_desc.dedisp_variant)
 DEDISP_CHOICE = {"auto": 0, "plain": 1, "sp512": 2, "sp1024": 3, "ws512": 4, "ws1024": 5, "g8": 6}
 
@@ -24,7 +27,7 @@ CAND_DTYPE = np.dtype([("dm_index", np.uint32), ("t_start", np.uint32),
 
 EXPORTS = ["aa_plan_arena_bytes", "aa_plan_create", "aa_plan_query", "aa_plan_nout", "aa_plan_delays",
            "aa_plan_dedisp_variant",
-           "aa_plan_geometry", "aa_run", "aa_run_staged", "aa_run_resident", "aa_get_stats", "aa_get_timeline", "aa_find_peaks", "aa_destroy", "aa_host_alloc", "aa_host_free",
+           "aa_plan_geometry", "aa_run", "aa_run_staged", "aa_run_resident", "aa_get_stats", "aa_get_timeline", "aa_find_peaks", "aa_find_peaks_device_noalloc", "aa_destroy", "aa_host_alloc", "aa_host_free",
            "aa_strerror", "aa_last_cuda_error",
            "aa_plan_dedisp_model", "aa_microbench_count", "aa_microbench_name", "aa_microbench", "aa_microbench_link"]
 
@@ -125,6 +128,9 @@ def load_library() -> ctypes.CDLL:
     lib.aa_plan_dedisp_model.argtypes = [ctypes.POINTER(PlanDescC), i32, i32, ctypes.POINTER(DedispModelC)]
     lib.aa_find_peaks.restype = ctypes.c_int
     lib.aa_find_peaks.argtypes = [vp, u64, vp, u64, ctypes.POINTER(u64), ctypes.c_int32]
+    lib.aa_find_peaks_device_noalloc.restype = ctypes.c_int
+    lib.aa_find_peaks_device_noalloc.argtypes = [vp, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32, ctypes.c_uint32,
+                                                 vp, ctypes.c_uint32, vp, vp, ctypes.POINTER(ctypes.c_int)]
     lib.aa_get_timeline.restype = ctypes.c_int
     lib.aa_get_timeline.argtypes = [vp, ctypes.POINTER(SubchunkTimesC), u64, ctypes.POINTER(u64)]
     lib.aa_host_alloc.restype = ctypes.c_int
@@ -171,6 +177,29 @@ def find_peaks(cands: np.ndarray, nthreads: int = 0) -> np.ndarray:
     n = ctypes.c_uint64(0)
     _check(lib, lib.aa_find_peaks(cands.ctypes.data, len(cands), out.ctypes.data, len(out), ctypes.byref(n), int(nthreads)))
     return out[:int(n.value)]
+
+
+def find_peaks_device_noalloc(cands_dev, ndms: int, t_end: int, wmax: int, out_dev, n_out_dev, stream=None,
+                              n: Optional[int] = None) -> None:
+    """aa_find_peaks_device_noalloc: peak finding on a device-resident candidate list without any device allocation,
+    for callers that must not allocate while they run (a streamed real-time loop that one cudaMalloc would stall, a
+    process whose device memory all belongs to a caching pool).  The caller brings everything: `cands_dev` (torch
+    uint8/any tensor holding n 16-byte records), `out_dev` (room for the peaks, unordered) and `n_out_dev` (one
+    uint32); the scratch is a fixed 8 MiB array inside libaa.so (limits: PEAKS_NOALLOC_MAX_*; AAError(AA_ERR_LIMIT)
+    beyond).  Asynchronous on `stream` (a torch stream, default: the current one); calls that could overlap on the
+    GPU share that scratch and must be ordered by the caller."""
+    import torch
+    lib = load_library()
+    if n is None:
+        n = cands_dev.numel() * cands_dev.element_size() // CAND_DTYPE.itemsize
+    max_out = out_dev.numel() * out_dev.element_size() // CAND_DTYPE.itemsize
+    st = stream if stream is not None else torch.cuda.current_stream()
+    err = ctypes.c_int(0)
+    rc = lib.aa_find_peaks_device_noalloc(cands_dev.data_ptr() if n else None, int(n), int(ndms), int(t_end), int(wmax),
+                                          out_dev.data_ptr() if max_out else None, int(max_out), n_out_dev.data_ptr(),
+                                          st.cuda_stream, ctypes.byref(err))
+    if rc != AA_OK:
+        raise AAError(rc, lib.aa_strerror(rc).decode() + (f" (cudaError {err.value})" if rc == AA_ERR_CUDA else ""))
 
 
 def microbench(ctas_per_sm: int = 2, trips: int = 2000, link_bytes: int = 1 << 30) -> dict:

@@ -1406,6 +1406,7 @@ const char *aa_strerror(int s)
         case AA_ERR_OOM: return "out of device or pinned memory";
         case AA_ERR_CUDA: return "CUDA call failed (see aa_last_cuda_error)";
         case AA_ERR_OVERFLOW: return "candidate buffer overflow (list truncated)";
+        case AA_ERR_LIMIT: return "request exceeds the fixed capacity of the no-allocation entry point (AA_PEAKS_NOALLOC_MAX_*)";
         default: return "unknown status";
     }
 }
