@@ -329,8 +329,15 @@ class Plan:
             _check(self.lib, v)
         return v
 
-    def _run(self, fn, ptr: int, max_cands: int, want_taps: bool, tap_out=None):
-        out = np.empty(int(max_cands), dtype=CAND_DTYPE)
+    def _run(self, fn, ptr: int, max_cands: int, want_taps: bool, tap_out=None, out=None):
+        # `out`: the caller's candidate array (CAND_DTYPE, C-contiguous), reused across calls; the returned list is then
+        # a view of it.  Without it every call makes a fresh np.empty(max_cands): up to 268 MB of new virtual memory
+        # whose first touch (page faults) lands inside aa_run's host stage -- fine for tests, not for a timed loop.
+        if out is not None:
+            assert out.dtype == CAND_DTYPE and out.flags.c_contiguous and out.ndim == 1
+            max_cands = len(out)
+        else:
+            out = np.empty(int(max_cands), dtype=CAND_DTYPE)
         n = ctypes.c_uint64(0)
         tap = None
         if tap_out is not None:                      # caller's buffer (e.g. a 68 GB dense plane, touched once)
@@ -346,19 +353,19 @@ class Plan:
         self.n_found = int(n.value)
         return out[:int(self.stats()["n_stored"])], tap
 
-    def run(self, host_input, max_cands: int = 1 << 22, want_taps: bool = True, tap_out=None):
+    def run(self, host_input, max_cands: int = 1 << 22, want_taps: bool = True, tap_out=None, out=None):
         """aa_run on a pinned host buffer (torch pinned tensor or its numpy view)."""
         ptr = host_input.data_ptr() if hasattr(host_input, "data_ptr") else host_input.ctypes.data
-        return self._run(self.lib.aa_run, ptr, max_cands, want_taps, tap_out)
+        return self._run(self.lib.aa_run, ptr, max_cands, want_taps, tap_out, out)
 
-    def run_staged(self, host_input, max_cands: int = 1 << 22, want_taps: bool = True):
+    def run_staged(self, host_input, max_cands: int = 1 << 22, want_taps: bool = True, tap_out=None, out=None):
         """aa_run_staged on an ordinary (pageable) numpy uint8 array; needs Plan(stage_input=True)."""
         ptr = host_input.data_ptr() if hasattr(host_input, "data_ptr") else host_input.ctypes.data
-        return self._run(self.lib.aa_run_staged, ptr, max_cands, want_taps)
+        return self._run(self.lib.aa_run_staged, ptr, max_cands, want_taps, tap_out, out)
 
-    def run_resident(self, device_input, max_cands: int = 1 << 22, want_taps: bool = True):
+    def run_resident(self, device_input, max_cands: int = 1 << 22, want_taps: bool = True, out=None):
         """aa_run_resident on a torch CUDA uint8 tensor holding the whole observation."""
-        return self._run(self.lib.aa_run_resident, device_input.data_ptr(), max_cands, want_taps)
+        return self._run(self.lib.aa_run_resident, device_input.data_ptr(), max_cands, want_taps, None, out)
 
     def stats(self) -> dict:
         s = StatsC()

@@ -144,6 +144,18 @@ def test_rank_placement_splits_the_cores_of_a_numa_node():
     two = [D.rank_cpus(r, 2, None, list(range(16))) for r in range(2)]
     assert sorted(two[0] + two[1]) == list(range(16))
     assert D._parse_cpulist("0-3,8,10-11\n") == [0, 1, 2, 3, 8, 10, 11]
-    info = D.place_rank(0, 1)                 # best effort on whatever host runs the tests; never raises
-    assert "cpus" in info
+    # best effort on whatever host runs the tests; never raises.  It narrows the process affinity and may set
+    # OMP_NUM_THREADS: put both back so that no later test runs on fewer cores
+    import os
+    aff, omp = os.sched_getaffinity(0), os.environ.get("OMP_NUM_THREADS")
+    try:
+        info = D.place_rank(0, 1)
+        assert "cpus" in info
+    finally:
+        os.sched_setaffinity(0, aff)
+        if omp is None:
+            os.environ.pop("OMP_NUM_THREADS", None)
+        else:
+            os.environ["OMP_NUM_THREADS"] = omp
+    assert os.sched_getaffinity(0) == aff and os.environ.get("OMP_NUM_THREADS") == omp
 
