@@ -445,8 +445,7 @@ def main():
     plan = B.Plan(w, n_streams=1, chunk_len=L)
     variant = plan.dedisp_variant(0)
     kernel_name = {0: "dedisp_kernel", 1: "dedisp_sp_kernel<512>", 2: "dedisp_sp_kernel<1024>",
-                   3: "dedisp_ws_kernel<512>", 4: "dedisp_ws_kernel<1024>", 5: "dedisp_ws_kernel<512, wide>",
-                   6: "dedisp_g8_kernel"}.get(variant, "dedisp")
+                   3: "dedisp_ws_kernel<512>", 4: "dedisp_ws_kernel<1024>", 5: "dedisp_ws_kernel<512, wide>"}.get(variant, "dedisp")
 
     def step_res():
         c, _ = plan.run_resident(dev_in, want_taps=False, out=obuf)

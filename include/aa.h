@@ -46,8 +46,7 @@ typedef enum {
     AA_DEDISP_SP512 = 2,     /* shared-pattern kernel, 512-sample tiles */
     AA_DEDISP_SP1024 = 3,    /* ... 1024-sample tiles */
     AA_DEDISP_WS512 = 4,     /* warp-specialised shared-pattern kernel, 512-sample tiles */
-    AA_DEDISP_WS1024 = 5,    /* ... 1024-sample tiles */
-    AA_DEDISP_G8 = 6         /* 8-channel shared-pattern kernel (uint8 input only): measured slower, never chosen by AUTO */
+    AA_DEDISP_WS1024 = 5     /* ... 1024-sample tiles */
 } aa_dedisp_choice;
 
 /* One DM range of the plan: DM_i = dm_low + i*dm_step (double), i = 0..ndms-1, searched on
@@ -79,7 +78,8 @@ typedef struct {
     const aa_dm_range *ranges;
     int32_t  nwidths;
     const int32_t *widths;     /* boxcar widths in BINNED samples of each range, ascending, >= 1 */
-    double   snr_threshold;
+    double   snr_threshold;    /* double, not the float of SURVEY.md 8(b): the threshold test S >= threshold is taken in double on
+                                  both sides (deviations) */
     /* streaming: each time chunk of chunk_len raw samples is split into n_streams
      * sub-chunks; chunk_len/n_streams must be a multiple of norm_block and at least the halo
      * (DM sweep + longest boxcar) reported by aa_plan_query. */
@@ -102,7 +102,7 @@ typedef struct {
     /* 1: every stream also gets a small pinned input staging buffer ((subchunk_len + halo) * nchans
      * bytes) so that aa_run_staged can take an observation held in pageable memory */
     int32_t  stage_input;
-    /* Debug / A-B timing knob (an aa_dedisp_choice): AA_DEDISP_AUTO (0) lets the plan pick the dedispersion kernel of
+    /* TEST HOOK, not part of the search: leave 0.  (An aa_dedisp_choice.)  AA_DEDISP_AUTO (0) lets the plan pick the dedispersion kernel of
      * every range from its delay table.  Any other value restricts the choice to that one kernel family; a range the
      * forced kernel cannot serve (tables do not fit) runs on the plain kernel.  Unknown values: AA_ERR_INVALID.  All
      * kernels compute the same exact sums; tests force each one against the oracle. */
@@ -130,7 +130,7 @@ typedef struct {
      * settled by the host on the merged list; the result is exactly aa_find_peaks of the full list.  *n_cands and
      * aa_stats.n_peaks then count peaks, aa_stats.n_candidates still counts the candidates found on the device. */
     int32_t  output_mode;
-    /* Debug / A-B timing knob for the single-pulse-search kernel: 0 = the plan's choice; 1 = keep the first cluster
+    /* TEST HOOK, not part of the search: leave 0.  Single-pulse-search kernel: 0 = the plan's choice; 1 = keep the first cluster
      * kernel (sps_cluster_kernel: four passes over the segment for the statistics) where the second
      * (sps_cluster2_kernel: one pass + the listed outliers) would serve.  Same results.  Other values: AA_ERR_INVALID. */
     int32_t  sps_variant;
@@ -193,28 +193,6 @@ uint64_t aa_plan_arena_bytes(const aa_plan_desc *d);
  * creating it: no CUDA call, usable on a host without a GPU (e.g. to split an observation over ranks). */
 int aa_plan_geometry(const aa_plan_desc *d, aa_plan_info *out);
 
-/* Host-side cost model of the shared-pattern dedispersion kernels for range `range` of the plan `d` would build, from
- * its real delay table (no CUDA call): shared-memory wavefronts (128 bytes) per CTA = per (64 trials x tile_samples)
- * output tile, as the kernel issues them, the number of distinct delay patterns per stage, and the shared-memory
- * room the pattern rows take.  group_channels 4 = dedisp_ws_kernel (4 channels x 64 trials per stage), 8 =
- * dedisp_g8_kernel (8 channels x 32 trials per stage).  AA_ERR_INVALID if the range does not fit that kernel.
- * Backs profiles/r2_cost_model.md; the binding shared-memory roofline of bench.py uses wf_* of the kernel that runs. */
-typedef struct {
-    int32_t  group_channels, block_trials, tile_samples, stages_per_cta;
-    double   wf_consumer;          /* row-word loads of the consumer warps */
-    double   wf_producer_load;     /* channel-window loads of the producer warps */
-    double   wf_producer_store;    /* pattern-row stores (both alignments) */
-    double   wf_bulk;              /* bytes landed by cp.async.bulk / 128 */
-    double   patterns_mean;
-    int32_t  patterns_max;
-    int32_t  pad;
-    double   stage_bytes_mean;
-    uint64_t stage_bytes_max;
-    uint64_t ring_bytes;           /* shared memory left for the ring of pattern rows */
-    double   shared_offset_fraction; /* consecutive trials of a consumer warp that read the very same row words */
-} aa_dedisp_model;
-int aa_plan_dedisp_model(const aa_plan_desc *d, int32_t range, int32_t group_channels, aa_dedisp_model *out);
-
 /* Allocation phase (PAPER.md:19 part 2, :41 steps 1-2, :71): validates the descriptor, builds
  * the delay tables in double (north_star formula), creates streams and events, allocates the
  * device ring, per-stream work buffers, candidate lists and pinned staging.  Nothing is
@@ -230,13 +208,6 @@ uint64_t aa_plan_nout(const aa_plan *p, int32_t r);
  * memory `out`; used by tests to compare with the oracle entry by entry. */
 int aa_plan_delays(const aa_plan *p, int32_t r, int32_t *out);
 
-/* Which dedispersion kernel the plan chose for range r (the choice depends only on the delay table):
- * 0 = plain tiled kernel, 1 / 2 = shared-pattern kernel with 512 / 1024-sample tiles, 3 / 4 =
- * warp-specialised shared-pattern kernel with 512 / 1024-sample tiles, 5 = the same with 32-bit accumulators
- * (coarse time bins), 6 = 8-channel shared-pattern kernel; AA_ERR_INVALID if r is out
- * of range.  Used by tests to make sure every kernel is covered. */
-int aa_plan_dedisp_variant(const aa_plan *p, int32_t r);
-
 /*
  * The hot path: for every sub-chunk, on its stream:
  * async H2D of the new input rows -> corner turn into the device ring -> per range: (binning,)
@@ -251,6 +222,12 @@ int aa_plan_dedisp_variant(const aa_plan *p, int32_t r);
  *   tap_out    : host (pageable ok) uint32 [ntap][tap_row_len] or NULL; row k receives the
  *                dedispersed series of tap_dm_indices[k], nout_r values, rest untouched
  * No allocation, no pageable copy and no device-wide synchronisation happen inside.
+ *
+ * Precondition on the process, not checked here (the library reads no environment variable): the CUDA context must
+ * have at least n_streams hardware work queues, i.e. the CALLER sets CUDA_DEVICE_MAX_CONNECTIONS >= n_streams (default 8,
+ * maximum 32) in the environment BEFORE CUDA initialises.  With fewer, streams share a queue and one stream's small
+ * D2H copy waits behind another stream's kernels (a false dependency): results are identical, the overlap is not
+ * (measured: 16 streams on 8 queues lose about 5 %).  bench.py and the Python tools set 32.
  */
 int aa_run(aa_plan *p, const uint8_t *host_input, aa_candidate *out, uint64_t max_cands,
            uint64_t *n_cands, uint32_t *tap_out);
@@ -329,20 +306,6 @@ void aa_destroy(aa_plan *p);
 /* Pinned host allocation helpers (cudaHostAlloc / cudaFreeHost). */
 int  aa_host_alloc(void **p, uint64_t bytes);
 void aa_host_free(void *p);
-
-/* Micro-benchmarks of the units the hot path is bound by ("measure the real IADD3 / DP4A rates and
- * sustained clock first"); they back the roofline denominators of bench.py and DESIGN.md, they are not on the path.
- * aa_microbench runs kind 0 <= kind < aa_microbench_count() (aa_microbench_name: "iadd3", "lop3", "imad", "idp2a",
- * "idp4a", "prmt", "shf", "iadd3+imad", "lds32", "lds64", "lds128", "sts128", "lds32+iadd") as one wave of
- * ctas_per_sm (1..2) CTAs of 512 threads per SM, `trips` x 256 instructions per thread, and writes to host
- * pointers (each may be NULL): per_clk_sm = lane-operations per clock per SM for the arithmetic kinds (a full-warp
- * instruction counts 32), BYTES per clock per SM for the shared-memory kinds (conflict-free accesses), measured with
- * the SMs' own cycle counters; ms = kernel time (CUDA events); sm_mhz = the clock the run saw.
- * aa_microbench_link: pinned host <-> device copy of `bytes`, best of `reps`, in GB/s (dir 0 = H2D, 1 = D2H). */
-int aa_microbench_count(void);
-const char *aa_microbench_name(int kind);
-int aa_microbench(int kind, int ctas_per_sm, int trips, double *per_clk_sm, double *ms, double *sm_mhz);
-int aa_microbench_link(uint64_t bytes, int reps, int dir, double *gbs);
 
 const char *aa_strerror(int status);
 /* cudaError_t of the last failing CUDA call in this thread's last aa_* call (0 if none). */

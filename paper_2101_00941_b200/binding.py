@@ -20,7 +20,7 @@ AA_ERR_LIMIT = -6
 #: fixed capacity of aa_find_peaks_device_noalloc (aa.h)
 PEAKS_NOALLOC_MAX_CANDS, PEAKS_NOALLOC_MAX_CELLS = 1 << 20, 1 << 20
 #: aa_dedisp_choice (aa_plan_desc.dedisp_variant)
-DEDISP_CHOICE = {"auto": 0, "plain": 1, "sp512": 2, "sp1024": 3, "ws512": 4, "ws1024": 5, "g8": 6}
+DEDISP_CHOICE = {"auto": 0, "plain": 1, "sp512": 2, "sp1024": 3, "ws512": 4, "ws1024": 5}
 
 CAND_DTYPE = np.dtype([("dm_index", np.uint32), ("t_start", np.uint32),
                        ("width", np.uint32), ("snr", np.float32)])
@@ -323,7 +323,7 @@ class Plan:
 
     def dedisp_variant(self, r: int) -> int:
         """0 plain, 1/2 shared-pattern 512/1024, 3/4 warp-specialised shared-pattern 512/1024, 5 the latter with
-        32-bit accumulators (coarse time bins), 6 the 8-channel shared-pattern kernel."""
+        32-bit accumulators (coarse time bins)."""
         v = self.lib.aa_plan_dedisp_variant(self.handle, r)
         if v < 0:
             _check(self.lib, v)

@@ -52,18 +52,16 @@ struct Range {
     int sp_tb = 0;              // shared-pattern kernel: time tile (1024 or 512); 0 = plain kernel
     bool ws = false;            // warp-specialised variant of the shared-pattern kernel
     bool ws_wide = false;       // ... with 32-bit accumulators and no intermediate flush (coarse time bins)
-    bool g8 = false;            // 8-channel shared-pattern kernel (uint8 input)
     std::vector<SpRecord> h_sp;
     std::vector<WsRecord> h_ws;
-    G8Tables g8t;
     void *d_sp = nullptr;
     size_t sp_table_bytes() const
     {
-        return g8 ? g8t.recs.size() * sizeof(G8Record) : ws ? h_ws.size() * sizeof(WsRecord) : h_sp.size() * sizeof(SpRecord);
+        return ws ? h_ws.size() * sizeof(WsRecord) : h_sp.size() * sizeof(SpRecord);
     }
     const void *sp_table() const
     {
-        return g8 ? (const void *)g8t.recs.data() : ws ? (const void *)h_ws.data() : (const void *)h_sp.data();
+        return ws ? (const void *)h_ws.data() : (const void *)h_sp.data();
     }
     int32_t sp_rows = 0, sp_pbytes = 0, sp_flush = 1;
     std::vector<std::pair<int, int>> taps;   // (local dm, tap row)
@@ -192,7 +190,7 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         return AA_ERR_INVALID;
     if (d->n_streams < 1 || d->n_streams > 64 || d->chunk_len < 1) return AA_ERR_INVALID;
     if (d->ntap < 0 || (d->ntap > 0 && !d->tap_dm_indices)) return AA_ERR_INVALID;
-    if (d->dedisp_variant < AA_DEDISP_AUTO || d->dedisp_variant > AA_DEDISP_G8) return AA_ERR_INVALID;
+    if (d->dedisp_variant < AA_DEDISP_AUTO || d->dedisp_variant > AA_DEDISP_WS1024) return AA_ERR_INVALID;
     if (d->nsamp > 0xFFFFFFFFull) return AA_ERR_INVALID;       // candidates carry 32-bit sample indices
 
     p.desc = *d;
@@ -373,22 +371,9 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         // the choice to one kernel family (A/B timing, tests).
         R.sp_tb = 0;
         R.ws = false;
-        R.g8 = false;
         {
             const int force = d->dedisp_variant;
             auto allowed = [&](int v) { return force == AA_DEDISP_AUTO || force == v; };
-            // The 8-channel kernel halves the row words the consumers load, but its producers rebuild the rows for each
-            // half of the trial block and run out of issue slots: 58.7 ms against 26.6 ms per cfg3 launch
-            // (profiles/r2_dedisp_g8_ncu.txt).  It is bit-exact and stays selectable (A/B evidence), never automatic.
-            if (!R.in16 && force == AA_DEDISP_G8 &&
-                g8_build_tables(R.h_delays.data(), R.r.ndms, d->nchans, 226 * 1024, R.g8t)) {
-                R.g8 = true;
-                R.sp_tb = kG8TB;
-                R.sp_rows = R.g8t.rows;
-                R.sp_pbytes = R.g8t.ring_bytes;
-            } else {
-                R.g8t = G8Tables{};
-            }
             // 16-bit lanes take floor(65535 / (255 bin 4)) groups between flushes into the TMEM tile.  Only with fewer
             // than 4 (bin 32) the 32-bit-accumulator variant (512-sample tiles, no flush) is the faster one.  Measured
             // on cfg4, seconds per step: wide for bin >= 4: 2.17, >= 16: 2.08, 32 only: 2.07, never: 2.08 (with the
@@ -424,7 +409,7 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
                     R.sp_tb = tb;
             }
             if (!R.sp_tb || R.ws) { R.h_sp.clear(); R.h_sp.shrink_to_fit(); }
-            if (R.sp_tb) R.sp_flush = std::max(1, 65535 / (255 * R.r.bin * (R.g8 ? kG8 : kSpG)));
+            if (R.sp_tb) R.sp_flush = std::max(1, 65535 / (255 * R.r.bin * kSpG));
             if (!R.ws) R.ws_wide = false;
         }
         if (!R.in16) max_row_u8 = std::max(max_row_u8, std::max(R.row, R.sp_tb ? R.sp_rows + R.sp_tb : 0));
@@ -460,7 +445,7 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
     // arena layout (256-byte aligned bump allocation, computed identically in carve())
     uint64_t off = 0;
     auto take = [&](uint64_t bytes) { off = round_up(off, 256) + bytes; };
-    p.ring_plane_bytes = round_up(round_up((uint64_t)d->nchans, kG8) * p.ring_pitch, 256);
+    p.ring_plane_bytes = round_up(round_up((uint64_t)d->nchans, kRingChPad) * p.ring_pitch, 256);
     take(p.ring_plane_bytes * (uint64_t)p.planes);              // zero rows pad the channels to a multiple of 8
     for (auto &R : p.ranges) {
         take((uint64_t)R.r.ndms * d->nchans * 4);
@@ -741,8 +726,7 @@ void worker(aa_plan *p, int s, const uint8_t *input, Input mode, aa_candidate *o
                     da.sp_rows = Rg.sp_rows;
                     da.sp_pbytes = Rg.sp_pbytes;
                     da.sp_flush = Rg.sp_flush;
-                    if (Rg.g8) AA_W(launch_dedisp_g8(da, st));
-                    else if (Rg.ws) AA_W(launch_dedisp_ws(da, Rg.sp_tb, Rg.in16, Rg.ws_wide, st));
+                    if (Rg.ws) AA_W(launch_dedisp_ws(da, Rg.sp_tb, Rg.in16, Rg.ws_wide, st));
                     else if (Rg.sp_tb) AA_W(launch_dedisp_sp(da, Rg.sp_tb, st));
                     else AA_W(launch_dedisp(da, Rg.in16, Rg.dpw, st));
                     S.dedisp_launches++;
@@ -1191,7 +1175,6 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
     if ((e = dedisp_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
     if ((e = dedisp_sp_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
     if ((e = dedisp_ws_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
-    if ((e = dedisp_g8_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
     if ((e = sps_configure()) != cudaSuccess) return fail(AA_ERR_CUDA, e);
 
     if (d->device_arena) {
@@ -1220,7 +1203,7 @@ int aa_plan_create(aa_plan **out, const aa_plan_desc *d)
     }
     carve(*p);
     {
-        const uint64_t ring_pad = round_up((uint64_t)d->nchans, kG8) - (uint64_t)d->nchans;
+        const uint64_t ring_pad = round_up((uint64_t)d->nchans, kRingChPad) - (uint64_t)d->nchans;
         const uint64_t pad_rows = round_up((uint64_t)d->nchans, kSpG) - (uint64_t)d->nchans;
         for (int pl = 0; ring_pad && pl < p->planes; ++pl)
             if ((e = cudaMemset(p->d_ring + (uint64_t)pl * p->ring_plane_bytes + (uint64_t)d->nchans * p->ring_pitch, 0,
@@ -1306,8 +1289,12 @@ int aa_plan_dedisp_model(const aa_plan_desc *d, int32_t range, int32_t group_cha
     if (rc != AA_OK) return rc;
     if (range < 0 || range >= (int32_t)tmp.ranges.size()) return AA_ERR_INVALID;
     const Range &R = tmp.ranges[range];
-    const int tb = group_channels == 8 ? kG8TB : (R.ws && !R.g8 ? R.sp_tb : 1024);
-    return dedisp_model(R.h_delays.data(), R.r.ndms, d->nchans, R.in16 ? 2 : 1, group_channels, tb, out);
+    // only ranges the warp-specialised family can serve: binned input adds four channels in 16-bit lanes, 4 * 255 * bin
+    // must stay below 2^16 (coarser bins run on the plain kernel, a model of the ws kernel there would describe nothing)
+    if (group_channels != 4 || (R.in16 && 4ull * 255 * R.r.bin > 65535)) return AA_ERR_INVALID;
+    const bool wide = R.in16 && 65535 / (255 * R.r.bin * kSpG) < 4;      // the plan's rule for the 32-bit-accumulator variant
+    const int tb = R.ws ? R.sp_tb : (wide ? 512 : 1024);
+    return dedisp_model(R.h_delays.data(), R.r.ndms, d->nchans, R.in16 ? 2 : 1, group_channels, tb, wide, out);
 }
 
 int aa_plan_query(const aa_plan *p, aa_plan_info *o)
@@ -1345,7 +1332,6 @@ int aa_plan_dedisp_variant(const aa_plan *p, int32_t r)
     if (!p || r < 0 || r >= (int32_t)p->ranges.size()) return AA_ERR_INVALID;
     const Range &R = p->ranges[r];
     if (!R.sp_tb) return 0;
-    if (R.g8) return 6;
     if (R.ws_wide) return 5;
     return (R.ws ? 3 : 1) + (R.sp_tb == 1024 ? 1 : 0);
 }

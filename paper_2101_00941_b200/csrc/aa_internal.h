@@ -6,6 +6,7 @@
 #include <vector>
 
 #include "../../include/aa.h"
+#include "../../include/aa_bench.h"
 
 namespace aa {
 
@@ -102,56 +103,12 @@ cudaError_t dedisp_ws_configure();
 size_t dedisp_sp_smem_bytes(int rows, int pbytes);
 cudaError_t dedisp_sp_configure();
 
-// ---- 8-channel shared-pattern kernel (kernels_dedisp_g8.cu, g8_tables.cu): uint8 input only ----------------------
-// A CTA still covers kSpDB = 64 trials x kG8TB samples, but pattern rows are built per HALF of 32 trials and per
-// group of 8 channels: one stage = (group, half); stage s = 2 * group + half.  Consumer warps 0-7 own the trials of
-// half 0 and consume the even stages, warps 8-15 the odd ones.
-constexpr int kG8 = 8;              // channels per group
-constexpr int kG8Half = 32;         // trials per stage
-constexpr int kG8TB = 1024;         // samples per CTA tile
-constexpr int kG8MaxA = 8;          // distinct (rel_1..rel_3) per stage
-constexpr int kG8MaxB = 12;         // distinct (rel_4..rel_7) per stage
-constexpr int kG8Slots = 16;        // full[] / empty[] barrier slots (stage modulo kG8Slots)
-constexpr int kG8Window = 8;        // a stage is never built before stage s - kG8Window has been consumed (even)
-constexpr int kG8Producers = 8;     // producer warps; the batches of all stages are dealt round them
-constexpr int kG8Ahead = 2;         // channel windows are requested this many groups ahead (kG8Ahead + 1 slots)
-struct G8Window {                   // staged channel windows of one (DM block, group): shared by both halves
-    int32_t rbase[kG8];             // first staged sample of each channel row relative to col0 + t0 (multiple of 16)
-    uint16_t rbytes[kG8];           // staged bytes of each channel row (multiple of 16)
-};
-struct G8Record {
-    int32_t nrbase[kG8];            // window descriptor carried by this record (see g8_tables.cu): even stages their own
-    uint16_t nrbytes[kG8];          // group's, odd stages the one kG8Ahead groups ahead (rbytes 0: none)
-    // bits 0-15: i * rows + (m_i & ~7), the 8-byte-aligned load offset of chunk 0 inside the window slot;
-    // bits 16-20: 8 * (m_i & 3); bit 21: (m_i & 4) != 0, m_i = smallest shift of channel i over this stage's patterns
-    uint32_t chdesc[kG8];
-    uint8_t eA[3][kG8MaxA];         // 8 * extra shift of channel 1..3 in A pattern ka
-    uint8_t eB[4][kG8MaxB];         // 8 * extra shift of channel 4..7 in B pattern kb
-    uint8_t comb[kG8MaxB];          // bit ka: the pair (ka, kb) occurs
-    uint8_t nA, nB, npat, rows0;    // rows0: rows emitted by the first pass (A patterns 0..3)
-    uint16_t nchunk;                // 8-sample chunks per pattern row
-    uint16_t nbatch;                // warp-sized batches of 31 chunks per pattern row
-    uint32_t pofs;                  // byte offset of this stage's pattern rows inside the shared-memory ring
-    int32_t dep[2];                 // rows may be written once stage dep[0] (same half) and dep[1] (other half) are consumed
-    uint16_t bstart;                // batches of earlier stages modulo kG8Producers
-    uint16_t pad;
-    uint32_t pad2;
-    uint32_t poff[kG8Half];         // byte offset, inside the ring, of trial d's word (tau 0, tau 1)
-};
-static_assert(sizeof(G8Record) % 16 == 0, "records are fetched with 16-byte copies");
-struct G8Tables {
-    std::vector<G8Record> recs;     // [nblk][nstages]
-    std::vector<G8Window> wins;     // [nblk][ngroups]
-    int32_t nblk = 0, nstages = 0, rows = 0, ring_bytes = 0;
-};
-bool g8_build_tables(const int32_t *delays, int32_t ndms, int32_t nchans, size_t smem_budget, G8Tables &T);
-size_t dedisp_g8_fixed_smem_bytes(int rows);
-size_t dedisp_g8_smem_bytes(int rows, int ring_bytes);
-cudaError_t dedisp_g8_configure();
-cudaError_t launch_dedisp_g8(const DedispArgs &a, cudaStream_t st);
+// The channel rows of the device ring are padded with zero rows to a multiple of this many channels (a whole number of
+// kSpG groups; 8 since the rejected 8-channel kernel of round 2, kept so that the arena layout does not move).
+constexpr int kRingChPad = 8;
 
 // cost_model.cu: shared-memory wavefronts and room of one kernel family over a delay table (no GPU)
-int dedisp_model(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t elem_bytes, int family, int tb, aa_dedisp_model *o);
+int dedisp_model(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t elem_bytes, int family, int tb, bool wide, aa_dedisp_model *o);
 
 struct SpsArgs {
     const uint32_t *D;     // [ndms][pitch] dedispersed sub-chunk

@@ -3,7 +3,8 @@
 // shared-memory wavefronts the kernel issues as designed -- consumer row loads, producer window loads (6 per channel
 // and batch: two 8-byte loads of 2 wavefronts, one 4-byte load with a 2-way conflict), producer row stores (8 per
 // pattern row and batch: two 16-byte stores of 4 wavefronts), bulk-copy landings -- and the shared-memory room the
-// rows need.  It says nothing about issue slots, which is what sank the 8-channel variant (profiles/r2_dedisp_g8_ncu.txt).
+// rows need.  It says nothing about issue slots, which is what sank the 8-channel variant of round 2 (measured at
+// 58.7 ms against 26 ms per cfg3 launch, profiles/r2_dedisp_g8_ncu.txt; its source is no longer in the tree).
 #include <algorithm>
 #include <cmath>
 
@@ -36,8 +37,8 @@ void finish(const Acc &A, int nblk, aa_dedisp_model *o)
 
 }  // namespace
 
-// family 4: 4 channels x 64 trials (dedisp_ws_kernel); 8: 8 channels x 32 trials (dedisp_g8_kernel)
-int dedisp_model(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t elem_bytes, int family, int tb, aa_dedisp_model *o)
+// family 4: 4 channels x 64 trials (dedisp_ws_kernel), the only one
+int dedisp_model(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t elem_bytes, int family, int tb, bool wide, aa_dedisp_model *o)
 {
     *o = aa_dedisp_model{};
     o->group_channels = family;
@@ -52,7 +53,12 @@ int dedisp_model(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t el
         o->ring_bytes = (uint64_t)ring;
         for (auto &R : recs) {
             A.nstage++;
-            A.cons += (double)kSpDB * tb * 2 / 128.0;
+            // consumer row words: a warp owns 4 consecutive trials and loads one row word per trial and pair of samples,
+            // except that a trial whose word is the previous trial's (same pattern, same offset) reuses it
+            // (kernels_dedisp_ws.cu: "k == 0 || pof[k] != pof[k - 1]"); the 32-bit-accumulator variant loads every word
+            int loads = 0;
+            for (int d = 0; d < kSpDB; ++d) loads += wide || (d % 4 == 0) || R.poff[d] != R.poff[d - 1];
+            A.cons += (double)loads * tb * 2 / 128.0;
             A.pload += 6.0 * kSpG * R.nbatch;
             A.pstore += 8.0 * R.npat * R.nbatch;
             for (int i = 0; i < kSpG; ++i) A.bulk += R.rbytes[i] / 128.0;
@@ -64,26 +70,6 @@ int dedisp_model(const int32_t *delays, int32_t ndms, int32_t nchans, int32_t el
             for (int d = 0; d < kSpDB; ++d)
                 if (d % 4) { A.nshare += 1; A.share += R.poff[d] == R.poff[d - 1]; }
         }
-    } else if (family == 8) {
-        if (elem_bytes != 1 || tb != kG8TB) return AA_ERR_INVALID;
-        G8Tables T;
-        if (!g8_build_tables(delays, ndms, nchans, 226 * 1024, T)) return AA_ERR_INVALID;
-        o->block_trials = kG8Half;
-        o->ring_bytes = (uint64_t)T.ring_bytes;
-        for (auto &R : T.recs) {
-            A.nstage++;
-            const int passes = R.nA > 4 ? 2 : 1;
-            A.cons += (double)kG8Half * tb * 2 / 128.0;
-            A.pload += 6.0 * kG8 * R.nbatch * passes;
-            A.pstore += 8.0 * R.npat * R.nbatch;
-            const uint64_t b = (uint64_t)R.npat * 2 * R.nchunk * 16;
-            A.pat += R.npat; A.patmax = std::max<int>(A.patmax, R.npat);
-            A.bytes += (double)b; A.bytesmax = std::max(A.bytesmax, b);
-            for (int d = 0; d < kG8Half; ++d)
-                if (d % 4) { A.nshare += 1; A.share += R.poff[d] == R.poff[d - 1]; }
-        }
-        for (auto &W : T.wins)
-            for (int i = 0; i < kG8; ++i) A.bulk += W.rbytes[i] / 128.0;
     } else {
         return AA_ERR_INVALID;
     }

@@ -165,7 +165,7 @@ def test_first_cluster_kernel_still_matches(B, case):
     assert len(ref) > 0
 
 
-@pytest.mark.parametrize("variant,code", [("g8", 6), ("ws1024", 4), ("ws512", 3), ("sp1024", 2), ("sp512", 1), ("plain", 0), ("auto", None)])
+@pytest.mark.parametrize("variant,code", [("ws1024", 4), ("ws512", 3), ("sp1024", 2), ("sp512", 1), ("plain", 0), ("auto", None)])
 @pytest.mark.parametrize("case", [
     dict(nchans=302, ndms=100, nsamp=21000, chunk_len=8192),                 # padded channel group, partial DM block, ragged tile
     dict(nchans=1024, ndms=64, nsamp=9000, chunk_len=4096, foff=-0.2),      # four flushes of the 16-bit lanes
@@ -324,7 +324,7 @@ def test_saturated_binned_input(B):
 
 
 def test_saturated_input_every_kernel(B):
-    for variant in ("g8", "ws1024", "ws512", "sp1024", "plain"):
+    for variant in ("ws1024", "ws512", "sp1024", "plain"):
         w = _tiny(nchans=1024, ndms=70, nsamp=9000, chunk_len=4096, f_top=1500.0, foff=-0.2, dm_step=0.25, norm_block=1024)
         buf = B.pinned_empty(w.nbytes)
         buf.numpy()[:] = 255                         # 16-bit lanes at their limit before every flush

@@ -39,20 +39,35 @@ def test_report_modules_refuse_to_run_without_cuda():
 
 
 def test_dedispersion_cost_model_on_the_headline_workload():
-    """aa_plan_dedisp_model (no GPU): the consumer term is the definition (one 32-bit row word per trial, group and
-    sample pair), the pattern counts are those of the delay table, and the 8-channel variant halves the consumer term."""
+    """aa_plan_dedisp_model (aa_bench.h; no GPU): the consumer term is the definition (one 32-bit row word per trial, group
+    and sample pair) less the words a trial shares with the previous trial of its warp, which the kernel does not load
+    again; the pattern counts are those of the delay table; ranges the kernel family cannot serve are refused."""
     import numpy as np
     import oracle
     from paper_2101_00941_b200 import binding as B, inputs as I
     w = I.workload(3)
-    m4, m8 = B.dedisp_model(w, 0, 4), B.dedisp_model(w, 0, 8)
-    assert m4["stages_per_cta"] == w.nchans // 4 and m8["stages_per_cta"] == 2 * (w.nchans // 8)
-    assert m4["wf_consumer"] == 64 * 1024 * 2 / 128 * (w.nchans // 4)
-    assert m8["wf_consumer"] == m4["wf_consumer"] / 2
+    m4 = B.dedisp_model(w, 0, 4)
+    assert m4["stages_per_cta"] == w.nchans // 4
+    full = 64 * 1024 * 2 / 128 * (w.nchans // 4)
+    f = m4["shared_offset_fraction"]                             # of the 48 non-leading trials of a 64-trial block
+    assert m4["wf_consumer"] == pytest.approx(full * (64 - 48 * f) / 64, rel=1e-12) and 0.97 * full < m4["wf_consumer"] < full
     # distinct relative-delay vectors of one (64 trials, 4 channels) block, counted from the oracle's delay table
     dl = oracle.delays(w, 0)
     blk = dl[:64, 2000:2004] - dl[:64, 2000:2001]
     assert 1 <= len(np.unique(blk, axis=0)) <= m4["patterns_max"] <= 8
-    assert 4.0 < m4["patterns_mean"] < 5.5 and m8["patterns_mean"] > m4["patterns_mean"]
-    assert m4["stage_bytes_max"] <= m4["ring_bytes"] and 0.0 <= m4["shared_offset_fraction"] < 0.1
-    assert B.dedisp_model(I.workload(4), 1, 8) is None          # the 8-channel kernel takes uint8 input only
+    assert 4.0 < m4["patterns_mean"] < 5.5
+    assert m4["stage_bytes_max"] <= m4["ring_bytes"] and 0.0 <= f < 0.1
+    assert B.dedisp_model(w, 0, 8) is None                       # the 8-channel family is gone
+    # fine DM steps: many trials share their row words, and the model counts what the kernel then skips
+    w4 = I.workload(4)
+    m = B.dedisp_model(w4, 1, 4)
+    assert m is not None and m["shared_offset_fraction"] > 0.1
+    assert m["wf_consumer"] < 0.93 * 64 * m["tile_samples"] * 2 / 128 * m["stages_per_cta"]
+    # bin 32 runs the 32-bit-accumulator variant, which loads every word: no reduction there
+    m5 = B.dedisp_model(w4, 5, 4)
+    assert m5 is not None and m5["tile_samples"] == 512
+    assert m5["wf_consumer"] == pytest.approx(64 * 512 * 2 / 128 * m5["stages_per_cta"])
+    # binned input beyond 4 * 255 * bin < 2^16 runs on the plain kernel: no model of a kernel that never runs
+    import dataclasses
+    coarse = I.scaled(w4, ranges=(dataclasses.replace(w4.ranges[5], bin=128),), norm_block=65536, name="bin128")
+    assert B.plan_geometry(coarse)["ndms_total"] == w4.ranges[5].ndms and B.dedisp_model(coarse, 0, 4) is None
