@@ -242,7 +242,164 @@ def _timed(fn, plan_stats, steps, warmup, barrier, dist_util):
     return dist_util.max_over_ranks(max(wall, dev)), acc
 
 
-def run_config(B, k, steps, warmup, link_gbs, max_cands=1 << 24):
+def _host_avail_gb():
+    try:
+        with open("/proc/meminfo") as f:
+            for line in f:
+                if line.startswith("MemAvailable:"):
+                    return int(line.split()[1]) / 1e6
+    except OSError:
+        pass
+    return 0.0
+
+
+def _wall(fn):
+    """One call, host clock, device idle on both sides."""
+    import torch
+    torch.cuda.synchronize()
+    a = time.perf_counter()
+    r = fn()
+    torch.cuda.synchronize()
+    return time.perf_counter() - a, r
+
+
+def stream_sweep(B, w, host, obuf, streams, xfer_s, known=None):
+    """The stream-count sweep BASELINE.json asks for (configs[2]: 1/2/4/8, configs[4]: 1/2/4/8/16; Fig. 2):
+    the time chunk of the workload split into n sub-chunks, one per stream; aa_run from the pinned host buffer, one
+    warm-up and one timed call per stream count.  `known` = {n: entry} for a count the caller has already timed.
+    kernel_events_ms is the sum of the kernels' CUDA-event durations of the same run (the dedispersion CTA fills an
+    SM, so kernels of different streams do not run side by side and the sum is the time the GPU spent computing).
+    The sorted candidate list must hash identically for every stream count: streams change scheduling, not results."""
+    import hashlib
+    out = {}
+    for n in streams:
+        if known and n in known:
+            out[str(n)] = known[n]
+            continue
+        if w.chunk_len % n:
+            out[str(n)] = {"skipped": f"chunk_len {w.chunk_len} is not a multiple of {n}"}
+            continue
+        with B.Plan(w, n_streams=n, chunk_len=w.chunk_len) as plan:
+            def one():
+                c, _ = plan.run(host, want_taps=False, out=obuf)
+                return c
+            one()
+            dt, c = _wall(one)
+            st = plan.stats()
+            kern = (st["dedisp_ms"] + st["sps_ms"] + st["prep_ms"]) / 1e3
+            out[str(n)] = {"ms": 1e3 * dt, "subchunk_len": w.chunk_len // n, "kernel_events_ms": 1e3 * kern,
+                           "overlap_efficiency": max(kern, xfer_s) / dt, "h2d_gbs_in_run": st["h2d_bytes"] / dt / 1e9,
+                           "real_time_factor": w.nsamp * w.tsamp / dt, "candidates": int(len(c)),
+                           "candidates_sha256": hashlib.sha256(c.tobytes()).hexdigest()[:16]}
+    hashes = {v["candidates_sha256"] for v in out.values() if "candidates_sha256" in v}
+    if len(hashes) > 1:
+        raise SystemExit(f"stream sweep of {w.name}: candidate lists differ between stream counts: {out}")
+    out["transfer_alone_s"] = xfer_s
+    return out
+
+
+def paper_path(B, w, host, x, obuf, ref_hash):
+    """The paper's own data path, timed on the bench workload (one warm-up, one timed call each):
+    staged -- the observation in ordinary PAGEABLE memory, copied by one host thread per stream into small pinned
+              buffers and from there to the device (aa_run_staged; PAPER.md:57, :63);
+    dense  -- the whole dedispersed DM x time plane returned to pageable host memory through per-stream pinned staging
+              and the stream threads (all-rows tap).
+    Needs host RAM beside the pinned observation; records {"skipped": reason} when there is not enough."""
+    import hashlib
+    out = {}
+    need = w.nbytes / 1e9 * 1.1
+    if _host_avail_gb() < need:
+        out["staged"] = {"skipped": f"needs {need:.0f} GB of free host memory for the pageable copy"}
+    else:
+        pageable = np.array(x)
+        with B.Plan(w, stage_input=True) as plan:
+            def one():
+                c, _ = plan.run_staged(pageable, want_taps=False, out=obuf)
+                return c
+            one()
+            dt, c = _wall(one)
+            st = plan.stats()
+            h = hashlib.sha256(c.tobytes()).hexdigest()[:16]
+            if h != ref_hash:
+                raise SystemExit(f"aa_run_staged returned other candidates ({h}) than aa_run ({ref_hash})")
+            out["staged"] = {"ms": 1e3 * dt, "n_streams": w.n_streams, "h2h_bytes": st["h2h_bytes"],
+                             "h2h_gbs_per_thread": st["h2h_bytes"] / max(st["h2h_ms"], 1e-9) / 1e6,
+                             "real_time_factor": w.nsamp * w.tsamp / dt, "candidates_sha256": h}
+        del pageable
+    g = B.plan_geometry(w)
+    dense_gb = w.ndms_total * (g["t_valid"] // min(r.bin for r in w.ranges)) * 4 / 1e9
+    if _host_avail_gb() < dense_gb * 1.05:
+        out["dense"] = {"skipped": f"needs {dense_gb:.0f} GB of free host memory for the DM x time plane"}
+    else:
+        with B.Plan(w, taps=list(range(w.ndms_total))) as plan:
+            dense = np.zeros((w.ndms_total, plan.info["tap_row_len"]), dtype=np.uint32)
+
+            def one():
+                c, _ = plan.run(host, want_taps=False, tap_out=dense, out=obuf)
+                return c
+            one()                                   # also touches the plane's pages
+            dt, c = _wall(one)
+            st = plan.stats()
+            h = hashlib.sha256(c.tobytes()).hexdigest()[:16]
+            if h != ref_hash:
+                raise SystemExit(f"the dense run returned other candidates ({h}) than the plain run ({ref_hash})")
+            out["dense"] = {"ms": 1e3 * dt, "n_streams": w.n_streams, "d2h_bytes": st["d2h_bytes"],
+                            "d2h_gbs_in_run": st["d2h_bytes"] / dt / 1e9, "plane_checksum": int(dense[::97, ::4099].sum()),
+                            "real_time_factor": w.nsamp * w.tsamp / dt, "candidates_sha256": h}
+        del dense
+    return out
+
+
+def search_variants(B, w, host, obuf):
+    """The SURVEY 8(f) variants on the bench workload's own buffer (one warm-up, two timed calls each): per-width measured
+    sigma (A18), decimated long boxcars (A20)."""
+    out = {}
+    for name, ch in (("sigma_mode_1", dict(sigma_mode=1)), ("width_decimation_16", dict(wdec=16))):
+        wv = I.scaled(w, name=w.name + "_" + name, **ch)
+        try:
+            with B.Plan(wv) as plan:
+                def one():
+                    c, _ = plan.run(host, want_taps=False, out=obuf)
+                    return c
+                one()
+                ts = [_wall(one) for _ in range(2)]
+                st = plan.stats()
+                out[name] = {"ms": 1e3 * sum(t for t, _ in ts) / 2, "candidates": int(len(ts[-1][1])),
+                             "sps_ms": st["sps_ms"], "dedisp_ms": st["dedisp_ms"], "real_time_factor": w.nsamp * w.tsamp * 2 / sum(t for t, _ in ts)}
+        except Exception as e:
+            out[name] = {"error": f"{type(e).__name__}: {e}"}
+    return out
+
+
+def bit_depth_variants(B, w, obuf):
+    """4- and 16-bit input (A19) of the bench workload: own pinned buffer each (17 / 69 GB for cfg3), generated from the
+    same seeded stream; one warm-up, two timed calls.  Call with the 8-bit buffer already released."""
+    out = {}
+    for nbits in (4, 16):
+        wv = I.scaled(w, nbits=nbits, name=w.name + f"_{nbits}bit")
+        if _host_avail_gb() < wv.nbytes / 1e9 * 1.1:
+            out[f"nbits_{nbits}"] = {"skipped": f"needs {wv.nbytes / 1e9:.0f} GB of pinned host memory"}
+            continue
+        try:
+            hv = B.pinned_empty(wv.nbytes)
+            I.fill(wv, hv.numpy().reshape(wv.nsamp, wv.row_bytes))
+            with B.Plan(wv) as plan:
+                def one():
+                    c, _ = plan.run(hv, want_taps=False, out=obuf)
+                    return c
+                one()
+                ts = [_wall(one) for _ in range(2)]
+                st = plan.stats()
+                out[f"nbits_{nbits}"] = {"ms": 1e3 * sum(t for t, _ in ts) / 2, "candidates": int(len(ts[-1][1])),
+                                         "h2d_bytes": st["h2d_bytes"], "h2d_gbs_in_run": st["h2d_bytes"] * 2 / sum(t for t, _ in ts) / 1e9,
+                                         "dedisp_ms": st["dedisp_ms"], "sps_ms": st["sps_ms"]}
+            del hv
+        except Exception as e:
+            out[f"nbits_{nbits}"] = {"error": f"{type(e).__name__}: {e}"}
+    return out
+
+
+def run_config(B, k, steps, warmup, link_gbs, max_cands=1 << 24, sweep=()):
     """One more BASELINE.json config end to end through aa_run (pinned host buffer, the workload's stream count):
     the `per_config` entries of the bench line.  Own pinned buffer, released before returning."""
     import hashlib
@@ -298,6 +455,13 @@ def run_config(B, k, steps, warmup, link_gbs, max_cands=1 << 24):
     del dev_in
     kernels_s = (st_res["dedisp_ms"] + st_res["sps_ms"] + st_res["prep_ms"]) / 1e3
     c = last["c"]
+    if sweep:
+        kern_e2e = (st["dedisp_ms"] + st["sps_ms"] + st["prep_ms"]) / 1e3
+        known = {w.n_streams: {"ms": 1e3 * step_s, "subchunk_len": L, "kernel_events_ms": 1e3 * kern_e2e,
+                               "overlap_efficiency": max(kern_e2e, xfer_s) / step_s, "h2d_gbs_in_run": st["h2d_bytes"] / step_s / 1e9,
+                               "real_time_factor": w.nsamp * w.tsamp / step_s, "candidates": int(len(c)),
+                               "candidates_sha256": hashlib.sha256(c.tobytes()).hexdigest()[:16]}}
+        out["sweep"] = stream_sweep(B, w, host, obuf, sweep, xfer_s, known)
     if len(last["r"]) != len(c):
         raise RuntimeError(f"resident leg found {len(last['r'])} candidates, end-to-end leg {len(c)}")
     out.update({
@@ -333,6 +497,10 @@ def main():
     ap.add_argument("--per-config", default="auto",
                     help="comma-separated other configs to run end to end after the main workload (3 steps each) and "
                          "report under per_config; 'auto' = 1,2,4,5 for the default single-GPU run of workload 3, 'none' = skip")
+    ap.add_argument("--extras", default="auto", choices=["auto", "all", "none"],
+                    help="stream sweep 1/2/4/8, the paper's data path (aa_run_staged from pageable memory; dense DM x time "
+                         "output) and the search variants (A18, A20, 4/16-bit input) on the bench workload, reported under "
+                         "`sweep`, `paper_path`, `variants`; 'auto' = all for the default single-GPU run")
     ap.add_argument("--shard-observation", action="store_true",
                     help="strong scaling: ONE observation split by time over the ranks (whole normalisation blocks + halo "
                          "per rank, candidate lists gathered on rank 0); default: one observation per rank (weak)")
@@ -432,6 +600,9 @@ def main():
         tp0 = time.perf_counter()
         n_peaks = len(B.find_peaks(last["c"]))
         peak_info = {"n": n_peaks, "ms": 1e3 * (time.perf_counter() - tp0), "where": "host threads, after aa_run, not in the timed region"}
+    import hashlib
+    e2e_hash = hashlib.sha256(last["c"].tobytes()).hexdigest()[:16] if last.get("c") is not None else None
+    kern_e2e_s = sum(s_["dedisp_ms"] + s_["sps_ms"] + s_["prep_ms"] for s_ in st_e2e) / 1e3 / args.steps
     last.pop("c", None)
     plan.close()
 
@@ -560,7 +731,25 @@ def main():
             cb = cpu_baseline(w, x, budget_rows=args.ref_rows, budget_blocks=args.ref_blocks)
             cb.pop("seconds", None)
             line["cpu_baseline"] = cb
+    # ---- on the bench workload itself: the stream sweep BASELINE.json asks for, the paper's own data path, the variants ----
+    extras = args.extras
+    if extras == "auto":
+        extras = "all" if (world == 1 and not args.nsamp and not args.shard_observation and args.nbits == 8
+                           and args.streams in (0, w.n_streams)) else "none"
+    if rank == 0 and extras != "none":
+        step_s = t_e2e / args.steps
+        known = {n_streams: {"ms": 1e3 * step_s, "subchunk_len": L, "kernel_events_ms": 1e3 * kern_e2e_s,
+                             "overlap_efficiency": max(kern_e2e_s, t_copy) / step_s, "h2d_gbs_in_run": h2d / step_s / 1e9,
+                             "real_time_factor": w.nsamp * w.tsamp / step_s, "candidates": n_cands, "candidates_sha256": e2e_hash}}
+        line["sweep"] = stream_sweep(B, w, host, obuf, [n for n in (1, 2, 4, 8) if w.chunk_len % n == 0], t_copy, known)
+        try:
+            line["paper_path"] = paper_path(B, w, host, x, obuf, e2e_hash)
+        except MemoryError as e:
+            line["paper_path"] = {"skipped": f"MemoryError: {e}"}
+        line["variants"] = search_variants(B, w, host, obuf)
     del host, x
+    if rank == 0 and extras != "none":
+        line["variants"].update(bit_depth_variants(B, w, obuf))
     # ---- the other configs of BASELINE.json, end to end (north_star: "the 4096-channel configs") ----
     pcs = args.per_config
     if pcs == "auto":
@@ -570,7 +759,7 @@ def main():
         line["per_config"] = {}
         for k in [int(v) for v in pcs.split(",") if v]:
             try:
-                line["per_config"][f"cfg{k}"] = run_config(B, k, 3, 1, mb["h2d_gbs"])
+                line["per_config"][f"cfg{k}"] = run_config(B, k, 3, 1, mb["h2d_gbs"], sweep=(1, 2, 4, 8, 16) if k == 5 else ())
             except Exception as e:                      # e.g. not enough host memory to pin 68.7 GB
                 line["per_config"][f"cfg{k}"] = {"error": f"{type(e).__name__}: {e}"}
     if rank == 0:

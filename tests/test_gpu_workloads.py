@@ -192,7 +192,7 @@ def test_cfg1_cfg2_peaks_on_the_device(B):
         assert any(abs(int(top["dm_index"]) - p.dm) <= 2 and abs(int(top["t_start"]) - p.t0) <= 2 * p.width + 2 for p in w.pulses)
 
 
-def _run_sampled(B, w, cells_extra, max_pulses=4, **plan_kw):
+def _run_sampled(B, w, cells_extra, max_pulses=4, also_streams=(), **plan_kw):
     buf, x = _pinned_fill(B, w)
     geo = oracle.geometry(w)
     cells = _pulse_cells(w, geo, max_pulses=max_pulses, extra=cells_extra)
@@ -210,6 +210,13 @@ def _run_sampled(B, w, cells_extra, max_pulses=4, **plan_kw):
         assert not plan.overflow
         assert plan.info["maxshift"] == geo["maxshift"] and plan.nout == geo["nout"]
         stats = plan.stats()
+    for ns in also_streams:                                       # same buffer, other stream counts: identical output
+        kw = dict(plan_kw, n_streams=ns)
+        with B.Plan(w, taps=taps, **kw) as plan:
+            c2, t2 = plan.run(buf, max_cands=1 << 24)
+            assert not plan.overflow and plan.info["n_subchunks"] >= ns
+            assert c2.tobytes() == cands.tobytes() and np.array_equal(t2, tap), f"{ns} streams differ"
+        del c2, t2
     n_cells, n_ref = _check_cells(w, x, cands, tap, tapidx, cells)
     return cands, n_cells, n_ref, stats
 
@@ -242,6 +249,29 @@ def test_cfg5_reduced_length_sampled_16_streams(B):
     assert n_cells >= 5
 
 
+@pytest.mark.parametrize("n_streams", [32, 64])
+def test_cfg3_shape_many_streams_sampled(B, n_streams):
+    """aa.h takes n_streams up to 64: the headline workload's shape with 65536-sample sub-chunks, one per stream, so
+    that every one of the 32 / 64 streams (and host threads) runs a sub-chunk; stratified rows x blocks (first, ragged
+    last, both sides of sub-chunk seams) against the oracle, and the whole list against the 4-stream run's."""
+    w = I.scaled(I.workload(3), nsamp=n_streams << 16, chunk_len=n_streams << 16, n_streams=n_streams,
+                 name=f"cfg3_{n_streams}streams")
+    w = I.scaled(w, pulses=(I.Pulse(dm=300.0, t0=150000, width=16, amp=0.35), I.Pulse(dm=1500.0, t0=(n_streams << 16) // 2, width=128, amp=0.12)))
+    extra, n_rows, blocks = _stratified_cells(w, 1 << 16, n_rows=12, n_seams=3, n_random_blocks=1, max_pulses=2)
+    assert len(blocks) >= 7
+    buf, x = _pinned_fill(B, w)
+    taps, tapidx = _global_rows(w, {0: sorted({d for _, rows, _ in extra for d in rows})})
+    with B.Plan(w, taps=taps, max_cands_per_subchunk=1 << 18) as plan:
+        assert plan.info["n_subchunks"] == n_streams and plan.info["subchunk_len"] == 1 << 16
+        cands, tap = plan.run(buf, max_cands=1 << 22)
+        assert not plan.overflow and plan.stats()["n_streams"] == n_streams
+    n_cells, n_ref = _check_cells(w, x, cands, tap, tapidx, extra)
+    assert n_cells >= 12 * 7 and n_ref > 0
+    with B.Plan(w, taps=taps, n_streams=4, max_cands_per_subchunk=1 << 18) as plan:
+        c4, t4 = plan.run(buf, max_cands=1 << 22)
+    assert c4.tobytes() == cands.tobytes() and np.array_equal(t4, tap)
+
+
 @pytest.mark.parametrize("variant", [dict(nbits=4), dict(nbits=16), dict(sigma_mode=1), dict(wdec=16), dict(sigma_mode=1, wdec=16)],
                          ids=["4bit", "16bit", "measured-sigma", "decimated-widths", "measured-sigma+decimated"])
 def test_cfg3_shape_search_variants_sampled(B, variant):
@@ -270,6 +300,8 @@ def test_cfg5_full_size_sampled(B):
     n_streams = 8
     extra, n_rows, blocks = _stratified_cells(w, w.chunk_len // n_streams, n_seams=2, n_random_blocks=1)
     assert n_rows >= 64 and len(blocks) >= 6
-    cands, n_cells, n_ref, stats = _run_sampled(B, w, extra, max_pulses=8, n_streams=n_streams)
+    # B:configs[4] asks for a stream sweep up to 16: the 16-stream run (65536-sample sub-chunks) must return the
+    # 8-stream run's bytes, which are the ones compared with the oracle
+    cands, n_cells, n_ref, stats = _run_sampled(B, w, extra, max_pulses=8, also_streams=(16,), n_streams=n_streams)
     assert n_cells >= 64 * 6 and n_ref > 0
     assert stats["h2d_bytes"] == w.nbytes
