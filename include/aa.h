@@ -120,9 +120,9 @@ typedef struct {
     /* Reading A18 (per-width measured sigma): 0 = S_w = (B_w - w mu) / (sigma sqrt w), white-noise
      * scaling of the block's statistics (BASELINE.json).  1 = S_w = (B_w - mu_w) / sigma_w with (mu_w, sigma_w) the same
      * robust estimator applied to the boxcar series of width w itself over the normalisation block (on the width's grid);
-     * a width with sigma_w = 0 or fewer than 32 boxcars in the block is skipped.  Needs normalisation blocks the
-     * cluster kernel takes (block / bin a multiple of 4, at most 131072 binned samples, 32-bit boxcar sums):
-     * AA_ERR_INVALID otherwise. */
+     * a width with sigma_w = 0 or fewer than 32 boxcars in the block is skipped.  Accepted on every range: where the
+     * block does not fit the cluster kernel (64-bit boxcar sums, block / bin not a multiple of 4 or above 131072
+     * samples) the generic kernel sweeps the block once per pass of the estimator (slower, same results). */
     int32_t  sigma_mode;
     /* 0 = aa_run returns every candidate (one per (DM, time), reading A11; BASELINE.json).  1 = it returns the PEAKS of
      * that list (reading A17, the rule of aa_find_peaks): each sub-chunk's list is thinned on the device before it

@@ -316,17 +316,9 @@ int build_geometry(aa_plan &p, const aa_plan_desc *d)
         if (R.flush_ch < 2) return AA_ERR_INVALID;
         R.wide = (long double)maxsample * d->nchans * R.r.bin * p.wmax >= 4294967296.0L;
         R.small31 = (long double)maxsample * d->nchans * R.r.bin * p.wmax < 2147483648.0L;
-        if (d->sigma_mode) {
-            // per-width statistics live in the cluster kernel: block of 4 C segments of at most 16384 samples, C <= 8
-            const uint64_t bl = p.norm_block / (uint64_t)R.r.bin;
-            bool fits = !R.wide && !p.big && bl % 4 == 0;
-            if (fits) {
-                fits = false;
-                for (uint64_t C = 1; C <= 8 && bl % (4 * C) == 0; C *= 2)
-                    if (bl / C <= 16384) { fits = true; break; }
-            }
-            if (!fits) return AA_ERR_INVALID;
-        }
+        // sigma_mode 1 (reading A18) runs everywhere: in the cluster kernel where the block fits its shared memory
+        // (32-bit boxcar sums, block a multiple of 4 C with segments of at most 16384 samples), else in the generic
+        // kernel, which sweeps the block once per pass of the estimator (64-bit sums, odd or very long blocks).
         if (R.in16) {
             auto it = std::find(p.bins.begin(), p.bins.end(), R.r.bin);
             if (it == p.bins.end()) { p.bins.push_back(R.r.bin); R.bin_slot = (int)p.bins.size() - 1; }

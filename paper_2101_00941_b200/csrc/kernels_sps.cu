@@ -49,6 +49,11 @@ struct Shared {
     unsigned long long warp_tot[NT / 32];
     int w[kMaxWidths];        // widths (a dynamically indexed kernel parameter would go through the ADU pipe)
     int dec[kMaxWidths];      // time grid of each width (reading A20): 1, or a power of two for widths above wdec
+    // reading A18 (sigma_mode 1): the width's own robust mean and sigma, and the exact sums they are made from
+    double wmu[kMaxWidths], wsg[kMaxWidths];
+    uint64_t wacc[kMaxWidths][NT / 32][4];     // per width and warp: count, sum B, sum B^2 (low 64 bits, high 64 bits)
+    uint64_t wcnt0[kMaxWidths];                // boxcars of the width in the block (first pass)
+    int wdone[kMaxWidths];                     // the width's statistics are final (or it has none)
 };
 
 // BIG: the block's sum of squares may pass 2^64 (16-bit input on thousands of channels): every thread keeps its part
@@ -121,24 +126,16 @@ __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const __grid_c
     }
     if (!(sigma > 0.0) || n_k < 32) return;
 
-    // ---- 2. per-width constants ---------------------------------------------------------
-    if (tid < a.nwidths) {
-        const double w = (double)sh.w[tid];
-        const double den = __dmul_rn(sigma, __dsqrt_rn(w));
-        sh.den[tid] = den;
-        sh.bthr[tid] = __double2ll_rd(w * mu + a.thr * den) - 1;
-    }
-    __syncthreads();
-
     const int64_t e = b1 < a.nemit ? b1 : (int64_t)a.nemit;     // taus [b0, e) may emit
     const int64_t navail = a.ncols < a.nout_left ? (int64_t)a.ncols : a.nout_left;
     const int halo = a.wmax - 1;
     const int ept = (TT + halo + 1 + NT - 1) / NT;              // scan slots per thread (covers P[0..TT+halo])
+    const bool measured = a.sigma_mode != 0;                    // reading A18
 
-    for (int64_t ts = b0; ts < e; ts += TT) {
+    // block-wide exclusive prefix sum of row[ts .. ts+n_in) into P[0 .. n_in]; returns n_in
+    auto build_prefix = [&](int64_t ts) -> int64_t {
         int64_t n_in = navail - ts;
         if (n_in > TT + halo) n_in = TT + halo;
-        // block-wide exclusive prefix sum of row[ts .. ts+n_in) into P[0 .. n_in]
         {
             const int64_t i0 = (int64_t)tid * ept;
             ACC run = 0;
@@ -164,6 +161,99 @@ __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const __grid_c
             }
             __syncthreads();
         }
+        return n_in;
+    };
+
+    // ---- 2a. reading A18: robust statistics of every width's own boxcar series over the block ----------------------
+    // The series of width w is B_w[t] for the t of the block on the width's grid (A20) with t + w <= nout.  The block does
+    // not fit shared memory here (64-bit sums, or a block no cluster takes), so each of the four passes of the estimator
+    // sweeps the block tile by tile through the same prefix sums as the search and adds up the exact integers
+    // (count, sum B, sum B^2 in 128 bits) of all widths at once; mu_w, sigma_w are formed as for the block itself.
+    if (measured) {
+        if (tid < kMaxWidths) {
+            sh.wmu[tid] = 0.0; sh.wsg[tid] = 0.0; sh.wcnt0[tid] = 0;
+            sh.wdone[tid] = tid < a.nwidths ? 0 : 1;
+        }
+        __syncthreads();
+        for (int pass = 0; pass < 4; ++pass) {
+            for (int i = tid; i < kMaxWidths * (NT / 32) * 4; i += NT) (&sh.wacc[0][0][0])[i] = 0;
+            bool open = false;
+            for (int j = 0; j < a.nwidths; ++j) open |= !sh.wdone[j];
+            __syncthreads();
+            if (!open) break;                                   // uniform
+            for (int64_t ts = b0; ts < b1; ts += TT) {
+                const int64_t n_in = build_prefix(ts);
+                for (int j = 0; j < a.nwidths; ++j) {
+                    if (sh.wdone[j]) continue;                  // uniform
+                    const int w = sh.w[j];
+                    const uint32_t gm = (uint32_t)(sh.dec[j] - 1);
+                    const double wm = sh.wmu[j], lim = __dmul_rn(3.0, sh.wsg[j]);
+                    uint64_t m = 0, S1 = 0;
+                    unsigned __int128 S2 = 0;
+                    for (int q = 0; q < TT / NT; ++q) {
+                        const int tl = q * NT + tid;
+                        const int64_t tau = ts + tl;
+                        if (tau < b1 && tau + w <= a.nout_left && tl + w <= n_in && ((a.tau0 + (uint32_t)tau) & gm) == 0) {
+                            const uint64_t B = (uint64_t)(ACC)(P[tl + w] - P[tl]);
+                            if (pass == 0 || fabs(__dsub_rn((double)B, wm)) <= lim) {
+                                m += 1;
+                                S1 += B;
+                                S2 += (unsigned __int128)B * B;
+                            }
+                        }
+                    }
+                    m = warp_sum(m); S1 = warp_sum(S1);
+                    const uint64_t lo = (uint64_t)S2;
+                    const uint64_t l0 = warp_sum(lo & 0xFFFFFFFFull), l1 = warp_sum(lo >> 32), hi = warp_sum((uint64_t)(S2 >> 64));
+                    if (lane == 0) {
+                        uint64_t *acc = sh.wacc[j][warp];
+                        const unsigned __int128 cur = ((unsigned __int128)acc[3] << 64 | acc[2]) + (unsigned __int128)l0 +
+                                                      ((unsigned __int128)l1 << 32) + ((unsigned __int128)hi << 64);
+                        acc[0] += m; acc[1] += S1; acc[2] = (uint64_t)cur; acc[3] = (uint64_t)(cur >> 64);
+                    }
+                }
+                __syncthreads();                                // the next tile overwrites P
+            }
+            if (tid < a.nwidths && !sh.wdone[tid]) {
+                uint64_t m = 0, S1 = 0;
+                unsigned __int128 S2 = 0;
+                for (int wp = 0; wp < NT / 32; ++wp) {
+                    m += sh.wacc[tid][wp][0]; S1 += sh.wacc[tid][wp][1];
+                    S2 += ((unsigned __int128)sh.wacc[tid][wp][3] << 64) | sh.wacc[tid][wp][2];
+                }
+                if (pass == 0) sh.wcnt0[tid] = m;
+                if (m == 0 || sh.wcnt0[tid] < 32) {
+                    sh.wdone[tid] = 1;                          // fewer than 32 boxcars: no statistics; an empty clip keeps the last ones
+                } else {
+                    const unsigned __int128 N = (unsigned __int128)m * S2 - (unsigned __int128)S1 * S1;
+                    const double dm = __ull2double_rn(m);
+                    sh.wmu[tid] = __ddiv_rn(__ull2double_rn(S1), dm);
+                    sh.wsg[tid] = __dsqrt_rn(__ddiv_rn(u128_to_double(N), __dmul_rn(dm, dm)));
+                }
+            }
+            __syncthreads();
+        }
+    }
+
+    // ---- 2. per-width constants ---------------------------------------------------------
+    if (tid < a.nwidths) {
+        if (measured) {
+            const double sg = sh.wcnt0[tid] >= 32 ? sh.wsg[tid] : 0.0;
+            const bool ok = sg > 0.0;
+            sh.den[tid] = ok ? sg : 0.0;
+            // B >= floor(mu_w + thr sigma_w) - 1 is necessary for S >= thr; a width without statistics never hits
+            sh.bthr[tid] = ok ? __double2ll_rd(sh.wmu[tid] + a.thr * sg) - 1 : 0x7FFFFFFFFFFFFFFFll;
+        } else {
+            const double w = (double)sh.w[tid];
+            const double den = __dmul_rn(sigma, __dsqrt_rn(w));
+            sh.den[tid] = den;
+            sh.bthr[tid] = __double2ll_rd(w * mu + a.thr * den) - 1;
+        }
+    }
+    __syncthreads();
+
+    for (int64_t ts = b0; ts < e; ts += TT) {
+        build_prefix(ts);
         // boxcars
         for (int q = 0; q < TT / NT; ++q) {
             const int tl = q * NT + tid;                 // tau within the tile
@@ -187,8 +277,14 @@ __global__ void __launch_bounds__(NT) sps_kernel(const SpsArgs a, const __grid_c
                         const int w = sh.w[j];
                         if (tau + w > a.nout_left || (tabs & (uint32_t)(sh.dec[j] - 1)) != 0) continue;
                         const long long B = (long long)(ACC)(P[tl + w] - p0);
-                        const double num = __dsub_rn((double)B, __dmul_rn((double)w, mu));
-                        const double S = __ddiv_rn(num, sh.den[j]);
+                        double S;
+                        if (measured) {
+                            const double sg = sh.den[j];
+                            if (!(sg > 0.0)) continue;
+                            S = __ddiv_rn(__dsub_rn((double)B, sh.wmu[j]), sg);
+                        } else {
+                            S = __ddiv_rn(__dsub_rn((double)B, __dmul_rn((double)w, mu)), sh.den[j]);
+                        }
                         if (best_w == 0 || S > best) { best = S; best_w = w; }
                     }
                     has = (best_w != 0) && (best >= a.thr);

@@ -254,21 +254,33 @@ def test_other_input_bit_depths(B, nbits, case):
     dict(sigma_mode=1, wdec=4, norm_block=131072, chunk_len=131072, nsamp=300000, ndms=4, widths=(1, 3, 8, 64)),        # cluster of 8
     dict(sigma_mode=1, bins=(1, 2, 4), nsamp=40000, chunk_len=8192, n_streams=2),
     dict(sigma_mode=1, nchans=302, ndms=100, nsamp=21000, chunk_len=8192, foff=-0.5, dm_step=0.25, norm_block=1024, n_streams=2),
+    # A18 outside the cluster kernel: per-width statistics swept tile by tile in the generic kernel
+    dict(sigma_mode=1, bins=(8,), norm_block=1040, chunk_len=8 * 1040, nsamp=50000, ndms=12, widths=(1, 4, 16, 32)),     # block of 130 samples: no cluster
+    dict(sigma_mode=1, wdec=4, bins=(8,), norm_block=1040, chunk_len=8 * 1040, nsamp=50000, ndms=12, widths=(1, 4, 16, 32, 64)),
+    dict(sigma_mode=1, bins=(8,), norm_block=20816, chunk_len=41632, nsamp=150000, ndms=6, widths=(1, 2, 3, 8, 100)),   # block of 2602 samples: two tiles per block, ragged
+    dict(sigma_mode=1, nbits=16, nchans=300, nsamp=12000, foff=-0.3, dm_step=4.0, chunk_len=4096, norm_block=2048, widths=(1, 2, 4, 8, 256), thr=4.0),   # 64-bit boxcar sums
+    dict(sigma_mode=1, wdec=2, nbits=16, nchans=1024, ndms=40, nsamp=30000, chunk_len=8192, foff=-0.2, dm_step=0.25, norm_block=4096, widths=(1, 2, 4, 64)),  # 128-bit block statistics too
+    dict(sigma_mode=1, norm_block=2048, chunk_len=4096, nsamp=4096 * 3 + 40, widths=(1, 2, 4, 8, 64)),                  # last block shorter than 32 + w: widths without statistics
 ])
 def test_search_variants_a18_a20(B, case):
     """Readings A20 (long boxcars on a coarser time grid) and A18 (S/N from each width's own statistics) against the
     oracle: dense plane bit for bit, candidates under the north_star tolerances."""
     case = dict(case)
-    wdec, sm = case.pop("wdec", 0), case.pop("sigma_mode", 0)
-    w = I.scaled(_tiny(**case), wdec=wdec, sigma_mode=sm)
+    wdec, sm, nbits = case.pop("wdec", 0), case.pop("sigma_mode", 0), case.pop("nbits", 8)
+    w = I.scaled(_tiny(**case), wdec=wdec, sigma_mode=sm, nbits=nbits)
     cands, ref, res = _check_against_oracle(B, w)
     assert res["only_gpu"] == 0 and res["only_oracle"] == 0 and res["width_ties"] == 0
     assert len(ref) > 0
 
 
-def test_measured_sigma_needs_cluster_sized_blocks(B):
-    with pytest.raises(B.AAError):
-        B.Plan(I.scaled(_tiny(bins=(8,), norm_block=1040, chunk_len=8 * 1040, nsamp=50000), sigma_mode=1))   # block of 130 samples
+def test_measured_sigma_is_accepted_on_every_range(B):
+    """Round 2 refused sigma_mode 1 where the cluster kernel does not serve (64-bit boxcar sums, blocks it cannot split):
+    cfg4 and 16-bit cfg3 could not run reading A18 at all.  Every such plan is accepted now (no GPU work here: geometry only);
+    the results are compared with the oracle in test_search_variants_a18_a20 and the sampled cfg3 / cfg4 tests."""
+    assert B.plan_geometry(I.scaled(I.workload(4), sigma_mode=1))["ndms_total"] == I.workload(4).ndms_total
+    assert B.plan_geometry(I.scaled(I.workload(3), nbits=16, sigma_mode=1))["ndms_total"] == 2048
+    with B.Plan(I.scaled(_tiny(bins=(8,), norm_block=1040, chunk_len=8 * 1040, nsamp=50000), sigma_mode=1)) as plan:   # block of 130 samples
+        assert plan.info["n_subchunks"] >= 1
 
 
 @pytest.mark.parametrize("case", [

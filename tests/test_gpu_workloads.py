@@ -242,6 +242,18 @@ def test_cfg4_reduced_length_sampled(B):
     assert n_cells >= 36 and n_ref > 0
 
 
+def test_cfg4_shape_measured_sigma_sampled(B):
+    """Reading A18 on the multi-range plan (B:configs[3]): ranges 0-4 keep per-width statistics in the cluster kernel, range 5
+    (bin 32: 255 * 4096 * 32 * 256 >= 2^32, 64-bit boxcar sums) in the generic kernel; sampled rows x blocks of every range
+    against the oracle."""
+    w = I.scaled(I.workload(4), nsamp=1 << 19, chunk_len=1 << 18, n_streams=4, name="cfg4_short_a18", sigma_mode=1)
+    w = I.scaled(w, pulses=(I.Pulse(dm=100.0, t0=70000, width=8, amp=0.3), I.Pulse(dm=700.4, t0=200000, width=64, amp=0.1),
+                            I.Pulse(dm=2000.0, t0=300000, width=256, amp=0.05)))
+    extra = [(r, [0, w.ranges[r].ndms // 2, w.ranges[r].ndms - 1], k) for r in range(6) for k in (0, 6)]
+    cands, n_cells, n_ref, _ = _run_sampled(B, w, extra)
+    assert n_cells >= 36 and n_ref > 0
+
+
 def test_cfg5_reduced_length_sampled_16_streams(B):
     w = I.scaled(I.workload(5), nsamp=1 << 21, chunk_len=1 << 20, n_streams=16, name="cfg5_short")
     extra = [(0, [0, 2047], 0), (0, [1000], 17), (0, [1, 2046], 31)]
@@ -272,8 +284,9 @@ def test_cfg3_shape_many_streams_sampled(B, n_streams):
     assert c4.tobytes() == cands.tobytes() and np.array_equal(t4, tap)
 
 
-@pytest.mark.parametrize("variant", [dict(nbits=4), dict(nbits=16), dict(sigma_mode=1), dict(wdec=16), dict(sigma_mode=1, wdec=16)],
-                         ids=["4bit", "16bit", "measured-sigma", "decimated-widths", "measured-sigma+decimated"])
+@pytest.mark.parametrize("variant", [dict(nbits=4), dict(nbits=16), dict(sigma_mode=1), dict(wdec=16), dict(sigma_mode=1, wdec=16),
+                                     dict(nbits=16, sigma_mode=1)],
+                         ids=["4bit", "16bit", "measured-sigma", "decimated-widths", "measured-sigma+decimated", "16bit+measured-sigma"])
 def test_cfg3_shape_search_variants_sampled(B, variant):
     """The S:8(f) rows (readings A18-A20) on the headline workload's shape: 4096 channels, 2048 trials, 131072-sample
     sub-chunks on 4 streams, the kernels bench.py times plus the ones these variants select (per-width statistics and
